@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py -- photons/s of the per-photon optical propagation hot path on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config C2] [--photons n]
+
+One "step" = one opx_propagate call (propagation kernel + hit binning + counters) over one batch of
+synthetic photons of the named BASELINE.json config (default C2 = configs[1]: toy RICH, 20 014
+triangles, 1e7 photons), inputs resident in HBM.  The BVH build is timed separately (`bvh_build_ms`)
+as SURVEY.md 8(d) prescribes.  N > 1 (torchrun): every rank propagates its own contiguous id range
+of the same size (weak scaling) and the per-rank hit-maps and counters are summed with one NCCL
+all-reduce per step.  Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "optical photons propagated/sec on 1 B200 (device-timed), % of roofline"
+UNIT = "photons/s"
+# FLOP model of SURVEY.md 8(d) / DESIGN.md 9: FMA = 2, add/mul/min/max/compare/divide = 1
+FLOP_NODE, FLOP_TRI, FLOP_SEGMENT, FLOP_INTERACTION = 48, 50, 15, 35
+BYTES_IN, BYTES_OUT, BYTES_BIN = 28, 34, 6          # per photon: inputs, hit record, re-read by k_bin
+# dram__bytes_read.sum + dram__bytes_write.sum of k_propagate per launch from the ncu --set full
+# capture summarised in profiles/ (None until one exists for the current kernel)
+NCU_TRAFFIC_BYTES = {"C2": None}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.proc = index, [], None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([x.strip() for x in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+        self.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        reasons = sorted({names[k] for r in self.rows if len(r) >= 7 for k in range(4) if r[3 + k].startswith("Active")})
+        return dict(sm_mhz=statistics.median(sm) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=reasons, samples=len(sm))
+
+
+def time_oracle(workload, n_sample, seed, repeats=1):
+    """The oracle as it stands on the host cores, on the first n_sample photon ids of the workload."""
+    import oracle
+    o, d, lam = workload.photon_range(0, n_sample)
+    best = None
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        r = oracle.trace_mesh(workload.scene, o, d, lam, seed=seed)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return n_sample / best, r["n_threads"], best, int(r["counters"][7])
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle timed on a bounded sample of the same workload per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import workloads
+    w = workloads.make_config(args.config, n=args.photons)
+    n_sample = min(w.n, args.reference_sample)
+    import oracle
+    o, d, lam = w.photon_range(0, n_sample)
+    for _ in range(args.warmup):
+        oracle.trace_mesh(w.scene, o[:2000], d[:2000], lam[:2000], seed=args.seed)
+    t0 = time.perf_counter()
+    threads = 0
+    for _ in range(args.steps):
+        r = oracle.trace_mesh(w.scene, o, d, lam, seed=args.seed)
+        threads = r["n_threads"]
+    dt = time.perf_counter() - t0
+    value = n_sample * args.steps / dt
+    sample = f"first {n_sample} photon ids of {args.config} per step, brute force over {w.scene.n_triangles} triangles"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{args.config}: {w.scene.n_triangles} triangles, {w.n} photons (sampled)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="opx", choices=["opx", "reference"])
+    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--photons", type=int, default=None, help="photons per GPU per step (default: the config's N)")
+    ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--cpu-sample", type=int, default=60000, help="photons of the cpu_baseline sample")
+    ap.add_argument("--reference-sample", type=int, default=20000)
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "opx" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2309_12496_b200 as pkg
+    import workloads
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = workloads.make_config(args.config, n=None)
+    n = args.photons if args.photons else min(w.n, 100_000_000)       # per GPU per step
+    if args.photons:
+        w = workloads.make_config(args.config, n=max(w.n, args.photons * world))
+    id_base = rank * n if (rank + 1) * n <= w.n else 0
+    o, d, lam = w.photon_range(id_base, id_base + n)
+    pin = [torch.from_numpy(x).pin_memory() for x in (o, d, lam)]
+    d_o, d_d, d_l = (x.to(dev, non_blocking=True) for x in pin)
+    stream = torch.cuda.current_stream(dev)
+
+    # ---- scene + BVH build (timed separately: SURVEY.md 8(d))
+    scene = pkg.Scene(w.scene)
+    scene.build(dev)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = pkg.launch_count()
+    torch.cuda.synchronize()
+    t_build = []
+    for _ in range(3):
+        t0 = time.perf_counter()
+        scene.build(dev)
+        t_build.append(1e3 * (time.perf_counter() - t0))
+    build_launches = (pkg.launch_count() - l0) // 3
+
+    records = scene.alloc_records(n, dev)
+    hitmap, counters = scene.alloc_accumulators(dev)
+
+    def step():
+        hitmap.zero_(); counters.zero_()
+        scene.propagate(d_o, d_d, d_l, seed=args.seed, photon_id_base=id_base, records=records, hitmap=hitmap,
+                        counters=counters, stream=stream)
+        if dist is not None:
+            dist.all_reduce(hitmap); dist.all_reduce(counters)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    scene.profile_begin(args.steps)
+    l0 = pkg.launch_count()
+    torch.cuda.synchronize()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    launches = pkg.launch_count() - l0                           # kernels of libopx.so only (torch fills not counted)
+    ms_prop, ms_bin = scene.profile_end()
+    clocks = sampler.stop()
+    if dist is not None:
+        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * n * args.steps / (ms_total * 1e-3)
+    cnt = counters.cpu().numpy()
+
+    # ---- end to end through the C ABI with host buffers (copies inside the timed region)
+    e2e = None
+    if rank == 0 or dist is not None:
+        host_out = pkg.alloc_host_records(n, scene.n_pixels)
+        chunk = min(n, 1 << 21)
+        scene.propagate_host(*pin, seed=args.seed, photon_id_base=id_base, chunk=chunk, out=host_out, stream=stream)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            host_out["hitmap"].zero_(); host_out["counters"].zero_()
+            scene.propagate_host(*pin, seed=args.seed, photon_id_base=id_base, chunk=chunk, out=host_out, stream=stream)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * n * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": BYTES_IN * n,
+               "d2h_bytes_per_step": BYTES_OUT * n + 4 * scene.n_pixels + 64, "chunk_photons": chunk,
+               "ms_per_step": 1e3 * dt / args.e2e_steps}
+        if not np.array_equal(host_out["counters"].numpy(), cnt if dist is None else host_out["counters"].numpy()):
+            raise SystemExit("bench: host path and device path disagree")
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (k_propagate), DESIGN.md section 9
+    peaks = measured_peaks()
+    stats = scene.propagate_stats(d_o, d_d, d_l, seed=args.seed, photon_id_base=id_base)
+    flop = (FLOP_NODE * stats["nodes"] + FLOP_TRI * stats["triangle_tests"] + FLOP_SEGMENT * stats["segments"]
+            + FLOP_INTERACTION * stats["interactions"])
+    t_prop = statistics.mean(ms_prop) * 1e-3
+    t_bin = statistics.mean(ms_bin) * 1e-3
+    fp32_peak_tflops = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    alu_achieved = flop / t_prop / 1e12
+    hbm_bytes = (BYTES_IN + BYTES_OUT) * n
+    hbm_achieved = hbm_bytes / t_prop / 1e9
+    t_alu_bound, t_hbm_bound = flop / (fp32_peak_tflops * 1e12), hbm_bytes / (peaks["hbm_gbs"] * 1e9)
+    if t_alu_bound >= t_hbm_bound:
+        roof = {"bound": "alu", "achieved": alu_achieved, "peak": fp32_peak_tflops, "unit": "TFLOP/s",
+                "frac": alu_achieved / fp32_peak_tflops}
+    else:
+        roof = {"bound": "hbm", "achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": hbm_achieved / peaks["hbm_gbs"]}
+    roof.update({
+        "traffic": NCU_TRAFFIC_BYTES.get(args.config), "kernel": "k_propagate", "kernel_ms": 1e3 * t_prop,
+        "kernel_share_of_step": t_prop / (ms_step * 1e-3), "bin_kernel_ms": 1e3 * t_bin, "peak_source": peaks["source"],
+        "peak_derivation": "148 SMs x 128 FP32 lanes x 2 FLOP x sm_max_mhz",
+        "flop_per_photon": flop / n, "bytes_per_photon": BYTES_IN + BYTES_OUT,
+        "segments_per_photon": stats["segments"] / n, "nodes_per_segment": stats["nodes"] / max(1, stats["segments"]),
+        "triangle_tests_per_segment": stats["triangle_tests"] / max(1, stats["segments"]),
+        "alu_tflops": alu_achieved, "alu_frac": alu_achieved / fp32_peak_tflops,
+        "hbm_gbs": hbm_achieved, "hbm_frac": hbm_achieved / peaks["hbm_gbs"],
+        "photons_per_s_alu_bound": n / t_alu_bound, "photons_per_s_hbm_bound": n / t_hbm_bound})
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        n_sample = min(n, args.cpu_sample)
+        v, threads, secs, segs = time_oracle(w, n_sample, args.seed)
+        cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"first {n_sample} photon ids of {args.config}, brute force over {w.scene.n_triangles} triangles, {secs:.1f} s",
+               "ray_triangle_tests_per_s": segs * w.scene.n_triangles / secs}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": f"{args.config}: {w.scene.n_triangles} triangles, {n} photons per GPU per step "
+                               f"({BYTES_IN + BYTES_OUT} B/photon = {(BYTES_IN + BYTES_OUT) * n / 1e6:.0f} MB per step)",
+                   "l2": "inputs + outputs per step exceed the 126 MB L2" if (BYTES_IN + BYTES_OUT) * n > 126e6 else "fits in L2",
+                   "photons_per_gpu": n, "triangles": w.scene.n_triangles, "pixels": scene.n_pixels, "seed": args.seed,
+                   "id_partition": "contiguous global photon-id range per rank; scene + BVH replicated"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
+        "bvh_build_ms": min(t_build), "bvh_build_launches": int(build_launches),
+        "states": dict(zip(pkg.STATE_NAMES, (int(x) for x in cnt[:7]))),
+        "context_paper": "paper: 1.2e6 photons/s per Tesla T4 and 2e5 per Xeon thread, end to end (PAPER.md:9); other hardware, not the target",
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

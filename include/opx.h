@@ -1,0 +1,221 @@
+/* opx.h -- C ABI of libopx.so: per-photon optical propagation on one B200 (sm_100a).
+ *
+ * The calls follow the paper's statement of the problem (arXiv:2309.12496; line numbers are
+ * /root/reference/PAPER.md):
+ *   - geometry  = triangle meshes grouped per material;
+ *   - materials = per-material efficiency-vs-wavelength tables: mirror reflectivity, detector
+ *                 quantum efficiency, applied in flight per interaction as the
+ *                 paper proposes;
+ *   - input     = "a vector input of initial positions and momenta", one ray per
+ *                 entry, here as origins, unit directions and wavelengths;
+ *   - output    = the global hit position of every photon and its 2-D detector
+ *                 pixel from the corner point A along two in-plane unit vectors,
+ *                 plus the pixel hit-map that replaces the paper's film/bitmap.
+ * What each call computes, step by step and operation by operation, is DESIGN.md sections 2 and 3.
+ *
+ * Conventions
+ *   Units: mm, nm.  All floating point data is IEEE binary32.
+ *   Ownership: the CALLER owns every device byte (photon arrays, hit records, hit-map, counters,
+ *     scene and build workspaces).  The library never allocates or frees device memory.  Host
+ *     pointers passed to opx_scene_create are read during that call only.  An opx_scene is host
+ *     memory owned by the library until opx_scene_destroy.
+ *   Streams: `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls
+ *     enqueue work and return without synchronising unless stated; an asynchronous CUDA failure is
+ *     reported by the next call as OPX_ERR_CUDA.
+ *   Errors: every entry point returns opx_status; nothing throws across the boundary.
+ *     opx_last_error() gives a thread-local message for the last non-OK status.
+ *   Device: requires compute capability 10.x (B200); anything else => OPX_ERR_UNSUPPORTED_DEVICE.
+ *   Threading: a built scene is immutable; concurrent opx_propagate calls on different streams
+ *     are allowed.
+ */
+#ifndef OPX_H_
+#define OPX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct opx_scene opx_scene; /* opaque, host side */
+
+typedef enum {
+    OPX_OK = 0,
+    OPX_ERR_INVALID_ARG = 1,
+    OPX_ERR_BAD_STATE = 2,           /* e.g. propagate before bvh_build */
+    OPX_ERR_WORKSPACE_TOO_SMALL = 3,
+    OPX_ERR_CUDA = 4,
+    OPX_ERR_UNSUPPORTED_DEVICE = 5
+} opx_status;
+
+typedef enum { OPX_MAT_ABSORBER = 0, OPX_MAT_MIRROR = 1, OPX_MAT_DETECTOR = 2 } opx_mat_kind;
+
+/* Terminal state of a photon. */
+typedef enum {
+    OPX_DETECTED = 0,         /* reached a detector pixel and passed the QE draw              */
+    OPX_QE_REJECTED = 1,      /* reached a detector pixel, failed the QE draw                 */
+    OPX_ABSORBED_SURFACE = 2, /* hit an absorber                                              */
+    OPX_ABSORBED_MIRROR = 3,  /* hit a mirror, failed the reflectivity draw                   */
+    OPX_DETECTOR_DEAD = 4,    /* hit a detector surface outside its pixel grid                */
+    OPX_BOUNCE_LIMIT = 5,     /* reflected max_bounces times                                  */
+    OPX_ESCAPED = 6           /* no surface along the segment (also NaN / zero directions)    */
+} opx_state;
+
+typedef struct {
+    float lambda_min_nm, lambda_max_nm; /* uniform wavelength grid of every table, max > min  */
+    uint32_t n_lambda;                  /* points per table, >= 2                             */
+    uint32_t max_bounces;               /* reflections before OPX_BOUNCE_LIMIT (16), 1..255   */
+    float t_min_mm;                     /* minimum hit distance after a bounce (1e-3), >= 0   */
+} opx_scene_params;
+
+typedef struct {
+    uint32_t kind;      /* opx_mat_kind                                                        */
+    const float* table; /* HOST, n_lambda values in [0,1]: reflectivity (mirror) or QE         */
+                        /* (detector); ignored (may be NULL) for an absorber                   */
+} opx_material;
+
+/* Detector pixel grid: a point p maps to a = (p-A).u, b = (p-A).v,
+ * iu = floor(a / pitch_u), iv = floor(b / pitch_v); inside iff 0 <= iu < nu and 0 <= iv < nv;
+ * pixel id = pixel_base + iv*nu + iu. */
+typedef struct {
+    float A[3], u[3], v[3]; /* corner point and the two in-plane unit vectors                  */
+    float pitch_u, pitch_v; /* > 0                                                             */
+    uint32_t nu, nv, pixel_base;
+} opx_pixel_frame;
+
+/* One surface = one mesh.  Surface id = index in the `meshes` array; global triangle id = triangles
+ * of mesh 0 in order, then mesh 1, ... (used for tie-breaks and for `last triangle` skipping). */
+typedef struct {
+    const float* vertices;   /* HOST, n_vertices x 3, xyz packed                               */
+    uint32_t n_vertices;
+    const uint32_t* indices; /* HOST, n_triangles x 3, each < n_vertices                       */
+    uint32_t n_triangles;
+    uint32_t material;       /* index into `materials`                                         */
+    int32_t pixel_frame;     /* index into `frames`; required (>= 0) iff the material is a     */
+                             /* detector, ignored otherwise                                    */
+} opx_mesh;
+
+/* Per-photon hit records, DEVICE pointers, each of length n (pos, dir: n x 3 packed).
+ *   pos     hit point of the last interaction (ESCAPED: origin of the last segment)
+ *   dir     direction of arrival (BOUNCE_LIMIT: the reflected direction)
+ *   pixel   detector pixel id, -1 unless state is DETECTED or QE_REJECTED
+ *   surface surface id of the last hit, -1 for ESCAPED
+ *   state   opx_state;  bounces = number of mirror reflections performed */
+typedef struct {
+    float* pos;
+    float* dir;
+    int32_t* pixel;
+    int32_t* surface;
+    uint8_t* state;
+    uint8_t* bounces;
+} opx_hits;
+
+/* Byte offsets of the arrays opx_bvh_build leaves in the scene workspace (for tests that check
+ * the BVH invariants; DESIGN.md section 8 gives the element layouts). */
+typedef struct {
+    uint64_t nodes;       /* (n_nodes) x 64 B                                                   */
+    uint64_t triangles;   /* (n_triangles) x 48 B, leaf order                                   */
+    uint64_t normals;     /* (n_triangles) x 16 B, leaf order: n.xyz, surface id bits           */
+    uint64_t surfaces;    /* (n_surfaces) x 8 B: material, frame                                */
+    uint64_t mat_kinds;   /* (n_materials) x 4 B                                                */
+    uint64_t tables;      /* (n_materials) x n_lambda x 4 B                                     */
+    uint64_t frames;      /* (n_frames) x 64 B                                                  */
+    uint64_t sorted_keys; /* (n_triangles) x 8 B Morton keys in leaf order (kept for checking)  */
+    uint64_t parents;     /* (2 n_triangles - 1) x 4 B: parent of internal node i / leaf T-1+i  */
+    uint64_t total_bytes;
+} opx_scene_layout;
+
+/* A0.  Validates and flattens the meshes into one global triangle list, computes the face normals
+ * and copies tables and frames.  Host only; no CUDA call.
+ * Errors: NULL pointers, n_lambda < 2, lambda_max <= lambda_min, max_bounces outside 1..255,
+ * negative t_min, material / frame / vertex index out of range, detector mesh without a frame,
+ * non-positive pitch, zero-sized pixel grid, table value outside [0,1] or NaN, more than 2^30
+ * triangles => OPX_ERR_INVALID_ARG.  n_meshes = 0 (an empty scene) is valid. */
+opx_status opx_scene_create(const opx_scene_params* params, const opx_mesh* meshes, uint32_t n_meshes,
+                            const opx_material* materials, uint32_t n_materials,
+                            const opx_pixel_frame* frames, uint32_t n_frames, opx_scene** out);
+
+/* Sizes of the two device workspaces opx_bvh_build needs: `scene_bytes` must stay alive and
+ * untouched for as long as the scene is used; `build_tmp_bytes` may be released once the stream has
+ * passed the build. */
+opx_status opx_scene_workspace_bytes(const opx_scene* scene, size_t* scene_bytes, size_t* build_tmp_bytes);
+
+/* A1-A4.  GPU LBVH build into the caller's workspaces (both 256-byte aligned device pointers):
+ * scene AABB + 63-bit Morton keys of the triangle AABB centres, LSD radix sort, Karras hierarchy,
+ * padded bottom-up refit, packing into 64-byte nodes and leaf-ordered triangles.  Uploads the
+ * flattened scene first (the host->device copies of pageable memory make this call synchronous with
+ * respect to the host up to the last upload).  May be called again to rebuild.
+ * Errors: OPX_ERR_WORKSPACE_TOO_SMALL, OPX_ERR_INVALID_ARG (NULL / misaligned),
+ * OPX_ERR_UNSUPPORTED_DEVICE, OPX_ERR_CUDA. */
+opx_status opx_bvh_build(opx_scene* scene, void* d_scene_ws, size_t scene_bytes,
+                         void* d_tmp_ws, size_t tmp_bytes, void* cuda_stream);
+
+/* A5-A12.  Propagates n photons (DEVICE pointers): origins and dirs n x 3 packed, wavelengths n, in
+ * nm.  Directions must be unit length; they are NOT renormalised.  Global photon id = photon_id_base
+ * + i keys the random stream (seed, id, bounce), so any chunking gives identical per-id results.
+ * Writes the hit records, ADDS detected photons to d_hitmap (n_pixels uint32) and ADDS to
+ * d_counters (8 uint64: one per opx_state 0..6, [7] = closest-hit queries); the caller zeroes both.
+ * d_hitmap may be NULL only if the scene has no pixels; d_counters may be NULL.  n = 0 is a no-op.
+ * Errors: OPX_ERR_BAD_STATE before opx_bvh_build; OPX_ERR_INVALID_ARG for NULL / misaligned
+ * (4-byte) pointers; OPX_ERR_CUDA. */
+opx_status opx_propagate(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,
+                         const float* d_origins, const float* d_dirs, const float* d_wavelengths,
+                         uint64_t seed, const opx_hits* out, uint32_t* d_hitmap, uint64_t* d_counters,
+                         void* cuda_stream);
+
+/* Same computation with the closest hit found by testing EVERY triangle on the GPU (no BVH
+ * traversal).  A debugging aid that separates the arithmetic of DESIGN.md section 3 from the BVH;
+ * O(n x triangles), never timed. */
+opx_status opx_propagate_brute(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,
+                               const float* d_origins, const float* d_dirs, const float* d_wavelengths,
+                               uint64_t seed, const opx_hits* out, uint32_t* d_hitmap,
+                               uint64_t* d_counters, void* cuda_stream);
+
+/* Size of the device staging workspace opx_propagate_host needs for chunks of `chunk` photons. */
+opx_status opx_propagate_host_workspace_bytes(const opx_scene* scene, uint64_t chunk, size_t* bytes);
+
+/* End-to-end form with HOST buffers (pinned memory recommended): origins, dirs, wavelengths and the
+ * six record arrays of `out` are host pointers of length n; h_hitmap (n_pixels, +=) and h_counters
+ * (8, +=, may be NULL) are host arrays.  Photons are streamed through the caller's device workspace
+ * in chunks of `chunk` photons, copies of one chunk overlapping the kernels of the other on two
+ * internal-order streams forked from `cuda_stream`.  Synchronises `cuda_stream` before returning. */
+opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,
+                              const float* h_origins, const float* h_dirs, const float* h_wavelengths,
+                              uint64_t seed, const opx_hits* h_out, uint32_t* h_hitmap,
+                              uint64_t* h_counters, void* d_workspace, size_t workspace_bytes,
+                              uint64_t chunk, void* cuda_stream);
+
+/* Per-kernel device times for a roofline report.  After opx_profile_begin(scene, max_calls) every
+ * opx_propagate call on this scene records CUDA events around its two kernels (propagation; binning
+ * + counters) on the call's stream, for at most max_calls calls.  opx_profile_end waits for those
+ * events, writes the per-call durations in milliseconds to ms_propagate / ms_bin (each max_calls
+ * floats, may be NULL), the number of recorded calls to n_calls, and switches recording off.  Not
+ * thread-safe with concurrent opx_propagate calls on the same scene. */
+opx_status opx_profile_begin(opx_scene* scene, uint32_t max_calls);
+opx_status opx_profile_end(opx_scene* scene, float* ms_propagate, float* ms_bin, uint32_t* n_calls);
+
+/* Work counters of the propagation kernel for the roofline model: runs the same
+ * traversal with an instrumented kernel that writes no records and ADDS to d_stats (4 uint64,
+ * DEVICE): [0] segments (closest-hit queries), [1] BVH nodes visited (two child boxes each),
+ * [2] ray/triangle tests, [3] surface interactions.  Never timed. */
+opx_status opx_propagate_stats(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,
+                               const float* d_origins, const float* d_dirs, const float* d_wavelengths,
+                               uint64_t seed, uint64_t* d_stats, void* cuda_stream);
+
+opx_status opx_scene_info(const opx_scene* scene, uint64_t* n_triangles, uint64_t* n_nodes,
+                          uint64_t* n_pixels, uint64_t* n_surfaces);
+opx_status opx_scene_get_layout(const opx_scene* scene, opx_scene_layout* out);
+
+/* Number of kernel launches the library has enqueued in this process (monotonic; for bench.py's
+ * gpu_launches accounting). */
+uint64_t opx_launch_count(void);
+
+void opx_scene_destroy(opx_scene* scene);
+const char* opx_last_error(void); /* thread-local, never NULL */
+const char* opx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OPX_H_ */

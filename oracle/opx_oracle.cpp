@@ -183,7 +183,7 @@ template <typename R> Vec3<R> face_normal(const float* v /*9*/) {
 // ---------------------------------------------------------------------------------- pixel map
 // DESIGN.md 3.6.  2-D detector coordinate relative to the corner A along the in-plane unit vectors
 // ("2D coordinates relative to the bottom left corner", Fig. 4).
-struct Frame {          // mirrors opx_pixel_frame of include/opx.h field by field (plain data)
+struct Frame {          // corner A, in-plane unit vectors u, v, pitches, grid size, first pixel id (plain data)
     float A[3], u[3], v[3], pitch_u, pitch_v;
     uint32_t nu, nv, pixel_base;
 };

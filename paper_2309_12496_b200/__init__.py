@@ -1,0 +1,9 @@
+"""paper_2309_12496_b200 -- B200-native per-photon optical propagation (arXiv:2309.12496).
+
+csrc/   CUDA kernels + the C ABI of include/opx.h  (-> lib/libopx.so, built by build.py)
+opx.py  thin ctypes/torch binding with the same names
+
+Nothing here imports the oracle, and there is no CPU fallback.
+"""
+from .opx import (EXPORTS, LIB_PATH, STATE_NAMES, OpxError, Scene, alloc_host_records,  # noqa: F401
+                  launch_count, load_library)

@@ -1,0 +1,351 @@
+// C-ABI entry points of libopx.so (include/opx.h): argument validation, scene flattening (A0),
+// workspace accounting, error reporting and the host-buffer streaming form of propagate.
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "opx_internal.cuh"
+
+namespace opx {
+
+static thread_local std::string g_last_error;
+static std::atomic<uint64_t> g_launches{0};
+
+opx_status fail(opx_status st, const std::string& msg) {
+    g_last_error = msg;
+    return st;
+}
+
+opx_status check_cuda(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return OPX_OK;
+    return fail(OPX_ERR_CUDA, std::string(what) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")");
+}
+
+void count_launch(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+// n = normalise((b-a) x (c-a)) in fp64, rounded once; zero-area triangle => 0.
+static void face_normal(const float* v, float* out) {
+    const double ux = (double)v[3] - (double)v[0], uy = (double)v[4] - (double)v[1], uz = (double)v[5] - (double)v[2];
+    const double wx = (double)v[6] - (double)v[0], wy = (double)v[7] - (double)v[1], wz = (double)v[8] - (double)v[2];
+    const double cx = uy * wz - uz * wy, cy = uz * wx - ux * wz, cz = ux * wy - uy * wx;
+    const double len = std::sqrt((cx * cx + cy * cy) + cz * cz);
+    if (!(len > 0.0)) { out[0] = out[1] = out[2] = 0.f; return; }
+    out[0] = (float)(cx / len); out[1] = (float)(cy / len); out[2] = (float)(cz / len);
+}
+
+static opx_status device_ok() {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return check_cuda(e, "cudaGetDevice");
+    int major = 0;
+    e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return check_cuda(e, "cudaDeviceGetAttribute");
+    if (major != 10) return fail(OPX_ERR_UNSUPPORTED_DEVICE, "libopx.so is built for sm_100a only (compute capability 10.x)");
+    return OPX_OK;
+}
+
+static bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) != 0; }
+
+}  // namespace opx
+
+using namespace opx;
+
+extern "C" {
+
+const char* opx_last_error(void) { return g_last_error.c_str(); }
+const char* opx_version(void) { return "opx 0.1 (sm_100a)"; }
+uint64_t opx_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+opx_status opx_scene_create(const opx_scene_params* params, const opx_mesh* meshes, uint32_t n_meshes,
+                            const opx_material* materials, uint32_t n_materials,
+                            const opx_pixel_frame* frames, uint32_t n_frames, opx_scene** out) {
+    if (!params || !out) return fail(OPX_ERR_INVALID_ARG, "params/out is NULL");
+    *out = nullptr;
+    if ((n_meshes && !meshes) || (n_materials && !materials) || (n_frames && !frames))
+        return fail(OPX_ERR_INVALID_ARG, "array pointer is NULL with a non-zero count");
+    if (params->n_lambda < 2) return fail(OPX_ERR_INVALID_ARG, "n_lambda must be >= 2");
+    if (!(params->lambda_max_nm > params->lambda_min_nm)) return fail(OPX_ERR_INVALID_ARG, "lambda_max must exceed lambda_min");
+    if (params->max_bounces < 1 || params->max_bounces > 255) return fail(OPX_ERR_INVALID_ARG, "max_bounces must be in 1..255");
+    if (!(params->t_min_mm >= 0.f)) return fail(OPX_ERR_INVALID_ARG, "t_min_mm must be >= 0");
+
+    auto* s = new opx_scene();
+    s->params = *params;
+    s->inv_dlambda = (float)((double)(params->n_lambda - 1) / ((double)params->lambda_max_nm - (double)params->lambda_min_nm));
+    auto bail = [&](const std::string& m) { delete s; return fail(OPX_ERR_INVALID_ARG, m); };
+
+    s->mat_kinds.resize(n_materials);
+    s->tables.assign((size_t)n_materials * params->n_lambda, 0.f);
+    for (uint32_t m = 0; m < n_materials; ++m) {
+        if (materials[m].kind > OPX_MAT_DETECTOR) return bail("material kind out of range");
+        s->mat_kinds[m] = materials[m].kind;
+        if (materials[m].kind == OPX_MAT_ABSORBER) continue;
+        if (!materials[m].table) return bail("mirror/detector material without a table");
+        for (uint32_t j = 0; j < params->n_lambda; ++j) {
+            const float y = materials[m].table[j];
+            if (!(y >= 0.f && y <= 1.f)) return bail("table value outside [0,1]");
+            s->tables[(size_t)m * params->n_lambda + j] = y;
+        }
+    }
+    s->frames.resize(n_frames);
+    for (uint32_t f = 0; f < n_frames; ++f) {
+        const opx_pixel_frame& in = frames[f];
+        if (!(in.pitch_u > 0.f) || !(in.pitch_v > 0.f)) return bail("pixel pitch must be > 0");
+        if (in.nu == 0 || in.nv == 0) return bail("pixel grid must be at least 1x1");
+        const uint64_t end = (uint64_t)in.pixel_base + (uint64_t)in.nu * in.nv;
+        if (end > 0x7fffffffull) return bail("pixel ids must fit in int32");
+        FrameDev& o = s->frames[f];
+        o.Ax = in.A[0]; o.Ay = in.A[1]; o.Az = in.A[2];
+        o.ux = in.u[0]; o.uy = in.u[1]; o.uz = in.u[2];
+        o.vx = in.v[0]; o.vy = in.v[1]; o.vz = in.v[2];
+        o.inv_pitch_u = (float)(1.0 / (double)in.pitch_u);   // rounded once from fp64
+        o.inv_pitch_v = (float)(1.0 / (double)in.pitch_v);
+        o.pad0 = 0.f; o.nu = in.nu; o.nv = in.nv; o.pixel_base = in.pixel_base; o.pad1 = 0;
+        if (end > s->n_pixels) s->n_pixels = end;
+    }
+    uint64_t total = 0;
+    for (uint32_t k = 0; k < n_meshes; ++k) total += meshes[k].n_triangles;
+    if (total > (1ull << 30)) { return bail("too many triangles (limit 2^30)"); }
+    s->tri.reserve(total * 9);
+    s->tri_surface.reserve(total);
+    s->surfaces.resize(n_meshes);
+    for (uint32_t k = 0; k < n_meshes; ++k) {
+        const opx_mesh& m = meshes[k];
+        if (m.material >= n_materials) return bail("mesh material index out of range");
+        const bool det = s->mat_kinds[m.material] == OPX_MAT_DETECTOR;
+        if (det && (m.pixel_frame < 0 || (uint32_t)m.pixel_frame >= n_frames)) return bail("detector mesh needs a valid pixel frame");
+        s->surfaces[k] = make_int2((int)m.material, det ? m.pixel_frame : -1);
+        if (m.n_triangles && (!m.vertices || !m.indices)) return bail("mesh vertices/indices is NULL");
+        for (uint32_t t = 0; t < m.n_triangles; ++t) {
+            for (int c = 0; c < 3; ++c) {
+                const uint32_t vi = m.indices[3 * (size_t)t + c];
+                if (vi >= m.n_vertices) return bail("vertex index out of range");
+                const float* v = m.vertices + 3 * (size_t)vi;
+                s->tri.push_back(v[0]); s->tri.push_back(v[1]); s->tri.push_back(v[2]);
+            }
+            s->tri_surface.push_back((int32_t)k);
+        }
+    }
+    s->normals.resize(total * 3);
+    for (uint64_t t = 0; t < total; ++t) face_normal(&s->tri[9 * t], &s->normals[3 * t]);
+    compute_layout(*s, &s->layout, nullptr);
+    *out = s;
+    return OPX_OK;
+}
+
+opx_status opx_scene_workspace_bytes(const opx_scene* scene, size_t* scene_bytes, size_t* build_tmp_bytes) {
+    if (!scene || !scene_bytes || !build_tmp_bytes) return fail(OPX_ERR_INVALID_ARG, "NULL argument");
+    opx_scene_layout lay;
+    size_t tmp = 0;
+    compute_layout(*scene, &lay, &tmp);
+    *scene_bytes = (size_t)lay.total_bytes;
+    *build_tmp_bytes = tmp;
+    return OPX_OK;
+}
+
+opx_status opx_bvh_build(opx_scene* scene, void* d_scene_ws, size_t scene_bytes, void* d_tmp_ws,
+                         size_t tmp_bytes, void* cuda_stream) {
+    if (!scene || !d_scene_ws || !d_tmp_ws) return fail(OPX_ERR_INVALID_ARG, "NULL argument");
+    if (misaligned(d_scene_ws, 256) || misaligned(d_tmp_ws, 256)) return fail(OPX_ERR_INVALID_ARG, "workspaces must be 256-byte aligned");
+    if (opx_status st = device_ok()) return st;
+    opx_scene_layout lay;
+    size_t tmp = 0;
+    compute_layout(*scene, &lay, &tmp);
+    if (scene_bytes < lay.total_bytes || tmp_bytes < tmp) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_scene_workspace_bytes)");
+    scene->built = false;
+    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_bvh_build")) return st;
+    if (opx_status st = build_bvh(*scene, d_scene_ws, d_tmp_ws, (cudaStream_t)cuda_stream)) return st;
+    scene->d_scene_ws = d_scene_ws;
+    scene->scene_bytes = scene_bytes;
+    scene->built = true;
+    return OPX_OK;
+}
+
+static opx_status propagate_common(const opx_scene* scene, bool brute, uint64_t n, uint64_t base,
+                                   const float* o, const float* d, const float* wl, uint64_t seed,
+                                   const opx_hits* out, uint32_t* hitmap, uint64_t* counters, void* stream) {
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate before opx_bvh_build");
+    if (n == 0) return OPX_OK;
+    if (!o || !d || !wl || !out) return fail(OPX_ERR_INVALID_ARG, "NULL photon/record pointer");
+    if (!out->pos || !out->dir || !out->pixel || !out->surface || !out->state || !out->bounces)
+        return fail(OPX_ERR_INVALID_ARG, "NULL hit-record array");
+    if (!hitmap && scene->n_pixels) return fail(OPX_ERR_INVALID_ARG, "d_hitmap is NULL but the scene has pixels");
+    if (misaligned(o, 4) || misaligned(d, 4) || misaligned(wl, 4) || misaligned(out->pos, 4) || misaligned(out->dir, 4) ||
+        misaligned(out->pixel, 4) || misaligned(out->surface, 4) || misaligned(hitmap, 4) || misaligned(counters, 8))
+        return fail(OPX_ERR_INVALID_ARG, "misaligned pointer");
+    if (n > (1ull << 40)) return fail(OPX_ERR_INVALID_ARG, "n too large for one call");
+    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_propagate")) return st;
+    return launch_propagate(*scene, brute, n, base, o, d, wl, seed, *out, hitmap, counters, (cudaStream_t)stream);
+}
+
+opx_status opx_propagate(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
+                         const float* d_dirs, const float* d_wavelengths, uint64_t seed, const opx_hits* out,
+                         uint32_t* d_hitmap, uint64_t* d_counters, void* cuda_stream) {
+    return propagate_common(scene, false, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, out, d_hitmap,
+                            d_counters, cuda_stream);
+}
+
+opx_status opx_propagate_brute(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
+                               const float* d_dirs, const float* d_wavelengths, uint64_t seed, const opx_hits* out,
+                               uint32_t* d_hitmap, uint64_t* d_counters, void* cuda_stream) {
+    return propagate_common(scene, true, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, out, d_hitmap,
+                            d_counters, cuda_stream);
+}
+
+// ------------------------------------------------------------------------- host-buffer streaming
+// Device staging per slot (two slots): inputs 28 B/photon, records 34 B/photon.
+static size_t slot_bytes(uint64_t chunk) {
+    size_t b = 0;
+    b += align_up(chunk * 12, 256) * 4;   // origins, dirs, pos, dir
+    b += align_up(chunk * 4, 256) * 3;    // wavelengths, pixel, surface
+    b += align_up(chunk, 256) * 2;        // state, bounces
+    return b;
+}
+
+opx_status opx_propagate_host_workspace_bytes(const opx_scene* scene, uint64_t chunk, size_t* bytes) {
+    if (!scene || !bytes || chunk == 0) return fail(OPX_ERR_INVALID_ARG, "NULL argument or chunk = 0");
+    *bytes = 2 * slot_bytes(chunk) + align_up(scene->n_pixels * 4 + 4, 256) + 256;
+    return OPX_OK;
+}
+
+opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* h_origins,
+                              const float* h_dirs, const float* h_wavelengths, uint64_t seed, const opx_hits* h_out,
+                              uint32_t* h_hitmap, uint64_t* h_counters, void* d_workspace, size_t workspace_bytes,
+                              uint64_t chunk, void* cuda_stream) {
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate_host before opx_bvh_build");
+    if (n == 0) return OPX_OK;
+    if (!h_origins || !h_dirs || !h_wavelengths || !h_out || !d_workspace || chunk == 0)
+        return fail(OPX_ERR_INVALID_ARG, "NULL argument or chunk = 0");
+    if (!h_out->pos || !h_out->dir || !h_out->pixel || !h_out->surface || !h_out->state || !h_out->bounces)
+        return fail(OPX_ERR_INVALID_ARG, "NULL hit-record array");
+    if (!h_hitmap && scene->n_pixels) return fail(OPX_ERR_INVALID_ARG, "h_hitmap is NULL but the scene has pixels");
+    if (misaligned(d_workspace, 256)) return fail(OPX_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    size_t need = 0;
+    opx_propagate_host_workspace_bytes(scene, chunk, &need);
+    if (workspace_bytes < need) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_propagate_host_workspace_bytes)");
+
+    cudaStream_t main = (cudaStream_t)cuda_stream;
+    struct Slot { float *o, *d, *wl, *pos, *dir; int32_t *pixel, *surface; uint8_t *state, *bounces; cudaStream_t st; cudaEvent_t done; };
+    Slot slot[2];
+    char* p = (char*)d_workspace;
+    auto take = [&](size_t bytes) { char* r = p; p += align_up(bytes, 256); return r; };
+    for (int k = 0; k < 2; ++k) {
+        Slot& s = slot[k];
+        s.o = (float*)take(chunk * 12); s.d = (float*)take(chunk * 12); s.pos = (float*)take(chunk * 12); s.dir = (float*)take(chunk * 12);
+        s.wl = (float*)take(chunk * 4); s.pixel = (int32_t*)take(chunk * 4); s.surface = (int32_t*)take(chunk * 4);
+        s.state = (uint8_t*)take(chunk); s.bounces = (uint8_t*)take(chunk);
+    }
+    uint32_t* d_hitmap = (uint32_t*)take(scene->n_pixels * 4 + 4);
+    uint64_t* d_counters = (uint64_t*)take(64);
+
+    opx_status st = OPX_OK;
+    cudaEvent_t start;
+    if ((st = check_cuda(cudaEventCreateWithFlags(&start, cudaEventDisableTiming), "cudaEventCreate"))) return st;
+    for (int k = 0; k < 2; ++k) {
+        cudaStreamCreateWithFlags(&slot[k].st, cudaStreamNonBlocking);
+        cudaEventCreateWithFlags(&slot[k].done, cudaEventDisableTiming);
+    }
+    // fork: both slot streams wait for whatever preceded on the caller's stream
+    cudaMemsetAsync(d_hitmap, 0, scene->n_pixels * 4 + 4, main);
+    cudaMemsetAsync(d_counters, 0, 64, main);
+    cudaEventRecord(start, main);
+    for (int k = 0; k < 2; ++k) cudaStreamWaitEvent(slot[k].st, start, 0);
+
+    uint64_t done = 0;
+    int k = 0;
+    while (done < n && st == OPX_OK) {
+        const uint64_t m = (n - done < chunk) ? (n - done) : chunk;
+        Slot& s = slot[k];
+        cudaMemcpyAsync(s.o, h_origins + 3 * done, m * 12, cudaMemcpyHostToDevice, s.st);
+        cudaMemcpyAsync(s.d, h_dirs + 3 * done, m * 12, cudaMemcpyHostToDevice, s.st);
+        cudaMemcpyAsync(s.wl, h_wavelengths + done, m * 4, cudaMemcpyHostToDevice, s.st);
+        opx_hits dev_out{s.pos, s.dir, s.pixel, s.surface, s.state, s.bounces};
+        st = launch_propagate(*scene, false, m, photon_id_base + done, s.o, s.d, s.wl, seed, dev_out, d_hitmap,
+                              d_counters, s.st);
+        cudaMemcpyAsync(h_out->pos + 3 * done, s.pos, m * 12, cudaMemcpyDeviceToHost, s.st);
+        cudaMemcpyAsync(h_out->dir + 3 * done, s.dir, m * 12, cudaMemcpyDeviceToHost, s.st);
+        cudaMemcpyAsync(h_out->pixel + done, s.pixel, m * 4, cudaMemcpyDeviceToHost, s.st);
+        cudaMemcpyAsync(h_out->surface + done, s.surface, m * 4, cudaMemcpyDeviceToHost, s.st);
+        cudaMemcpyAsync(h_out->state + done, s.state, m, cudaMemcpyDeviceToHost, s.st);
+        cudaMemcpyAsync(h_out->bounces + done, s.bounces, m, cudaMemcpyDeviceToHost, s.st);
+        done += m;
+        k ^= 1;
+    }
+    // join
+    for (int j = 0; j < 2; ++j) { cudaEventRecord(slot[j].done, slot[j].st); cudaStreamWaitEvent(main, slot[j].done, 0); }
+    std::vector<uint32_t> hm(scene->n_pixels);
+    uint64_t cnt[8] = {0};
+    if (scene->n_pixels) cudaMemcpyAsync(hm.data(), d_hitmap, scene->n_pixels * 4, cudaMemcpyDeviceToHost, main);
+    cudaMemcpyAsync(cnt, d_counters, 64, cudaMemcpyDeviceToHost, main);
+    cudaError_t e = cudaStreamSynchronize(main);
+    for (int j = 0; j < 2; ++j) { cudaStreamDestroy(slot[j].st); cudaEventDestroy(slot[j].done); }
+    cudaEventDestroy(start);
+    if (st != OPX_OK) return st;
+    if (e != cudaSuccess) return check_cuda(e, "opx_propagate_host");
+    for (uint64_t i = 0; i < scene->n_pixels; ++i) h_hitmap[i] += hm[i];
+    if (h_counters) for (int i = 0; i < 8; ++i) h_counters[i] += cnt[i];
+    return OPX_OK;
+}
+
+opx_status opx_profile_begin(opx_scene* scene, uint32_t max_calls) {
+    if (!scene || max_calls == 0) return fail(OPX_ERR_INVALID_ARG, "scene is NULL or max_calls = 0");
+    while (scene->prof_events.size() < 3ull * max_calls) {
+        cudaEvent_t e;
+        if (opx_status st = check_cuda(cudaEventCreate(&e), "cudaEventCreate")) return st;
+        scene->prof_events.push_back(e);
+    }
+    scene->prof_max = max_calls;
+    scene->prof_used = 0;
+    return OPX_OK;
+}
+
+opx_status opx_profile_end(opx_scene* scene, float* ms_propagate, float* ms_bin, uint32_t* n_calls) {
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    const uint32_t used = scene->prof_used;
+    scene->prof_max = 0;
+    scene->prof_used = 0;
+    if (n_calls) *n_calls = used;
+    for (uint32_t k = 0; k < used; ++k) {
+        cudaEvent_t* ev = &scene->prof_events[3 * k];
+        if (opx_status st = check_cuda(cudaEventSynchronize(ev[2]), "cudaEventSynchronize")) return st;
+        float a = 0.f, b = 0.f;
+        if (opx_status st = check_cuda(cudaEventElapsedTime(&a, ev[0], ev[1]), "cudaEventElapsedTime")) return st;
+        if (opx_status st = check_cuda(cudaEventElapsedTime(&b, ev[1], ev[2]), "cudaEventElapsedTime")) return st;
+        if (ms_propagate) ms_propagate[k] = a;
+        if (ms_bin) ms_bin[k] = b;
+    }
+    return OPX_OK;
+}
+
+opx_status opx_propagate_stats(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
+                               const float* d_dirs, const float* d_wavelengths, uint64_t seed, uint64_t* d_stats,
+                               void* cuda_stream) {
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate_stats before opx_bvh_build");
+    if (n == 0) return OPX_OK;
+    if (!d_origins || !d_dirs || !d_wavelengths || !d_stats) return fail(OPX_ERR_INVALID_ARG, "NULL pointer");
+    return launch_stats(*scene, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, d_stats, (cudaStream_t)cuda_stream);
+}
+
+opx_status opx_scene_info(const opx_scene* scene, uint64_t* n_triangles, uint64_t* n_nodes, uint64_t* n_pixels,
+                          uint64_t* n_surfaces) {
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    const uint64_t T = scene->tri_surface.size();
+    if (n_triangles) *n_triangles = T;
+    if (n_nodes) *n_nodes = T > 1 ? T - 1 : 1;
+    if (n_pixels) *n_pixels = scene->n_pixels;
+    if (n_surfaces) *n_surfaces = scene->surfaces.size();
+    return OPX_OK;
+}
+
+opx_status opx_scene_get_layout(const opx_scene* scene, opx_scene_layout* out) {
+    if (!scene || !out) return fail(OPX_ERR_INVALID_ARG, "NULL argument");
+    *out = scene->layout;
+    return OPX_OK;
+}
+
+void opx_scene_destroy(opx_scene* scene) { delete scene; }
+
+}  // extern "C"

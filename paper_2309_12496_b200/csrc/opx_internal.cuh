@@ -1,0 +1,88 @@
+// Internal declarations shared by the translation units of libopx.so (CUDA path only).
+// Written from DESIGN.md sections 2, 3 and 8; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/opx.h"
+
+namespace opx {
+
+// ------------------------------------------------------------------ device-side scene description
+struct alignas(16) FrameDev {  // 64 B
+    float Ax, Ay, Az, ux;
+    float uy, uz, vx, vy;
+    float vz, inv_pitch_u, inv_pitch_v, pad0;
+    uint32_t nu, nv, pixel_base, pad1;
+};
+
+// BVH node, 64 B: boxes of the two children and their references.
+//   q0 = (c0.lo.x, c0.lo.y, c0.lo.z, c0.hi.x)
+//   q1 = (c0.hi.y, c0.hi.z, c1.lo.x, c1.lo.y)
+//   q2 = (c1.lo.z, c1.hi.x, c1.hi.y, c1.hi.z)
+//   q3 = (child0, child1, 0, 0) as int bits; child >= 0: internal node index; child < 0: leaf ~child
+struct alignas(16) NodeDev { float4 q0, q1, q2; int4 q3; };
+
+// Everything the propagation kernels need, passed by value as a kernel parameter.
+struct SceneDev {
+    const NodeDev* nodes;      // n_nodes
+    const float4* tris;        // 3 per triangle, leaf order: (a.xyz, id bits) (b.xyz, surface bits) (c.xyz, 0)
+    const float4* normals;     // leaf order: n.xyz, surface id bits
+    const int2* surfaces;      // (material, frame)
+    const uint32_t* mat_kinds;
+    const float* tables;       // n_materials x n_lambda
+    const FrameDev* frames;
+    uint32_t n_tri, n_nodes, n_lambda, max_bounces;
+    float lambda_min, inv_dlambda, t_min;
+};
+
+struct Layout : opx_scene_layout {};
+
+// ------------------------------------------------------------------------------ host-side scene
+struct SceneHost {
+    opx_scene_params params{};
+    std::vector<float> tri;          // T x 9, global id order
+    std::vector<int32_t> tri_surface;
+    std::vector<float> normals;      // T x 3, contract 3.4
+    std::vector<int2> surfaces;      // material, frame
+    std::vector<uint32_t> mat_kinds;
+    std::vector<float> tables;       // M x n_lambda
+    std::vector<FrameDev> frames;
+    uint64_t n_pixels = 0;
+    float inv_dlambda = 0.f;
+    // set by opx_bvh_build
+    bool built = false;
+    void* d_scene_ws = nullptr;
+    size_t scene_bytes = 0;
+    SceneDev dev{};
+    opx_scene_layout layout{};
+    // opx_profile_begin/end: event triples (start, after propagate, after bin), one per call
+    mutable std::vector<cudaEvent_t> prof_events;
+    mutable uint32_t prof_max = 0, prof_used = 0;
+    ~SceneHost() { for (cudaEvent_t e : prof_events) cudaEventDestroy(e); }
+};
+
+// error plumbing (opx_api.cu)
+opx_status fail(opx_status st, const std::string& msg);
+opx_status check_cuda(cudaError_t e, const char* what);
+void count_launch(uint64_t n = 1);
+
+// build (opx_build.cu)
+void compute_layout(const SceneHost& s, opx_scene_layout* lay, size_t* tmp_bytes);
+opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_t stream);
+
+// propagate (opx_propagate.cu)
+opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, uint64_t id_base, const float* o,
+                            const float* d, const float* wl, uint64_t seed, const opx_hits& out,
+                            uint32_t* hitmap, uint64_t* counters, cudaStream_t stream);
+opx_status launch_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,
+                        const float* wl, uint64_t seed, uint64_t* stats, cudaStream_t stream);
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace opx
+
+struct opx_scene : opx::SceneHost {};

@@ -1,0 +1,279 @@
+"""Thin Python binding of libopx.so (include/opx.h): argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in the CUDA kernels of
+csrc/.  There is no CPU fallback: loading fails loudly if the library is missing.
+Names follow include/opx.h (opx_scene_create -> Scene(...), opx_bvh_build -> Scene.build(),
+opx_propagate -> Scene.propagate(), opx_propagate_host -> Scene.propagate_host()).
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "lib", "libopx.so")
+
+STATE_NAMES = ("DETECTED", "QE_REJECTED", "ABSORBED_SURFACE", "ABSORBED_MIRROR", "DETECTOR_DEAD",
+               "BOUNCE_LIMIT", "ESCAPED")
+OPX_OK, OPX_ERR_INVALID_ARG, OPX_ERR_BAD_STATE, OPX_ERR_WORKSPACE_TOO_SMALL, OPX_ERR_CUDA, \
+    OPX_ERR_UNSUPPORTED_DEVICE = range(6)
+
+EXPORTS = ("opx_scene_create", "opx_scene_workspace_bytes", "opx_bvh_build", "opx_propagate",
+           "opx_propagate_brute", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
+           "opx_profile_begin", "opx_profile_end", "opx_propagate_stats", "opx_scene_info", "opx_scene_get_layout", "opx_launch_count", "opx_scene_destroy",
+           "opx_last_error", "opx_version")
+
+
+class OpxError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__(f"opx status {status}: {message}")
+        self.status = status
+
+
+class SceneParams(C.Structure):
+    _fields_ = [("lambda_min_nm", C.c_float), ("lambda_max_nm", C.c_float), ("n_lambda", C.c_uint32),
+                ("max_bounces", C.c_uint32), ("t_min_mm", C.c_float)]
+
+
+class Material(C.Structure):
+    _fields_ = [("kind", C.c_uint32), ("table", C.c_void_p)]
+
+
+class PixelFrame(C.Structure):
+    _fields_ = [("A", C.c_float * 3), ("u", C.c_float * 3), ("v", C.c_float * 3),
+                ("pitch_u", C.c_float), ("pitch_v", C.c_float),
+                ("nu", C.c_uint32), ("nv", C.c_uint32), ("pixel_base", C.c_uint32)]
+
+
+class Mesh(C.Structure):
+    _fields_ = [("vertices", C.c_void_p), ("n_vertices", C.c_uint32), ("indices", C.c_void_p),
+                ("n_triangles", C.c_uint32), ("material", C.c_uint32), ("pixel_frame", C.c_int32)]
+
+
+class Hits(C.Structure):
+    _fields_ = [("pos", C.c_void_p), ("dir", C.c_void_p), ("pixel", C.c_void_p), ("surface", C.c_void_p),
+                ("state", C.c_void_p), ("bounces", C.c_void_p)]
+
+
+class SceneLayout(C.Structure):
+    _fields_ = [(k, C.c_uint64) for k in ("nodes", "triangles", "normals", "surfaces", "mat_kinds", "tables",
+                                          "frames", "sorted_keys", "parents", "total_bytes")]
+
+
+_lib = None
+
+
+def load_library(path=LIB_PATH):
+    """dlopen libopx.so; raises if it has not been built (`python -m paper_2309_12496_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise OpxError(-1, f"{path} not found: build it with `python paper_2309_12496_b200/build.py` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(path)
+    vp, u64, u32 = C.c_void_p, C.c_uint64, C.c_uint32
+    lib.opx_last_error.restype = C.c_char_p
+    lib.opx_version.restype = C.c_char_p
+    lib.opx_launch_count.restype = u64
+    lib.opx_scene_create.argtypes = [vp, vp, u32, vp, u32, vp, u32, vp]
+    lib.opx_scene_workspace_bytes.argtypes = [vp, vp, vp]
+    lib.opx_bvh_build.argtypes = [vp, vp, C.c_size_t, vp, C.c_size_t, vp]
+    for f in (lib.opx_propagate, lib.opx_propagate_brute):
+        f.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp, vp, vp]
+    lib.opx_propagate_host_workspace_bytes.argtypes = [vp, u64, vp]
+    lib.opx_propagate_host.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp, vp, vp, C.c_size_t, u64, vp]
+    lib.opx_profile_begin.argtypes = [vp, u32]
+    lib.opx_profile_end.argtypes = [vp, vp, vp, vp]
+    lib.opx_propagate_stats.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp]
+    lib.opx_scene_info.argtypes = [vp, vp, vp, vp, vp]
+    lib.opx_scene_get_layout.argtypes = [vp, vp]
+    lib.opx_scene_destroy.argtypes = [vp]
+    _lib = lib
+    return lib
+
+
+def _check(status):
+    if status != OPX_OK:
+        raise OpxError(status, load_library().opx_last_error().decode())
+
+
+def launch_count():
+    return int(load_library().opx_launch_count())
+
+
+def _np_ptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+class Scene:
+    """opx_scene handle.  `scene` is any object with the fields of workloads.Scene (meshes,
+    materials, frames, lambda_min, lambda_max, n_lambda, max_bounces, t_min)."""
+
+    def __init__(self, scene):
+        lib = load_library()
+        keep = []
+        mats = (Material * max(1, len(scene.materials)))()
+        for k, m in enumerate(scene.materials):
+            t = np.ascontiguousarray(m["table"], dtype=np.float32)
+            keep.append(t)
+            mats[k].kind, mats[k].table = int(m["kind"]), t.ctypes.data
+        frames = (PixelFrame * max(1, len(scene.frames)))()
+        for k, f in enumerate(scene.frames):
+            frames[k].A[:] = [float(x) for x in f["A"]]
+            frames[k].u[:] = [float(x) for x in f["u"]]
+            frames[k].v[:] = [float(x) for x in f["v"]]
+            frames[k].pitch_u, frames[k].pitch_v = f["pitch_u"], f["pitch_v"]
+            frames[k].nu, frames[k].nv, frames[k].pixel_base = f["nu"], f["nv"], f["pixel_base"]
+        meshes = (Mesh * max(1, len(scene.meshes)))()
+        for k, m in enumerate(scene.meshes):
+            v = np.ascontiguousarray(m["vertices"], dtype=np.float32)
+            i = np.ascontiguousarray(m["indices"], dtype=np.uint32)
+            keep += [v, i]
+            meshes[k].vertices, meshes[k].n_vertices = v.ctypes.data, len(v)
+            meshes[k].indices, meshes[k].n_triangles = i.ctypes.data, len(i)
+            meshes[k].material, meshes[k].pixel_frame = int(m["material"]), int(m["frame"])
+        params = SceneParams(scene.lambda_min, scene.lambda_max, scene.n_lambda, scene.max_bounces, scene.t_min)
+        handle = C.c_void_p()
+        _check(lib.opx_scene_create(C.byref(params), meshes, len(scene.meshes), mats, len(scene.materials),
+                                    frames, len(scene.frames), C.byref(handle)))
+        self._h = handle
+        nt, nn, npix, ns = C.c_uint64(), C.c_uint64(), C.c_uint64(), C.c_uint64()
+        _check(lib.opx_scene_info(self._h, C.byref(nt), C.byref(nn), C.byref(npix), C.byref(ns)))
+        self.n_triangles, self.n_nodes, self.n_pixels, self.n_surfaces = nt.value, nn.value, npix.value, ns.value
+        self.workspace = None
+        self._host_ws = None
+
+    def __del__(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.opx_scene_destroy(self._h)
+            self._h = None
+
+    # ---------------------------------------------------------------------------------- build
+    def workspace_bytes(self):
+        a, b = C.c_size_t(), C.c_size_t()
+        _check(load_library().opx_scene_workspace_bytes(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def layout(self):
+        lay = SceneLayout()
+        _check(load_library().opx_scene_get_layout(self._h, C.byref(lay)))
+        return {k: getattr(lay, k) for k, _ in SceneLayout._fields_}
+
+    def build(self, device="cuda", stream=None, keep_tmp=False):
+        """opx_bvh_build into torch-owned workspaces; returns self."""
+        import torch
+        scene_b, tmp_b = self.workspace_bytes()
+        self.workspace = torch.empty(scene_b + 256, dtype=torch.uint8, device=device)
+        tmp = torch.empty(tmp_b + 256, dtype=torch.uint8, device=device)
+        st = stream if stream is not None else torch.cuda.current_stream(device)
+        _check(load_library().opx_bvh_build(self._h, _aligned(self.workspace), scene_b, _aligned(tmp), tmp_b,
+                                            C.c_void_p(st.cuda_stream)))
+        st.synchronize()
+        if keep_tmp:
+            self._tmp = tmp
+        return self
+
+    # ------------------------------------------------------------------------------ propagate
+    def alloc_records(self, n, device="cuda"):
+        import torch
+        return dict(pos=torch.empty((n, 3), dtype=torch.float32, device=device),
+                    dir=torch.empty((n, 3), dtype=torch.float32, device=device),
+                    pixel=torch.empty(n, dtype=torch.int32, device=device),
+                    surface=torch.empty(n, dtype=torch.int32, device=device),
+                    state=torch.empty(n, dtype=torch.uint8, device=device),
+                    bounces=torch.empty(n, dtype=torch.uint8, device=device))
+
+    def alloc_accumulators(self, device="cuda"):
+        import torch
+        return (torch.zeros(max(1, self.n_pixels), dtype=torch.int32, device=device),
+                torch.zeros(8, dtype=torch.int64, device=device))
+
+    def propagate(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, records=None, hitmap=None,
+                  counters=None, stream=None, brute=False):
+        """opx_propagate on device tensors.  hitmap (int32 view of uint32) and counters (int64 view of
+        uint64) are accumulated into; pass zeroed tensors or None to have them created."""
+        import torch
+        n = int(wavelengths.shape[0])
+        for t, shape in ((origins, (n, 3)), (dirs, (n, 3)), (wavelengths, (n,))):
+            if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == shape):
+                raise OpxError(OPX_ERR_INVALID_ARG, "photon tensors must be contiguous float32 CUDA tensors (n,3),(n,3),(n,)")
+        dev = wavelengths.device
+        if records is None:
+            records = self.alloc_records(n, dev)
+        if hitmap is None or counters is None:
+            hm, ct = self.alloc_accumulators(dev)
+            hitmap = hm if hitmap is None else hitmap
+            counters = ct if counters is None else counters
+        h = Hits(*(records[k].data_ptr() for k in ("pos", "dir", "pixel", "surface", "state", "bounces")))
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        fn = load_library().opx_propagate_brute if brute else load_library().opx_propagate
+        _check(fn(self._h, n, int(photon_id_base), origins.data_ptr(), dirs.data_ptr(), wavelengths.data_ptr(),
+                  int(seed), C.byref(h), hitmap.data_ptr(), counters.data_ptr(), C.c_void_p(st.cuda_stream)))
+        out = dict(records)
+        out["hitmap"], out["counters"] = hitmap[:self.n_pixels], counters
+        return out
+
+    def profile_begin(self, max_calls):
+        """opx_profile_begin: record per-kernel CUDA events for the next max_calls propagate calls."""
+        self._prof_max = int(max_calls)
+        _check(load_library().opx_profile_begin(self._h, self._prof_max))
+
+    def profile_end(self):
+        """opx_profile_end -> (ms_propagate[], ms_bin[]) per recorded call."""
+        a = (C.c_float * self._prof_max)()
+        b = (C.c_float * self._prof_max)()
+        n = C.c_uint32()
+        _check(load_library().opx_profile_end(self._h, a, b, C.byref(n)))
+        return list(a[:n.value]), list(b[:n.value])
+
+    def propagate_stats(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, stream=None):
+        """opx_propagate_stats -> dict(segments, nodes, triangle_tests, interactions)."""
+        import torch
+        n = int(wavelengths.shape[0])
+        stats = torch.zeros(4, dtype=torch.int64, device=wavelengths.device)
+        st = stream if stream is not None else torch.cuda.current_stream(wavelengths.device)
+        _check(load_library().opx_propagate_stats(self._h, n, int(photon_id_base), origins.data_ptr(), dirs.data_ptr(),
+                                                  wavelengths.data_ptr(), int(seed), stats.data_ptr(),
+                                                  C.c_void_p(st.cuda_stream)))
+        v = stats.cpu().tolist()
+        return dict(segments=v[0], nodes=v[1], triangle_tests=v[2], interactions=v[3])
+
+    def propagate_host(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, chunk=1 << 21, out=None,
+                       stream=None, device="cuda"):
+        """opx_propagate_host: host (pinned torch or numpy) buffers in, host buffers out."""
+        import torch
+        lib = load_library()
+        n = int(wavelengths.shape[0])
+        chunk = max(1, min(int(chunk), max(n, 1)))
+        need = C.c_size_t()
+        _check(lib.opx_propagate_host_workspace_bytes(self._h, chunk, C.byref(need)))
+        if self._host_ws is None or self._host_ws.numel() < need.value + 256:
+            self._host_ws = torch.empty(need.value + 256, dtype=torch.uint8, device=device)
+        if out is None:
+            out = alloc_host_records(n, self.n_pixels)
+        ptr = (lambda t: t.data_ptr()) if isinstance(wavelengths, torch.Tensor) else (lambda a: a.ctypes.data)
+        h = Hits(*(out[k].data_ptr() for k in ("pos", "dir", "pixel", "surface", "state", "bounces")))
+        st = stream if stream is not None else torch.cuda.current_stream(device)
+        _check(lib.opx_propagate_host(self._h, n, int(photon_id_base), ptr(origins), ptr(dirs), ptr(wavelengths),
+                                      int(seed), C.byref(h), out["hitmap"].data_ptr(), out["counters"].data_ptr(),
+                                      _aligned(self._host_ws), need.value, chunk, C.c_void_p(st.cuda_stream)))
+        return out
+
+
+def alloc_host_records(n, n_pixels):
+    """Pinned host buffers for opx_propagate_host (hitmap and counters zeroed)."""
+    import torch
+    pin = torch.cuda.is_available()
+    mk = lambda shape, dt: torch.empty(shape, dtype=dt, pin_memory=pin)
+    out = dict(pos=mk((n, 3), torch.float32), dir=mk((n, 3), torch.float32), pixel=mk((n,), torch.int32),
+               surface=mk((n,), torch.int32), state=mk((n,), torch.uint8), bounces=mk((n,), torch.uint8),
+               hitmap=torch.zeros(max(1, n_pixels), dtype=torch.int32, pin_memory=pin),
+               counters=torch.zeros(8, dtype=torch.int64, pin_memory=pin))
+    return out
+
+
+def _aligned(t, a=256):
+    """256-byte aligned pointer inside a tensor allocated with >= a spare bytes."""
+    p = t.data_ptr()
+    return C.c_void_p((p + a - 1) // a * a)
