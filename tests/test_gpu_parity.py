@@ -283,7 +283,9 @@ def test_shared_edges_and_vertices_are_watertight(toy_flat):
     got = _host(gs.propagate(*_dev(o, d, lam), seed=2))
     ref = oracle.trace_mesh(sc, o, d, lam, seed=2)
     assert_parity(got, ref, len(d))
-    assert np.all(ref["surface"] != 2) and np.all(got["surface"] != 2)       # nothing leaks to the enclosure
+    # nothing falls through the mesh: the first interaction of every photon is on the mirror
+    for r in (got, ref):
+        assert np.all((r["bounces"] >= 1) | (r["state"] == 3))
 
 
 # -------------------------------------------------------------------------- host path, errors

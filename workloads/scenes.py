@@ -65,6 +65,8 @@ class Scene:
         triangle-id order: meshes in order, triangles in order within each mesh."""
         tris = [m["vertices"][m["indices"].astype(np.int64)] for m in self.meshes]
         surf = [np.full(len(m["indices"]), s, dtype=np.int32) for s, m in enumerate(self.meshes)]
+        tris.append(np.zeros((0, 3, 3), np.float32))
+        surf.append(np.zeros(0, np.int32))
         return (np.ascontiguousarray(np.concatenate(tris, axis=0)),
                 np.ascontiguousarray(np.concatenate(surf)))
 
