@@ -1,0 +1,208 @@
+// Device functions of the arithmetic contract, shared by the propagation kernels
+// of opx_propagate.cu.  Every contract operation is an explicit round-to-nearest intrinsic
+// (__fmul_rn, __fsub_rn, __fmaf_rn, __fdiv_rn): the result does not depend on contraction choices.
+#pragma once
+#include "opx_internal.cuh"
+
+namespace opx {
+
+__device__ constexpr float kInf = __builtin_huge_valf();
+
+// ---------------------------------------------------------------------------- Philox4x32-10 (3.1)
+__device__ __forceinline__ float philox_uniform(uint64_t seed, uint64_t g, uint32_t b) {
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+    uint32_t c0 = (uint32_t)g, c1 = (uint32_t)(g >> 32), c2 = b, c3 = 0u;
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
+        const uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return __fmul_rn((float)(c0 >> 8), 5.9604644775390625e-8f);   // 2^-24, exact
+}
+
+// ------------------------------------------------------------------------------ table lookup (3.2)
+__device__ __forceinline__ float table_lerp(const float* __restrict__ y, uint32_t n_lambda, float lambda_min,
+                                            float inv_dl, float lambda) {
+    const float x = __fmul_rn(__fsub_rn(lambda, lambda_min), inv_dl);
+    const float xf = floorf(x);
+    int j;
+    if (!(xf >= 0.f)) j = 0;
+    else if (xf > (float)(n_lambda - 2)) j = (int)n_lambda - 2;
+    else j = (int)xf;
+    float f = __fsub_rn(x, (float)j);
+    if (!(f >= 0.f)) f = 0.f;
+    if (f > 1.f) f = 1.f;
+    const float y0 = __ldg(y + j), y1 = __ldg(y + j + 1);
+    return __fmaf_rn(f, __fsub_rn(y1, y0), y0);
+}
+
+// ------------------------------------------------------------------------------- ray set-up (3.3)
+struct RayW {                 // watertight-test constants of one segment
+    float okx, oky, okz;      // origin permuted to (kx, ky, kz)
+    float Sx, Sy, Sz;
+    int kx, ky, kz;
+};
+
+__device__ __forceinline__ float sel3(float x, float y, float z, int k) { return k == 0 ? x : (k == 1 ? y : z); }
+
+__device__ __forceinline__ RayW ray_setup(float ox, float oy, float oz, float dx, float dy, float dz) {
+    RayW r;
+    int kz = 0;
+    float best = fabsf(dx);
+    if (fabsf(dy) > best) { kz = 1; best = fabsf(dy); }
+    if (fabsf(dz) > best) { kz = 2; }
+    int kx = kz == 2 ? 0 : kz + 1;
+    int ky = kx == 2 ? 0 : kx + 1;
+    const float dkz = sel3(dx, dy, dz, kz);
+    if (dkz < 0.f) { const int t = kx; kx = ky; ky = t; }
+    r.kx = kx; r.ky = ky; r.kz = kz;
+    r.Sx = __fdiv_rn(sel3(dx, dy, dz, kx), dkz);
+    r.Sy = __fdiv_rn(sel3(dx, dy, dz, ky), dkz);
+    r.Sz = __fdiv_rn(1.f, dkz);
+    r.okx = sel3(ox, oy, oz, kx); r.oky = sel3(ox, oy, oz, ky); r.okz = sel3(ox, oy, oz, kz);
+    return r;
+}
+
+// Contract triangle test.  Returns true with t when the triangle is hit at finite t > tmin.
+__device__ __forceinline__ bool tri_test(const RayW& r, const float4 a, const float4 b, const float4 c, float tmin, float& t_out) {
+    const float Akx = __fsub_rn(sel3(a.x, a.y, a.z, r.kx), r.okx), Aky = __fsub_rn(sel3(a.x, a.y, a.z, r.ky), r.oky), Akz = __fsub_rn(sel3(a.x, a.y, a.z, r.kz), r.okz);
+    const float Bkx = __fsub_rn(sel3(b.x, b.y, b.z, r.kx), r.okx), Bky = __fsub_rn(sel3(b.x, b.y, b.z, r.ky), r.oky), Bkz = __fsub_rn(sel3(b.x, b.y, b.z, r.kz), r.okz);
+    const float Ckx = __fsub_rn(sel3(c.x, c.y, c.z, r.kx), r.okx), Cky = __fsub_rn(sel3(c.x, c.y, c.z, r.ky), r.oky), Ckz = __fsub_rn(sel3(c.x, c.y, c.z, r.kz), r.okz);
+    const float Ax = __fmaf_rn(-r.Sx, Akz, Akx), Ay = __fmaf_rn(-r.Sy, Akz, Aky);
+    const float Bx = __fmaf_rn(-r.Sx, Bkz, Bkx), By = __fmaf_rn(-r.Sy, Bkz, Bky);
+    const float Cx = __fmaf_rn(-r.Sx, Ckz, Ckx), Cy = __fmaf_rn(-r.Sy, Ckz, Cky);
+    const float U = __fsub_rn(__fmul_rn(Cx, By), __fmul_rn(Cy, Bx));
+    const float V = __fsub_rn(__fmul_rn(Ax, Cy), __fmul_rn(Ay, Cx));
+    const float W = __fsub_rn(__fmul_rn(Bx, Ay), __fmul_rn(By, Ax));
+    float t;
+    if (U == 0.f || V == 0.f || W == 0.f) {
+        const double Ud = __dsub_rn(__dmul_rn((double)Cx, (double)By), __dmul_rn((double)Cy, (double)Bx));
+        const double Vd = __dsub_rn(__dmul_rn((double)Ax, (double)Cy), __dmul_rn((double)Ay, (double)Cx));
+        const double Wd = __dsub_rn(__dmul_rn((double)Bx, (double)Ay), __dmul_rn((double)By, (double)Ax));
+        if ((Ud < 0.0 || Vd < 0.0 || Wd < 0.0) && (Ud > 0.0 || Vd > 0.0 || Wd > 0.0)) return false;
+        const double det = __dadd_rn(__dadd_rn(Ud, Vd), Wd);
+        if (det == 0.0) return false;
+        const double Az = (double)__fmul_rn(r.Sz, Akz), Bz = (double)__fmul_rn(r.Sz, Bkz), Cz = (double)__fmul_rn(r.Sz, Ckz);
+        const double T = __fma_rn(Wd, Cz, __fma_rn(Vd, Bz, __dmul_rn(Ud, Az)));
+        t = __double2float_rn(__ddiv_rn(T, det));
+    } else {
+        if ((U < 0.f || V < 0.f || W < 0.f) && (U > 0.f || V > 0.f || W > 0.f)) return false;
+        const float det = __fadd_rn(__fadd_rn(U, V), W);
+        if (det == 0.f) return false;
+        const float Az = __fmul_rn(r.Sz, Akz), Bz = __fmul_rn(r.Sz, Bkz), Cz = __fmul_rn(r.Sz, Ckz);
+        const float T = __fmaf_rn(W, Cz, __fmaf_rn(V, Bz, __fmul_rn(U, Az)));
+        t = __fdiv_rn(T, det);
+    }
+    if (!(fabsf(t) < kInf) || !(t > tmin)) return false;      // NaN and +-inf rejected
+    t_out = t;
+    return true;
+}
+
+struct Hit { float t; int j; int gid; };   // j: leaf-order index; gid: global triangle id
+
+// Tests leaf-order triangle j and keeps the lexicographic minimum of (t, global id).
+__device__ __forceinline__ void consider(const SceneDev& sc, const RayW& rw, int j, float tmin, int last, Hit& h) {
+    const float4 a = __ldg(sc.tris + 3 * (size_t)j), b = __ldg(sc.tris + 3 * (size_t)j + 1), c = __ldg(sc.tris + 3 * (size_t)j + 2);
+    const int gid = __float_as_int(a.w);
+    if (gid == last) return;
+    float t;
+    if (!tri_test(rw, a, b, c, tmin, t)) return;
+    if (t < h.t || (t == h.t && gid < h.gid)) { h.t = t; h.j = j; h.gid = gid; }
+}
+
+// ------------------------------------------------------------------- photon state + interaction
+struct Photon {
+    float ox, oy, oz, dx, dy, dz;      // current segment
+    float px, py, pz;                   // record position
+    float lambda;
+    uint64_t g;                         // global photon id
+    uint32_t b;                         // reflections so far
+    int last, state, surface, pixel;
+};
+
+__device__ __forceinline__ void photon_init(Photon& p, float ox, float oy, float oz, float dx, float dy, float dz,
+                                            float lambda, uint64_t g) {
+    p.ox = ox; p.oy = oy; p.oz = oz; p.dx = dx; p.dy = dy; p.dz = dz; p.px = ox; p.py = oy; p.pz = oz;
+    p.lambda = lambda; p.g = g; p.b = 0; p.last = -1; p.state = -1; p.surface = -1; p.pixel = -1;
+}
+
+// Applies the outcome of one closest-hit query.  Returns true when the photon
+// was reflected and continues with a new segment; otherwise p.state holds the terminal state.
+__device__ __forceinline__ bool interact(const SceneDev& sc, const Hit& h, Photon& p, uint64_t seed) {
+    if (h.j < 0) { p.state = OPX_ESCAPED; p.px = p.ox; p.py = p.oy; p.pz = p.oz; p.surface = -1; return false; }
+    p.px = __fmaf_rn(h.t, p.dx, p.ox); p.py = __fmaf_rn(h.t, p.dy, p.oy); p.pz = __fmaf_rn(h.t, p.dz, p.oz);   // 3.7
+    const float4 nrm = __ldg(sc.normals + h.j);
+    p.surface = __float_as_int(nrm.w);
+    const int2 sf = __ldg(sc.surfaces + p.surface);
+    const uint32_t kind = __ldg(sc.mat_kinds + sf.x);
+    const float* table = sc.tables + (size_t)sf.x * sc.n_lambda;
+    if (kind == OPX_MAT_ABSORBER) { p.state = OPX_ABSORBED_SURFACE; return false; }
+    if (kind == OPX_MAT_MIRROR) {
+        const float u = philox_uniform(seed, p.g, p.b);
+        if (!(u < table_lerp(table, sc.n_lambda, sc.lambda_min, sc.inv_dlambda, p.lambda))) { p.state = OPX_ABSORBED_MIRROR; return false; }
+        const float c = __fmaf_rn(p.dz, nrm.z, __fmaf_rn(p.dy, nrm.y, __fmul_rn(p.dx, nrm.x)));   // 3.5
+        const float m2c = __fmul_rn(-2.f, c);
+        p.dx = __fmaf_rn(m2c, nrm.x, p.dx); p.dy = __fmaf_rn(m2c, nrm.y, p.dy); p.dz = __fmaf_rn(m2c, nrm.z, p.dz);
+        p.ox = p.px; p.oy = p.py; p.oz = p.pz; p.last = h.gid; ++p.b;
+        if (p.b == sc.max_bounces) { p.state = OPX_BOUNCE_LIMIT; return false; }
+        return true;
+    }
+    // detector (3.6)
+    const float4* f = reinterpret_cast<const float4*>(sc.frames + sf.y);
+    const float4 f0 = __ldg(f), f1 = __ldg(f + 1), f2 = __ldg(f + 2);
+    const uint4 f3 = __ldg(reinterpret_cast<const uint4*>(f) + 3);
+    const float qx = __fsub_rn(p.px, f0.x), qy = __fsub_rn(p.py, f0.y), qz = __fsub_rn(p.pz, f0.z);
+    const float ca = __fmaf_rn(qz, f1.y, __fmaf_rn(qy, f1.x, __fmul_rn(qx, f0.w)));
+    const float cb = __fmaf_rn(qz, f2.x, __fmaf_rn(qy, f1.w, __fmul_rn(qx, f1.z)));
+    const float fu = floorf(__fmul_rn(ca, f2.y)), fv = floorf(__fmul_rn(cb, f2.z));
+    if (!(fu >= 0.f) || !(fv >= 0.f) || !(fu < (float)f3.x) || !(fv < (float)f3.y)) { p.state = OPX_DETECTOR_DEAD; return false; }
+    p.pixel = (int)(f3.z + (uint32_t)fv * f3.x + (uint32_t)fu);
+    const float u = philox_uniform(seed, p.g, p.b);
+    p.state = (u < table_lerp(table, sc.n_lambda, sc.lambda_min, sc.inv_dlambda, p.lambda)) ? OPX_DETECTED : OPX_QE_REJECTED;
+    return false;
+}
+
+__device__ __forceinline__ void store_record(const opx_hits& out, uint64_t i, const Photon& p) {
+    out.pos[3 * i] = p.px; out.pos[3 * i + 1] = p.py; out.pos[3 * i + 2] = p.pz;
+    out.dir[3 * i] = p.dx; out.dir[3 * i + 1] = p.dy; out.dir[3 * i + 2] = p.dz;
+    out.pixel[i] = p.pixel; out.surface[i] = p.surface;
+    out.state[i] = (uint8_t)p.state; out.bounces[i] = (uint8_t)p.b;
+}
+
+// Slab test of one segment against the two child boxes of a node.  px = -o*inv_d.  Boxes are padded
+// at build time, which is what makes this cheap fma form conservative with respect to tri_test.
+struct Slab { float ix, iy, iz, px, py, pz; };
+
+__device__ __forceinline__ Slab slab_setup(float ox, float oy, float oz, float dx, float dy, float dz) {
+    Slab s;
+    s.ix = __fdiv_rn(1.f, dx); s.iy = __fdiv_rn(1.f, dy); s.iz = __fdiv_rn(1.f, dz);
+    s.px = -ox * s.ix; s.py = -oy * s.iy; s.pz = -oz * s.iz;
+    return s;
+}
+
+// child 0: lo = (q0.x,q0.y,q0.z) hi = (q0.w,q1.x,q1.y); child 1: lo = (q1.z,q1.w,q2.x) hi = (q2.y,q2.z,q2.w).
+// tcap = t_best * (1 + 4e-7) (or a negative number for a lane that must not hit anything).
+__device__ __forceinline__ void slab2(const Slab& s, const float4 q0, const float4 q1, const float4 q2, float tcap,
+                                      float& n0, float& f0, float& n1, float& f1) {
+    float a, b;
+    a = __fmaf_rn(q0.x, s.ix, s.px); b = __fmaf_rn(q0.w, s.ix, s.px);
+    n0 = fminf(a, b); f0 = fmaxf(a, b);
+    a = __fmaf_rn(q0.y, s.iy, s.py); b = __fmaf_rn(q1.x, s.iy, s.py);
+    n0 = fmaxf(n0, fminf(a, b)); f0 = fminf(f0, fmaxf(a, b));
+    a = __fmaf_rn(q0.z, s.iz, s.pz); b = __fmaf_rn(q1.y, s.iz, s.pz);
+    n0 = fmaxf(n0, fminf(a, b)); f0 = fminf(f0, fmaxf(a, b));
+    a = __fmaf_rn(q1.z, s.ix, s.px); b = __fmaf_rn(q2.y, s.ix, s.px);
+    n1 = fminf(a, b); f1 = fmaxf(a, b);
+    a = __fmaf_rn(q1.w, s.iy, s.py); b = __fmaf_rn(q2.z, s.iy, s.py);
+    n1 = fmaxf(n1, fminf(a, b)); f1 = fminf(f1, fmaxf(a, b));
+    a = __fmaf_rn(q2.x, s.iz, s.pz); b = __fmaf_rn(q2.w, s.iz, s.pz);
+    n1 = fmaxf(n1, fminf(a, b)); f1 = fminf(f1, fmaxf(a, b));
+    n0 = fmaxf(n0, 0.f); n1 = fmaxf(n1, 0.f);
+    f0 = fminf(f0 * 1.0000004f, tcap); f1 = fminf(f1 * 1.0000004f, tcap);
+}
+
+}  // namespace opx

@@ -1,0 +1,247 @@
+// k_propagate_packet: the product kernel for A5-A10.
+//
+// One CTA owns a tile of kTile consecutive photons:
+//   1. stage   the tile's inputs are copied to shared memory with coalesced streaming loads;
+//   2. sort    photons are ordered by a 16-bit pseudo-angle of their direction about the tile's mean
+//              direction (Cherenkov photons of a track lie on a cone = a ring in the octahedral
+//              plane), with a 4-pass 4-bit radix sort in shared memory;
+//   3. trace   every warp takes groups of 32 neighbouring photons and walks the BVH as ONE packet:
+//              node loads are warp-uniform (one broadcast transaction instead of 32), control flow
+//              is uniform, and the traversal stack is shared by the warp and lives in the registers
+//              of its lanes (entry k in lane k, read back with a shuffle; entries >= 32 overflow to
+//              shared memory).  Each lane still intersects its own ray against every triangle the
+//              packet reaches, so results are exactly the per-photon results of DESIGN.md section 2;
+//   4. store   records are written back into the photon's own shared-memory slot and the tile is
+//              written out with coalesced streaming stores.
+#pragma once
+#include "opx_device.cuh"
+
+namespace opx {
+namespace {
+
+constexpr int kPktThreads = 512;
+constexpr int kPktWarps = kPktThreads / 32;          // 16
+constexpr int kTile = 2048;                          // photons per CTA tile
+constexpr int kItems = kTile / kPktThreads;          // 4
+constexpr int kPktStack = 96;                        // depth bound of the Karras tree (see opx_lane.cuh)
+constexpr int kStackSmem = kPktStack - 32;
+
+struct PacketSmem {
+    float o[kTile * 3];          // in: origins            out: hit positions
+    float d[kTile * 3];          // in: directions         out: arrival directions
+    float wl[kTile];             // in: wavelengths        out: pixel ids (int bits)
+    int surface[kTile];          // sort scratch (second key buffer), then out: surface ids
+    uint32_t key[kTile];         // (angle16 << 16) | index in tile, sorted in place (ping-pong with `surface`)
+    uint8_t state[kTile];
+    uint8_t bounces[kTile];
+    int stack[kPktWarps][kStackSmem];
+    uint32_t cnt[16][kPktWarps]; // radix: [digit][warp]
+    float red[kPktWarps][2];
+    float bcast[2];
+    uint32_t scan_tot[8];
+};
+
+// Octahedral map of a direction to [-1,1]^2 (NaN-safe: garbage maps to 0,0).
+__device__ __forceinline__ void octa(float dx, float dy, float dz, float& u, float& v) {
+    const float s = fabsf(dx) + fabsf(dy) + fabsf(dz);
+    const float inv = (s > 0.f && s < kInf) ? 1.f / s : 0.f;
+    u = dx * inv; v = dy * inv;
+    if (dz < 0.f) {
+        const float uu = (1.f - fabsf(v)) * (u >= 0.f ? 1.f : -1.f), vv = (1.f - fabsf(u)) * (v >= 0.f ? 1.f : -1.f);
+        u = uu; v = vv;
+    }
+    if (!(fabsf(u) <= 1.f)) u = 0.f;
+    if (!(fabsf(v) <= 1.f)) v = 0.f;
+}
+
+__device__ __forceinline__ float block_sum(PacketSmem& sm, float x, int slot) {
+    for (int off = 16; off > 0; off >>= 1) x += __shfl_xor_sync(0xffffffffu, x, off);
+    if ((threadIdx.x & 31) == 0) sm.red[threadIdx.x >> 5][slot] = x;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float r = 0.f;
+        for (int w = 0; w < kPktWarps; ++w) r += sm.red[w][slot];
+        sm.bcast[slot] = r;
+    }
+    __syncthreads();
+    return sm.bcast[slot];
+}
+
+// One stable 4-bit radix pass src -> dst over kTile packed keys.  Warp w owns the 32*kItems consecutive
+// entries [w*32*kItems, ...) and ranks them in kItems rounds with __match_any_sync.
+__device__ __forceinline__ void smem_radix_pass(PacketSmem& sm, const uint32_t* src, uint32_t* dst, int shift) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (threadIdx.x < 16 * kPktWarps) (&sm.cnt[0][0])[threadIdx.x] = 0;
+    __syncthreads();
+    uint32_t val[kItems], off[kItems];
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+        val[r] = src[w * (32 * kItems) + r * 32 + lane];
+        const uint32_t dgt = (val[r] >> shift) & 15u;
+        const uint32_t peers = __match_any_sync(0xffffffffu, dgt);
+        const int leader = __ffs(peers) - 1;
+        uint32_t old = 0;
+        if (lane == leader) { old = sm.cnt[dgt][w]; sm.cnt[dgt][w] = old + __popc(peers); }
+        old = __shfl_sync(0xffffffffu, old, leader);
+        off[r] = old + __popc(peers & ((1u << lane) - 1u));
+        __syncwarp();
+    }
+    __syncthreads();
+    // exclusive scan of the 16 x kPktWarps counters in (digit, warp) order: 256 values, 8 warps
+    if (threadIdx.x < 16 * kPktWarps) {
+        const uint32_t c = (&sm.cnt[0][0])[threadIdx.x];
+        uint32_t inc = c;
+        for (int o2 = 1; o2 < 32; o2 <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o2); if (lane >= o2) inc += y; }
+        if (lane == 31) sm.scan_tot[w] = inc;
+        (&sm.cnt[0][0])[threadIdx.x] = inc - c;
+    }
+    __syncthreads();
+    if (threadIdx.x < 16 * kPktWarps) {
+        uint32_t add = 0;
+        for (int k = 0; k < w; ++k) add += sm.scan_tot[k];
+        (&sm.cnt[0][0])[threadIdx.x] += add;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) dst[sm.cnt[(val[r] >> shift) & 15u][w] + off[r]] = val[r];
+    __syncthreads();
+}
+
+// Closest hit of 32 rays walked as one packet.  `alive` lanes carry a ray; the others follow along
+// without ever hitting anything.  All control flow is warp-uniform.
+__device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW& rw, const Slab& sl, float tmin, int last,
+                                                  bool alive, int lane, int* s_stack) {
+    Hit h{kInf, -1, 0x7fffffff};
+    float tcap = alive ? kInf : -1.f;
+    int stk = 0;            // entry `lane` of the warp's stack
+    int sp = 0, ref = 0;
+    for (;;) {
+        if (ref >= 0) {
+            const NodeDev* nd = sc.nodes + ref;
+            const float4 q0 = __ldg(&nd->q0), q1 = __ldg(&nd->q1), q2 = __ldg(&nd->q2);
+            const int4 q3 = __ldg(&nd->q3);
+            float n0, f0, n1, f1;
+            slab2(sl, q0, q1, q2, tcap, n0, f0, n1, f1);
+            const bool hit0 = n0 <= f0, hit1 = n1 <= f1;
+            const unsigned b0 = __ballot_sync(0xffffffffu, hit0), b1 = __ballot_sync(0xffffffffu, hit1);
+            if (b0 && b1) {
+                // order by majority vote of the lanes: a lane prefers child 1 if it enters it first
+                const unsigned p1 = __ballot_sync(0xffffffffu, hit1 && (!hit0 || n1 < n0));
+                const bool one_first = 2 * __popc(p1) > __popc(b0 | b1);
+                const int near = one_first ? q3.y : q3.x, far = one_first ? q3.x : q3.y;
+                if (sp < 32) { if (lane == sp) stk = far; } else s_stack[sp - 32] = far;
+                ++sp;
+                ref = near;
+                continue;
+            }
+            if (b0) { ref = q3.x; continue; }
+            if (b1) { ref = q3.y; continue; }
+        } else {
+            consider(sc, rw, ~ref, tmin, last, h);
+            if (alive) tcap = h.t * 1.0000004f;
+        }
+        if (sp == 0) break;
+        --sp;
+        ref = sp < 32 ? __shfl_sync(0xffffffffu, stk, sp) : s_stack[sp - 32];
+    }
+    return h;
+}
+
+__global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const SceneDev sc, uint64_t n, uint64_t id_base,
+                                                                     const float* __restrict__ origins,
+                                                                     const float* __restrict__ dirs,
+                                                                     const float* __restrict__ wl, uint64_t seed, opx_hits out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    PacketSmem& sm = *reinterpret_cast<PacketSmem*>(smem_raw);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const uint64_t tile_base = (uint64_t)blockIdx.x * kTile;
+    const int m = (int)min((uint64_t)kTile, n - tile_base);
+
+    // 1. stage the tile (coalesced, streaming: read once)
+    for (int k = threadIdx.x; k < 3 * m; k += kPktThreads) {
+        sm.o[k] = __ldcs(origins + 3 * tile_base + k);
+        sm.d[k] = __ldcs(dirs + 3 * tile_base + k);
+    }
+    for (int k = threadIdx.x; k < m; k += kPktThreads) sm.wl[k] = __ldcs(wl + tile_base + k);
+    __syncthreads();
+
+    // 2. sort key: 16-bit pseudo-angle about the tile's mean direction in the octahedral plane
+    {
+        float u[kItems], v[kItems];
+        float su = 0.f, sv = 0.f;
+#pragma unroll
+        for (int r = 0; r < kItems; ++r) {
+            const int i = r * kPktThreads + threadIdx.x;
+            u[r] = 0.f; v[r] = 0.f;
+            if (i < m) { octa(sm.d[3 * i], sm.d[3 * i + 1], sm.d[3 * i + 2], u[r], v[r]); su += u[r]; sv += v[r]; }
+        }
+        const float cu = block_sum(sm, su, 0) / (float)m, cv = block_sum(sm, sv, 1) / (float)m;
+#pragma unroll
+        for (int r = 0; r < kItems; ++r) {
+            const int i = r * kPktThreads + threadIdx.x;
+            uint32_t key = 0xffffu;
+            if (i < m) {
+                const float du = u[r] - cu, dv = v[r] - cv;
+                const float a = fabsf(du) + fabsf(dv);
+                const float pp = a > 0.f ? dv / a : 0.f;                     // diamond angle in [0,4)
+                const float ang = du >= 0.f ? (dv >= 0.f ? pp : 4.f + pp) : 2.f - pp;
+                key = min(65535u, (uint32_t)(ang * 16384.f));
+            }
+            sm.key[i] = (key << 16) | (uint32_t)i;
+        }
+        __syncthreads();
+        uint32_t* alt = reinterpret_cast<uint32_t*>(sm.surface);
+        smem_radix_pass(sm, sm.key, alt, 16);
+        smem_radix_pass(sm, alt, sm.key, 20);
+        smem_radix_pass(sm, sm.key, alt, 24);
+        smem_radix_pass(sm, alt, sm.key, 28);
+    }
+
+    // 3. each warp takes groups of 32 neighbouring photons and walks them as a packet
+    const int groups = (m + 31) >> 5;
+    for (int gidx = w; gidx < groups; gidx += kPktWarps) {
+        const int slot = gidx * 32 + lane;
+        bool alive = slot < m;
+        const bool valid = alive;
+        const int i = alive ? (int)(sm.key[slot] & 0xffffu) : 0;
+        Photon p;
+        photon_init(p, sm.o[3 * i], sm.o[3 * i + 1], sm.o[3 * i + 2], sm.d[3 * i], sm.d[3 * i + 1], sm.d[3 * i + 2], sm.wl[i],
+                    id_base + tile_base + (uint64_t)i);
+        while (__any_sync(0xffffffffu, alive)) {
+            const RayW rw = ray_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz);
+            const Slab sl = slab_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz);
+            const float tmin = p.b == 0 ? 0.f : sc.t_min;
+            const Hit h = closest_hit_packet(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]);
+            if (alive) alive = interact(sc, h, p, seed);
+        }
+        if (valid) {      // the photon's own slot: nobody else reads or writes it
+            sm.o[3 * i] = p.px; sm.o[3 * i + 1] = p.py; sm.o[3 * i + 2] = p.pz;
+            sm.d[3 * i] = p.dx; sm.d[3 * i + 1] = p.dy; sm.d[3 * i + 2] = p.dz;
+            sm.wl[i] = __int_as_float(p.pixel);
+            sm.surface[i] = p.surface;
+            sm.state[i] = (uint8_t)p.state; sm.bounces[i] = (uint8_t)p.b;
+        }
+    }
+    __syncthreads();
+
+    // 4. write the tile's records (coalesced, streaming)
+    for (int k = threadIdx.x; k < 3 * m; k += kPktThreads) {
+        __stcs(out.pos + 3 * tile_base + k, sm.o[k]);
+        __stcs(out.dir + 3 * tile_base + k, sm.d[k]);
+    }
+    for (int k = threadIdx.x; k < m; k += kPktThreads) {
+        __stcs(out.pixel + tile_base + k, __float_as_int(sm.wl[k]));
+        __stcs(out.surface + tile_base + k, sm.surface[k]);
+    }
+    if ((reinterpret_cast<uintptr_t>(out.state) & 3) == 0 && (reinterpret_cast<uintptr_t>(out.bounces) & 3) == 0 && (m & 3) == 0) {
+        for (int k = threadIdx.x; k < m / 4; k += kPktThreads) {      // tile_base is a multiple of 4
+            __stcs(reinterpret_cast<uint32_t*>(out.state + tile_base) + k, reinterpret_cast<const uint32_t*>(sm.state)[k]);
+            __stcs(reinterpret_cast<uint32_t*>(out.bounces + tile_base) + k, reinterpret_cast<const uint32_t*>(sm.bounces)[k]);
+        }
+    } else {
+        for (int k = threadIdx.x; k < m; k += kPktThreads) { out.state[tile_base + k] = sm.state[k]; out.bounces[tile_base + k] = sm.bounces[k]; }
+    }
+}
+
+}  // namespace
+}  // namespace opx

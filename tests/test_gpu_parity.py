@@ -274,7 +274,8 @@ def test_shared_edges_and_vertices_are_watertight(toy_flat):
     sc, gs = toy_flat
     v = sc.meshes[0]["vertices"].astype(np.float64)
     rng = np.random.default_rng(1)
-    pick = rng.choice(len(v), 4000, replace=False)
+    ii, jj = np.meshgrid(np.arange(2, 99), np.arange(2, 99))             # interior vertices of the 101x101 grid
+    pick = rng.choice((jj * 101 + ii).ravel(), 4000, replace=False)
     tgt = v[pick]
     tgt[2000:] = 0.5 * (tgt[2000:] + v[np.minimum(pick[2000:] + 1, len(v) - 1)])     # edge midpoints
     d = (tgt / np.linalg.norm(tgt, axis=1, keepdims=True)).astype(np.float32)
