@@ -15,8 +15,9 @@ __device__ __forceinline__ float philox_uniform(uint64_t seed, uint64_t g, uint3
     uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-        const uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
-        const uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+        const uint64_t p0 = (uint64_t)M0 * c0, p1 = (uint64_t)M1 * c2;     // one IMAD.WIDE each
+        const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
         const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
         c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
         k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
@@ -67,11 +68,10 @@ __device__ __forceinline__ RayW ray_setup(float ox, float oy, float oz, float dx
     return r;
 }
 
-// Contract triangle test.  Returns true with t when the triangle is hit at finite t > tmin.
-__device__ __forceinline__ bool tri_test(const RayW& r, const float4 a, const float4 b, const float4 c, float tmin, float& t_out) {
-    const float Akx = __fsub_rn(sel3(a.x, a.y, a.z, r.kx), r.okx), Aky = __fsub_rn(sel3(a.x, a.y, a.z, r.ky), r.oky), Akz = __fsub_rn(sel3(a.x, a.y, a.z, r.kz), r.okz);
-    const float Bkx = __fsub_rn(sel3(b.x, b.y, b.z, r.kx), r.okx), Bky = __fsub_rn(sel3(b.x, b.y, b.z, r.ky), r.oky), Bkz = __fsub_rn(sel3(b.x, b.y, b.z, r.kz), r.okz);
-    const float Ckx = __fsub_rn(sel3(c.x, c.y, c.z, r.kx), r.okx), Cky = __fsub_rn(sel3(c.x, c.y, c.z, r.ky), r.oky), Ckz = __fsub_rn(sel3(c.x, c.y, c.z, r.kz), r.okz);
+// Contract triangle test on vertex components already permuted to (kx, ky, kz) and shifted to the ray
+// origin (A = a - o, ...).  Returns true with t when the triangle is hit at finite t > tmin.
+__device__ __forceinline__ bool tri_test(const RayW& r, float Akx, float Aky, float Akz, float Bkx, float Bky, float Bkz,
+                                         float Ckx, float Cky, float Ckz, float tmin, float& t_out) {
     const float Ax = __fmaf_rn(-r.Sx, Akz, Akx), Ay = __fmaf_rn(-r.Sy, Akz, Aky);
     const float Bx = __fmaf_rn(-r.Sx, Bkz, Bkx), By = __fmaf_rn(-r.Sy, Bkz, Bky);
     const float Cx = __fmaf_rn(-r.Sx, Ckz, Ckx), Cy = __fmaf_rn(-r.Sy, Ckz, Cky);
@@ -104,14 +104,19 @@ __device__ __forceinline__ bool tri_test(const RayW& r, const float4 a, const fl
 
 struct Hit { float t; int j; int gid; };   // j: leaf-order index; gid: global triangle id
 
-// Tests leaf-order triangle j and keeps the lexicographic minimum of (t, global id).
+// Tests leaf-order triangle j and keeps the lexicographic minimum of (t, global id).  The vertex
+// components are fetched already permuted (per-lane offsets kx, ky, kz into the 48-byte record: the
+// lanes of a warp read the same sectors), so no register selects are needed.
 __device__ __forceinline__ void consider(const SceneDev& sc, const RayW& rw, int j, float tmin, int last, Hit& h) {
-    const float4 a = __ldg(sc.tris + 3 * (size_t)j), b = __ldg(sc.tris + 3 * (size_t)j + 1), c = __ldg(sc.tris + 3 * (size_t)j + 2);
-    const int gid = __float_as_int(a.w);
+    const float* t = reinterpret_cast<const float*>(sc.tris + 3 * (size_t)j);
+    const int gid = __float_as_int(__ldg(t + 3));
     if (gid == last) return;
-    float t;
-    if (!tri_test(rw, a, b, c, tmin, t)) return;
-    if (t < h.t || (t == h.t && gid < h.gid)) { h.t = t; h.j = j; h.gid = gid; }
+    const float Akx = __fsub_rn(__ldg(t + rw.kx), rw.okx), Aky = __fsub_rn(__ldg(t + rw.ky), rw.oky), Akz = __fsub_rn(__ldg(t + rw.kz), rw.okz);
+    const float Bkx = __fsub_rn(__ldg(t + 4 + rw.kx), rw.okx), Bky = __fsub_rn(__ldg(t + 4 + rw.ky), rw.oky), Bkz = __fsub_rn(__ldg(t + 4 + rw.kz), rw.okz);
+    const float Ckx = __fsub_rn(__ldg(t + 8 + rw.kx), rw.okx), Cky = __fsub_rn(__ldg(t + 8 + rw.ky), rw.oky), Ckz = __fsub_rn(__ldg(t + 8 + rw.kz), rw.okz);
+    float tt;
+    if (!tri_test(rw, Akx, Aky, Akz, Bkx, Bky, Bkz, Ckx, Cky, Ckz, tmin, tt)) return;
+    if (tt < h.t || (tt == h.t && gid < h.gid)) { h.t = tt; h.j = j; h.gid = gid; }
 }
 
 // ------------------------------------------------------------------- photon state + interaction
@@ -173,19 +178,21 @@ __device__ __forceinline__ void store_record(const opx_hits& out, uint64_t i, co
     out.state[i] = (uint8_t)p.state; out.bounces[i] = (uint8_t)p.b;
 }
 
-// Slab test of one segment against the two child boxes of a node.  px = -o*inv_d.  Boxes are padded
-// at build time, which is what makes this cheap fma form conservative with respect to tri_test.
+// Slab test of one segment against the two child boxes of a node.  px = -o*inv_d.  The boxes are
+// padded at build time by >= 128 ulp of the largest scene coordinate, which is what makes this cheap
+// form (approximate reciprocal, one fma per plane, no re-scaling of the exit distance) conservative
+// with respect to tri_test: its rounding error is a few ulp of that coordinate.
 struct Slab { float ix, iy, iz, px, py, pz; };
 
 __device__ __forceinline__ Slab slab_setup(float ox, float oy, float oz, float dx, float dy, float dz) {
     Slab s;
-    s.ix = __fdiv_rn(1.f, dx); s.iy = __fdiv_rn(1.f, dy); s.iz = __fdiv_rn(1.f, dz);
+    s.ix = __fdividef(1.f, dx); s.iy = __fdividef(1.f, dy); s.iz = __fdividef(1.f, dz);
     s.px = -ox * s.ix; s.py = -oy * s.iy; s.pz = -oz * s.iz;
     return s;
 }
 
 // child 0: lo = (q0.x,q0.y,q0.z) hi = (q0.w,q1.x,q1.y); child 1: lo = (q1.z,q1.w,q2.x) hi = (q2.y,q2.z,q2.w).
-// tcap = t_best * (1 + 4e-7) (or a negative number for a lane that must not hit anything).
+// tcap = t_best (or a negative number for a lane that must not hit anything).
 __device__ __forceinline__ void slab2(const Slab& s, const float4 q0, const float4 q1, const float4 q2, float tcap,
                                       float& n0, float& f0, float& n1, float& f1) {
     float a, b;
@@ -202,7 +209,25 @@ __device__ __forceinline__ void slab2(const Slab& s, const float4 q0, const floa
     a = __fmaf_rn(q2.x, s.iz, s.pz); b = __fmaf_rn(q2.w, s.iz, s.pz);
     n1 = fmaxf(n1, fminf(a, b)); f1 = fminf(f1, fmaxf(a, b));
     n0 = fmaxf(n0, 0.f); n1 = fmaxf(n1, 0.f);
-    f0 = fminf(f0 * 1.0000004f, tcap); f1 = fminf(f1 * 1.0000004f, tcap);
+    f0 = fminf(f0, tcap); f1 = fminf(f1, tcap);
+}
+
+// The same test when the signs of the direction components are known at compile time (kOct bit 0/1/2
+// set = dx/dy/dz negative): the entry plane of each axis is known, so no min/max per axis is needed.
+template <int kOct>
+__device__ __forceinline__ void slab2_oct(const Slab& s, const float4 q0, const float4 q1, const float4 q2, float tcap,
+                                          float& n0, float& f0, float& n1, float& f1) {
+    constexpr bool sx = kOct & 1, sy = kOct & 2, sz = kOct & 4;
+    const float lx0 = q0.x, ly0 = q0.y, lz0 = q0.z, hx0 = q0.w, hy0 = q1.x, hz0 = q1.y;
+    const float lx1 = q1.z, ly1 = q1.w, lz1 = q2.x, hx1 = q2.y, hy1 = q2.z, hz1 = q2.w;
+    n0 = fmaxf(fmaxf(__fmaf_rn(sx ? hx0 : lx0, s.ix, s.px), __fmaf_rn(sy ? hy0 : ly0, s.iy, s.py)),
+               fmaxf(__fmaf_rn(sz ? hz0 : lz0, s.iz, s.pz), 0.f));
+    f0 = fminf(fminf(__fmaf_rn(sx ? lx0 : hx0, s.ix, s.px), __fmaf_rn(sy ? ly0 : hy0, s.iy, s.py)),
+               fminf(__fmaf_rn(sz ? lz0 : hz0, s.iz, s.pz), tcap));
+    n1 = fmaxf(fmaxf(__fmaf_rn(sx ? hx1 : lx1, s.ix, s.px), __fmaf_rn(sy ? hy1 : ly1, s.iy, s.py)),
+               fmaxf(__fmaf_rn(sz ? hz1 : lz1, s.iz, s.pz), 0.f));
+    f1 = fminf(fminf(__fmaf_rn(sx ? lx1 : hx1, s.ix, s.px), __fmaf_rn(sy ? ly1 : hy1, s.iy, s.py)),
+               fminf(__fmaf_rn(sz ? lz1 : hz1, s.iz, s.pz), tcap));
 }
 
 }  // namespace opx

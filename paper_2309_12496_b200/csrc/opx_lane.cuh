@@ -26,7 +26,7 @@ __device__ __forceinline__ Hit closest_hit_lane(const SceneDev& sc, const RayW& 
             const float4 q0 = __ldg(&nd->q0), q1 = __ldg(&nd->q1), q2 = __ldg(&nd->q2);
             const int4 q3 = __ldg(&nd->q3);
             float n0, f0, n1, f1;
-            slab2(sl, q0, q1, q2, h.t * 1.0000004f, n0, f0, n1, f1);
+            slab2(sl, q0, q1, q2, h.t, n0, f0, n1, f1);
             const bool hit0 = n0 <= f0, hit1 = n1 <= f1;
             if (hit0 && hit1) {
                 int near = q3.x, far = q3.y;

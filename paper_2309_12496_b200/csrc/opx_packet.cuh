@@ -108,7 +108,9 @@ __device__ __forceinline__ void smem_radix_pass(PacketSmem& sm, const uint32_t* 
 }
 
 // Closest hit of 32 rays walked as one packet.  `alive` lanes carry a ray; the others follow along
-// without ever hitting anything.  All control flow is warp-uniform.
+// without ever hitting anything.  All control flow is warp-uniform.  kOct = 0..7: every alive lane's
+// direction lies in that sign octant (specialised slab test); kOct = 8: mixed signs (generic test).
+template <int kOct>
 __device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW& rw, const Slab& sl, float tmin, int last,
                                                   bool alive, int lane, int* s_stack) {
     Hit h{kInf, -1, 0x7fffffff};
@@ -121,7 +123,8 @@ __device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW
             const float4 q0 = __ldg(&nd->q0), q1 = __ldg(&nd->q1), q2 = __ldg(&nd->q2);
             const int4 q3 = __ldg(&nd->q3);
             float n0, f0, n1, f1;
-            slab2(sl, q0, q1, q2, tcap, n0, f0, n1, f1);
+            if (kOct < 8) slab2_oct<kOct>(sl, q0, q1, q2, tcap, n0, f0, n1, f1);
+            else slab2(sl, q0, q1, q2, tcap, n0, f0, n1, f1);
             const bool hit0 = n0 <= f0, hit1 = n1 <= f1;
             const unsigned b0 = __ballot_sync(0xffffffffu, hit0), b1 = __ballot_sync(0xffffffffu, hit1);
             if (b0 && b1) {
@@ -138,7 +141,7 @@ __device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW
             if (b1) { ref = q3.y; continue; }
         } else {
             consider(sc, rw, ~ref, tmin, last, h);
-            if (alive) tcap = h.t * 1.0000004f;
+            if (alive) tcap = h.t;
         }
         if (sp == 0) break;
         --sp;
@@ -211,7 +214,23 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
             const RayW rw = ray_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz);
             const Slab sl = slab_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz);
             const float tmin = p.b == 0 ? 0.f : sc.t_min;
-            const Hit h = closest_hit_packet(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]);
+            // sign octant of the packet: specialised traversal when all alive lanes agree
+            const int oct = (p.dx < 0.f ? 1 : 0) | (p.dy < 0.f ? 2 : 0) | (p.dz < 0.f ? 4 : 0);
+            const unsigned am = __ballot_sync(0xffffffffu, alive);
+            const int oct0 = __shfl_sync(0xffffffffu, oct, __ffs(am) - 1);
+            const bool uni = __all_sync(0xffffffffu, !alive || oct == oct0);
+            Hit h;
+            switch (uni ? oct0 : 8) {
+                case 0: h = closest_hit_packet<0>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
+                case 1: h = closest_hit_packet<1>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
+                case 2: h = closest_hit_packet<2>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
+                case 3: h = closest_hit_packet<3>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
+                case 4: h = closest_hit_packet<4>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
+                case 5: h = closest_hit_packet<5>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
+                case 6: h = closest_hit_packet<6>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
+                case 7: h = closest_hit_packet<7>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
+                default: h = closest_hit_packet<8>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
+            }
             if (alive) alive = interact(sc, h, p, seed);
         }
         if (valid) {      // the photon's own slot: nobody else reads or writes it
