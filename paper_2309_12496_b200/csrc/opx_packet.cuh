@@ -26,20 +26,25 @@ constexpr int kItems = kTile / kPktThreads;          // 4
 constexpr int kPktStack = 96;                        // depth bound of the Karras tree (see opx_lane.cuh)
 constexpr int kStackSmem = kPktStack - 32;
 
+constexpr int kRadixBits = 6, kRadix = 1 << kRadixBits;      // 2 passes over the 12-bit key
+
 struct PacketSmem {
     float o[kTile * 3];          // in: origins            out: hit positions
     float d[kTile * 3];          // in: directions         out: arrival directions
     float wl[kTile];             // in: wavelengths        out: pixel ids (int bits)
     int surface[kTile];          // sort scratch (second key buffer), then out: surface ids
-    uint32_t key[kTile];         // (angle16 << 16) | index in tile, sorted in place (ping-pong with `surface`)
+    uint32_t key[kTile];         // (angle12 << 16) | index in tile, sorted (ping-pong with `surface`)
     uint8_t state[kTile];
     uint8_t bounces[kTile];
-    int stack[kPktWarps][kStackSmem];
-    uint32_t cnt[16][kPktWarps]; // radix: [digit][warp]
+    union {
+        int stack[kPktWarps][kStackSmem];        // traversal: stack entries >= 32 of each warp
+        uint32_t cnt[kRadix][kPktWarps];         // sort: radix counters [digit][warp]
+    };
     float red[kPktWarps][2];
     float bcast[2];
-    uint32_t scan_tot[8];
+    uint32_t scan_tot[kPktWarps];
 };
+static_assert(sizeof(int) * kStackSmem >= sizeof(uint32_t) * kRadix, "radix counters alias the stack overflow area");
 
 // Octahedral map of a direction to [-1,1]^2 (NaN-safe: garbage maps to 0,0).
 __device__ __forceinline__ void octa(float dx, float dy, float dz, float& u, float& v) {
@@ -54,30 +59,35 @@ __device__ __forceinline__ void octa(float dx, float dy, float dz, float& u, flo
     if (!(fabsf(v) <= 1.f)) v = 0.f;
 }
 
-__device__ __forceinline__ float block_sum(PacketSmem& sm, float x, int slot) {
-    for (int off = 16; off > 0; off >>= 1) x += __shfl_xor_sync(0xffffffffu, x, off);
-    if ((threadIdx.x & 31) == 0) sm.red[threadIdx.x >> 5][slot] = x;
+__device__ __forceinline__ void block_sum2(PacketSmem& sm, float x, float y, float& sx, float& sy) {
+    for (int off = 16; off > 0; off >>= 1) { x += __shfl_xor_sync(0xffffffffu, x, off); y += __shfl_xor_sync(0xffffffffu, y, off); }
+    if ((threadIdx.x & 31) == 0) { sm.red[threadIdx.x >> 5][0] = x; sm.red[threadIdx.x >> 5][1] = y; }
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (threadIdx.x < 2) {
         float r = 0.f;
-        for (int w = 0; w < kPktWarps; ++w) r += sm.red[w][slot];
-        sm.bcast[slot] = r;
+        for (int w = 0; w < kPktWarps; ++w) r += sm.red[w][threadIdx.x];
+        sm.bcast[threadIdx.x] = r;
     }
     __syncthreads();
-    return sm.bcast[slot];
+    sx = sm.bcast[0]; sy = sm.bcast[1];
 }
 
-// One stable 4-bit radix pass src -> dst over kTile packed keys.  Warp w owns the 32*kItems consecutive
-// entries [w*32*kItems, ...) and ranks them in kItems rounds with __match_any_sync.
+// One stable radix pass (kRadixBits bits) src -> dst over kTile packed keys.  Warp w owns the
+// 32*kItems consecutive entries [w*32*kItems, ...) and ranks them in kItems rounds with
+// __match_any_sync; the kRadix x kPktWarps counters are scanned in (digit, warp) order.
 __device__ __forceinline__ void smem_radix_pass(PacketSmem& sm, const uint32_t* src, uint32_t* dst, int shift) {
+    constexpr int kCnt = kRadix * kPktWarps, kPer = kCnt / kPktThreads;   // 1024 counters, 2 per thread
+    static_assert(kCnt % kPktThreads == 0, "counter scan layout");
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    if (threadIdx.x < 16 * kPktWarps) (&sm.cnt[0][0])[threadIdx.x] = 0;
+    uint32_t* cnt = &sm.cnt[0][0];
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) cnt[k * kPktThreads + threadIdx.x] = 0;
     __syncthreads();
     uint32_t val[kItems], off[kItems];
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
         val[r] = src[w * (32 * kItems) + r * 32 + lane];
-        const uint32_t dgt = (val[r] >> shift) & 15u;
+        const uint32_t dgt = (val[r] >> shift) & (kRadix - 1);
         const uint32_t peers = __match_any_sync(0xffffffffu, dgt);
         const int leader = __ffs(peers) - 1;
         uint32_t old = 0;
@@ -87,23 +97,22 @@ __device__ __forceinline__ void smem_radix_pass(PacketSmem& sm, const uint32_t* 
         __syncwarp();
     }
     __syncthreads();
-    // exclusive scan of the 16 x kPktWarps counters in (digit, warp) order: 256 values, 8 warps
-    if (threadIdx.x < 16 * kPktWarps) {
-        const uint32_t c = (&sm.cnt[0][0])[threadIdx.x];
-        uint32_t inc = c;
+    {   // exclusive scan: thread t owns counters [t*kPer, t*kPer + kPer)
+        uint32_t c[kPer], sum = 0;
+#pragma unroll
+        for (int k = 0; k < kPer; ++k) { c[k] = cnt[threadIdx.x * kPer + k]; sum += c[k]; }
+        uint32_t inc = sum;
         for (int o2 = 1; o2 < 32; o2 <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o2); if (lane >= o2) inc += y; }
         if (lane == 31) sm.scan_tot[w] = inc;
-        (&sm.cnt[0][0])[threadIdx.x] = inc - c;
-    }
-    __syncthreads();
-    if (threadIdx.x < 16 * kPktWarps) {
-        uint32_t add = 0;
-        for (int k = 0; k < w; ++k) add += sm.scan_tot[k];
-        (&sm.cnt[0][0])[threadIdx.x] += add;
+        __syncthreads();
+        uint32_t run = inc - sum;
+        for (int k = 0; k < w; ++k) run += sm.scan_tot[k];
+#pragma unroll
+        for (int k = 0; k < kPer; ++k) { cnt[threadIdx.x * kPer + k] = run; run += c[k]; }
     }
     __syncthreads();
 #pragma unroll
-    for (int r = 0; r < kItems; ++r) dst[sm.cnt[(val[r] >> shift) & 15u][w] + off[r]] = val[r];
+    for (int r = 0; r < kItems; ++r) dst[sm.cnt[(val[r] >> shift) & (kRadix - 1)][w] + off[r]] = val[r];
     __syncthreads();
 }
 
@@ -160,15 +169,29 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
     const uint64_t tile_base = (uint64_t)blockIdx.x * kTile;
     const int m = (int)min((uint64_t)kTile, n - tile_base);
 
-    // 1. stage the tile (coalesced, streaming: read once)
-    for (int k = threadIdx.x; k < 3 * m; k += kPktThreads) {
-        sm.o[k] = __ldcs(origins + 3 * tile_base + k);
-        sm.d[k] = __ldcs(dirs + 3 * tile_base + k);
+    // 1. stage the tile (coalesced, streaming: read once); 16-byte loads for full, aligned tiles
+    const bool vec = m == kTile && ((reinterpret_cast<uintptr_t>(origins) | reinterpret_cast<uintptr_t>(dirs) |
+                                     reinterpret_cast<uintptr_t>(wl)) & 15) == 0;
+    if (vec) {
+        const float4* go = reinterpret_cast<const float4*>(origins + 3 * tile_base);
+        const float4* gd = reinterpret_cast<const float4*>(dirs + 3 * tile_base);
+        const float4* gw = reinterpret_cast<const float4*>(wl + tile_base);
+#pragma unroll
+        for (int k = 0; k < 3 * kTile / 4 / kPktThreads; ++k) {
+            reinterpret_cast<float4*>(sm.o)[k * kPktThreads + threadIdx.x] = __ldcs(go + k * kPktThreads + threadIdx.x);
+            reinterpret_cast<float4*>(sm.d)[k * kPktThreads + threadIdx.x] = __ldcs(gd + k * kPktThreads + threadIdx.x);
+        }
+        reinterpret_cast<float4*>(sm.wl)[threadIdx.x] = __ldcs(gw + threadIdx.x);
+    } else {
+        for (int k = threadIdx.x; k < 3 * m; k += kPktThreads) {
+            sm.o[k] = __ldcs(origins + 3 * tile_base + k);
+            sm.d[k] = __ldcs(dirs + 3 * tile_base + k);
+        }
+        for (int k = threadIdx.x; k < m; k += kPktThreads) sm.wl[k] = __ldcs(wl + tile_base + k);
     }
-    for (int k = threadIdx.x; k < m; k += kPktThreads) sm.wl[k] = __ldcs(wl + tile_base + k);
     __syncthreads();
 
-    // 2. sort key: 16-bit pseudo-angle about the tile's mean direction in the octahedral plane
+    // 2. sort key: 12-bit pseudo-angle about the tile's mean direction in the octahedral plane
     {
         float u[kItems], v[kItems];
         float su = 0.f, sv = 0.f;
@@ -178,26 +201,26 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
             u[r] = 0.f; v[r] = 0.f;
             if (i < m) { octa(sm.d[3 * i], sm.d[3 * i + 1], sm.d[3 * i + 2], u[r], v[r]); su += u[r]; sv += v[r]; }
         }
-        const float cu = block_sum(sm, su, 0) / (float)m, cv = block_sum(sm, sv, 1) / (float)m;
+        float cu, cv;
+        block_sum2(sm, su, sv, cu, cv);
+        cu /= (float)m; cv /= (float)m;
 #pragma unroll
         for (int r = 0; r < kItems; ++r) {
             const int i = r * kPktThreads + threadIdx.x;
-            uint32_t key = 0xffffu;
+            uint32_t key = 0xfffu;
             if (i < m) {
                 const float du = u[r] - cu, dv = v[r] - cv;
                 const float a = fabsf(du) + fabsf(dv);
                 const float pp = a > 0.f ? dv / a : 0.f;                     // diamond angle in [0,4)
                 const float ang = du >= 0.f ? (dv >= 0.f ? pp : 4.f + pp) : 2.f - pp;
-                key = min(65535u, (uint32_t)(ang * 16384.f));
+                key = min(4095u, (uint32_t)(ang * 1024.f));
             }
             sm.key[i] = (key << 16) | (uint32_t)i;
         }
         __syncthreads();
         uint32_t* alt = reinterpret_cast<uint32_t*>(sm.surface);
         smem_radix_pass(sm, sm.key, alt, 16);
-        smem_radix_pass(sm, alt, sm.key, 20);
-        smem_radix_pass(sm, sm.key, alt, 24);
-        smem_radix_pass(sm, alt, sm.key, 28);
+        smem_radix_pass(sm, alt, sm.key, 22);
     }
 
     // 3. each warp takes groups of 32 neighbouring photons and walks them as a packet
