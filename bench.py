@@ -157,8 +157,12 @@ def main():
     if args.photons:
         w = workloads.make_config(args.config, n=max(w.n, args.photons * world))
     id_base = rank * n if (rank + 1) * n <= w.n else 0
-    o, d, lam = w.photon_range(id_base, id_base + n)
-    pin = [torch.from_numpy(x).pin_memory() for x in (o, d, lam)]
+    pin = [torch.empty((n, 3), dtype=torch.float32).pin_memory(), torch.empty((n, 3), dtype=torch.float32).pin_memory(),
+           torch.empty(n, dtype=torch.float32).pin_memory()]
+    for a in range(0, n, 5_000_000):                                  # generate in slices to bound host memory
+        b = min(n, a + 5_000_000)
+        for dst, src in zip(pin, w.photon_range(id_base + a, id_base + b)):
+            dst[a:b] = torch.from_numpy(src)
     d_o, d_d, d_l = (x.to(dev, non_blocking=True) for x in pin)
     stream = torch.cuda.current_stream(dev)
 

@@ -217,7 +217,7 @@ def _hex_fan(k):
     return np.array(pts), np.array(tris, dtype=np.uint32)
 
 
-def lhcb_like_scene(enclosure_pitch=12.9, edge=5.0):
+def lhcb_like_scene(enclosure_pitch=11.3, edge=5.0, th1=0.40, d1=900.0, d2=455.0):
     """BASELINE.json config 3: an LHCb-RICH1-like scene of ~1e6 triangles.
 
     Two mirror-symmetric halves (sigma = +-1 in y).  Per half: two spherical primary-mirror
@@ -227,6 +227,10 @@ def lhcb_like_scene(enclosure_pitch=12.9, edge=5.0):
     pixels.  Absorbing backing plates 1 mm behind every mirror tile and an absorbing box
     tessellated at `enclosure_pitch` bring the scene to ~1e6 triangles.  Positions are
     this build's choice (the config gives counts and radii only); see DESIGN.md.
+    th1 = tilt of each primary half about x, d1 = primary vertex -> flat mirror centre,
+    d2 = flat mirror centre -> detector plane; the defaults keep the flat mirrors outside the
+    250 + 53 mrad light cone of the tracks, so that ~63 % of C3-style photons reach a detector
+    plane after two reflections (checked with the oracle).
     """
     sc = Scene()
     refl, qe = c2_tables()
@@ -235,7 +239,6 @@ def lhcb_like_scene(enclosure_pitch=12.9, edge=5.0):
     m_det = sc.add_material(MAT_DETECTOR, qe)
 
     R, V = 2710.0, np.array([0.0, 0.0, 1400.0])
-    th1 = 0.30
     ex = np.array([1.0, 0.0, 0.0])
     r_hex = 88.0
     k = int(np.ceil(r_hex / edge))
@@ -265,7 +268,7 @@ def lhcb_like_scene(enclosure_pitch=12.9, edge=5.0):
         # ---- secondary flat mirror: 4 x 2 tiles of 380 x 350 mm on a 5 mm grid
         r1 = np.array([0.0, sigma * np.sin(2 * th1), -np.cos(2 * th1)])
         r2 = np.array([0.0, sigma * np.cos(th1), np.sin(th1)])
-        M = V + 800.0 * r1
+        M = V + d1 * r1
         n = (r1 - r2) / np.linalg.norm(r1 - r2)       # faces the incoming light (n . r1 > 0 side is the back)
         e1 = ex
         e2 = np.cross(n, e1)
@@ -277,7 +280,7 @@ def lhcb_like_scene(enclosure_pitch=12.9, edge=5.0):
                 sc.add_mesh("secondary_backing", fv + 1.0 * n, ft, m_abs)
                 allv.append(fv)
         # ---- detector plane: 25 x 20 modules of 64 mm, each its own surface + pixel frame
-        D = M + 555.0 * r2
+        D = M + d2 * r2
         du = ex
         dv = np.cross(-r2, du)
         halfgrid = 4 * PIXEL_PITCH_MM
