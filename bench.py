@@ -152,11 +152,11 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
 
+    from paper_2309_12496_b200.sharding import allreduce_accumulators, shard_range
     w = workloads.make_config(args.config, n=None)
-    n = args.photons if args.photons else min(w.n, 100_000_000)       # per GPU per step
-    if args.photons:
-        w = workloads.make_config(args.config, n=max(w.n, args.photons * world))
-    id_base = rank * n if (rank + 1) * n <= w.n else 0
+    n = args.photons if args.photons else min(w.n, 100_000_000)       # per GPU per step (weak scaling)
+    w = workloads.make_config(args.config, n=max(w.n, n * world))     # the job: world * n photons, ids 0..world*n
+    id_base, n = shard_range(n * world, rank, world)                  # contiguous global id range of this rank
     pin = [torch.empty((n, 3), dtype=torch.float32).pin_memory(), torch.empty((n, 3), dtype=torch.float32).pin_memory(),
            torch.empty(n, dtype=torch.float32).pin_memory()]
     for a in range(0, n, 5_000_000):                                  # generate in slices to bound host memory
@@ -186,8 +186,7 @@ def main():
         hitmap.zero_(); counters.zero_()
         scene.propagate(d_o, d_d, d_l, seed=args.seed, photon_id_base=id_base, records=records, hitmap=hitmap,
                         counters=counters, stream=stream)
-        if dist is not None:
-            dist.all_reduce(hitmap); dist.all_reduce(counters)
+        allreduce_accumulators(hitmap, counters)                      # the one exchange step (no-op at N = 1)
 
     for _ in range(args.warmup):
         step()

@@ -1,0 +1,62 @@
+"""World-size-2 gloo test of the multi-GPU host logic (no GPU needed): contiguous id shards +
+one sum all-reduce of hit-map and counters reproduce the single-rank result exactly.  The per-shard
+records come from the oracle here (the CUDA path cannot run on CPU); what is under test is
+paper_2309_12496_b200.sharding and the keying of the random stream by the global photon id."""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+import oracle
+import workloads as wl
+from paper_2309_12496_b200.sharding import allreduce_accumulators, shard_range
+
+
+def test_shard_range_tiles_exactly():
+    for n, world in [(10, 3), (7, 8), (10_000_000, 8), (0, 2), (5, 1)]:
+        spans = [shard_range(n, r, world) for r in range(world)]
+        assert spans[0][0] == 0 and sum(c for _, c in spans) == n
+        for (s0, c0), (s1, _) in zip(spans, spans[1:]):
+            assert s0 + c0 == s1
+        counts = [c for _, c in spans]
+        assert max(counts) - min(counts) <= 1
+    with pytest.raises(ValueError):
+        shard_range(10, 2, 2)
+
+
+def _worker(rank, world, port, n_total, seed, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    w = wl.make_config("C3", n=600_000)
+    start, count = shard_range(n_total, rank, world)
+    o, d, lam = w.photon_range(300_000 + start, 300_000 + start + count)
+    r = oracle.trace_mesh(w.scene, o, d, lam, seed=seed, id_base=300_000 + start, n_threads=2)
+    hitmap = torch.from_numpy(r["hitmap"].astype(np.int32))
+    counters = torch.from_numpy(r["counters"].astype(np.int64))
+    allreduce_accumulators(hitmap, counters)
+    np.save(os.path.join(out_dir, f"state_{rank}.npy"), r["state"])
+    if rank == 0:
+        np.save(os.path.join(out_dir, "hitmap.npy"), hitmap.numpy())
+        np.save(os.path.join(out_dir, "counters.npy"), counters.numpy())
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_shards_reproduce_single_rank(tmp_path):
+    n_total, seed, world = 3001, 13, 2
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    mp.spawn(_worker, args=(world, port, n_total, seed, str(tmp_path)), nprocs=world, join=True)
+    w = wl.make_config("C3", n=600_000)
+    o, d, lam = w.photon_range(300_000, 300_000 + n_total)
+    ref = oracle.trace_mesh(w.scene, o, d, lam, seed=seed, id_base=300_000)
+    state = np.concatenate([np.load(tmp_path / f"state_{r}.npy") for r in range(world)])
+    assert np.array_equal(state, ref["state"])
+    assert np.array_equal(np.load(tmp_path / "hitmap.npy").astype(np.uint32), ref["hitmap"])
+    assert np.array_equal(np.load(tmp_path / "counters.npy").astype(np.uint64), ref["counters"])
+    assert ref["hitmap"].sum() > 0
