@@ -2,9 +2,9 @@
 //
 // One CTA owns a tile of kTile consecutive photons:
 //   1. stage   the tile's inputs are copied to shared memory with coalesced streaming loads;
-//   2. sort    photons are ordered by a 16-bit pseudo-angle of their direction about the tile's mean
+//   2. sort    photons are ordered by a 12-bit pseudo-angle of their direction about the tile's mean
 //              direction (Cherenkov photons of a track lie on a cone = a ring in the octahedral
-//              plane), with a 4-pass 4-bit radix sort in shared memory;
+//              plane), with a 2-pass 6-bit radix sort in shared memory;
 //   3. trace   every warp takes groups of 32 neighbouring photons and walks the BVH as ONE packet:
 //              node loads are warp-uniform (one broadcast transaction instead of 32), control flow
 //              is uniform, and the traversal stack is shared by the warp and lives in the registers
