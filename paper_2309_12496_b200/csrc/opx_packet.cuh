@@ -119,42 +119,67 @@ __device__ __forceinline__ void smem_radix_pass(PacketSmem& sm, const uint32_t* 
 // Closest hit of 32 rays walked as one packet.  `alive` lanes carry a ray; the others follow along
 // without ever hitting anything.  All control flow is warp-uniform.  kOct = 0..7: every alive lane's
 // direction lies in that sign octant (specialised slab test); kOct = 8: mixed signs (generic test).
+struct PacketStack { int stk = 0, sp = 0; };   // stk: entry `lane` of the warp's stack (entries >= 32 in shared memory)
+
+constexpr int kDone = 0x7fffffff;
+
+// Walks internal nodes from `ref` until the packet reaches a leaf (returns its ref < 0) or the
+// traversal is finished (returns kDone).  This small loop is the only code specialised per octant.
 template <int kOct>
+__device__ __forceinline__ int descend(const SceneDev& sc, const Slab& sl, float tcap, int ref, PacketStack& st, int lane, int* s_stack) {
+    for (;;) {
+        if (ref < 0) return ref;
+        const NodeDev* nd = sc.nodes + ref;
+        const float4 q0 = __ldg(&nd->q0), q1 = __ldg(&nd->q1), q2 = __ldg(&nd->q2);
+        const int4 q3 = __ldg(&nd->q3);
+        float n0, f0, n1, f1;
+        if (kOct < 8) slab2_oct<kOct>(sl, q0, q1, q2, tcap, n0, f0, n1, f1);
+        else slab2(sl, q0, q1, q2, tcap, n0, f0, n1, f1);
+        const bool hit0 = n0 <= f0, hit1 = n1 <= f1;
+        const unsigned b0 = __ballot_sync(0xffffffffu, hit0), b1 = __ballot_sync(0xffffffffu, hit1);
+        if (b0 && b1) {
+            // order by majority vote of the lanes: a lane prefers child 1 if it enters it first
+            const unsigned p1 = __ballot_sync(0xffffffffu, hit1 && (!hit0 || n1 < n0));
+            const bool one_first = 2 * __popc(p1) > __popc(b0 | b1);
+            const int far = one_first ? q3.x : q3.y;
+            if (st.sp < 32) { if (lane == st.sp) st.stk = far; } else s_stack[st.sp - 32] = far;
+            ++st.sp;
+            ref = one_first ? q3.y : q3.x;
+            continue;
+        }
+        if (b0) { ref = q3.x; continue; }
+        if (b1) { ref = q3.y; continue; }
+        if (st.sp == 0) return kDone;
+        --st.sp;
+        ref = st.sp < 32 ? __shfl_sync(0xffffffffu, st.stk, st.sp) : s_stack[st.sp - 32];
+    }
+}
+
+// `oct` (warp-uniform) = 0..7: every alive lane's direction lies in that sign octant; 8: mixed signs.
 __device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW& rw, const Slab& sl, float tmin, int last,
-                                                  bool alive, int lane, int* s_stack) {
+                                                  bool alive, int lane, int* s_stack, int oct) {
     Hit h{kInf, -1, 0x7fffffff};
     float tcap = alive ? kInf : -1.f;
-    int stk = 0;            // entry `lane` of the warp's stack
-    int sp = 0, ref = 0;
+    PacketStack st;
+    int ref = 0;
     for (;;) {
-        if (ref >= 0) {
-            const NodeDev* nd = sc.nodes + ref;
-            const float4 q0 = __ldg(&nd->q0), q1 = __ldg(&nd->q1), q2 = __ldg(&nd->q2);
-            const int4 q3 = __ldg(&nd->q3);
-            float n0, f0, n1, f1;
-            if (kOct < 8) slab2_oct<kOct>(sl, q0, q1, q2, tcap, n0, f0, n1, f1);
-            else slab2(sl, q0, q1, q2, tcap, n0, f0, n1, f1);
-            const bool hit0 = n0 <= f0, hit1 = n1 <= f1;
-            const unsigned b0 = __ballot_sync(0xffffffffu, hit0), b1 = __ballot_sync(0xffffffffu, hit1);
-            if (b0 && b1) {
-                // order by majority vote of the lanes: a lane prefers child 1 if it enters it first
-                const unsigned p1 = __ballot_sync(0xffffffffu, hit1 && (!hit0 || n1 < n0));
-                const bool one_first = 2 * __popc(p1) > __popc(b0 | b1);
-                const int near = one_first ? q3.y : q3.x, far = one_first ? q3.x : q3.y;
-                if (sp < 32) { if (lane == sp) stk = far; } else s_stack[sp - 32] = far;
-                ++sp;
-                ref = near;
-                continue;
-            }
-            if (b0) { ref = q3.x; continue; }
-            if (b1) { ref = q3.y; continue; }
-        } else {
-            consider(sc, rw, ~ref, tmin, last, h);
-            if (alive) tcap = h.t;
+        switch (oct) {
+            case 0: ref = descend<0>(sc, sl, tcap, ref, st, lane, s_stack); break;
+            case 1: ref = descend<1>(sc, sl, tcap, ref, st, lane, s_stack); break;
+            case 2: ref = descend<2>(sc, sl, tcap, ref, st, lane, s_stack); break;
+            case 3: ref = descend<3>(sc, sl, tcap, ref, st, lane, s_stack); break;
+            case 4: ref = descend<4>(sc, sl, tcap, ref, st, lane, s_stack); break;
+            case 5: ref = descend<5>(sc, sl, tcap, ref, st, lane, s_stack); break;
+            case 6: ref = descend<6>(sc, sl, tcap, ref, st, lane, s_stack); break;
+            case 7: ref = descend<7>(sc, sl, tcap, ref, st, lane, s_stack); break;
+            default: ref = descend<8>(sc, sl, tcap, ref, st, lane, s_stack); break;
         }
-        if (sp == 0) break;
-        --sp;
-        ref = sp < 32 ? __shfl_sync(0xffffffffu, stk, sp) : s_stack[sp - 32];
+        if (ref == kDone) break;
+        consider(sc, rw, ~ref, tmin, last, h);
+        if (alive) tcap = h.t;
+        if (st.sp == 0) break;
+        --st.sp;
+        ref = st.sp < 32 ? __shfl_sync(0xffffffffu, st.stk, st.sp) : s_stack[st.sp - 32];
     }
     return h;
 }
@@ -242,18 +267,7 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
             const unsigned am = __ballot_sync(0xffffffffu, alive);
             const int oct0 = __shfl_sync(0xffffffffu, oct, __ffs(am) - 1);
             const bool uni = __all_sync(0xffffffffu, !alive || oct == oct0);
-            Hit h;
-            switch (uni ? oct0 : 8) {
-                case 0: h = closest_hit_packet<0>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
-                case 1: h = closest_hit_packet<1>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
-                case 2: h = closest_hit_packet<2>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
-                case 3: h = closest_hit_packet<3>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
-                case 4: h = closest_hit_packet<4>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
-                case 5: h = closest_hit_packet<5>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
-                case 6: h = closest_hit_packet<6>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
-                case 7: h = closest_hit_packet<7>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
-                default: h = closest_hit_packet<8>(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w]); break;
-            }
+            const Hit h = closest_hit_packet(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w], uni ? oct0 : 8);
             if (alive) alive = interact(sc, h, p, seed);
         }
         if (valid) {      // the photon's own slot: nobody else reads or writes it
