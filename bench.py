@@ -75,14 +75,14 @@ class ClockSampler(threading.Thread):
                     reasons=reasons, samples=len(sm))
 
 
-def time_oracle(workload, n_sample, seed, repeats=1):
+def time_oracle(workload, n_sample, seed, repeats=1, n_threads=None):
     """The oracle as it stands on the host cores, on the first n_sample photon ids of the workload."""
     import oracle
     o, d, lam = workload.photon_range(0, n_sample)
     best = None
     for _ in range(repeats):
         t0 = time.perf_counter()
-        r = oracle.trace_mesh(workload.scene, o, d, lam, seed=seed)
+        r = oracle.trace_mesh(workload.scene, o, d, lam, seed=seed, n_threads=n_threads)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
     return n_sample / best, r["n_threads"], best, int(r["counters"][7])
@@ -118,6 +118,44 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def run_sweep(args, scene, photons, records, hitmap, counters, n, stream, w, pkg):
+    """BASELINE.json config 4: photons/s and achieved HBM GB/s versus chunk size.  The resident batch of
+    n photons is streamed repeatedly (global ids keep advancing, so every pass draws new random
+    numbers) until --total photons have gone through, in calls of `chunk` photons each."""
+    import torch
+    d_o, d_d, d_l = photons
+    rows = []
+    for chunk in [int(c) for c in args.chunks.split(",") if int(c) <= n]:
+        def one_pass(base):
+            for a in range(0, n - chunk + 1, chunk):
+                rec = {k: v[a:a + chunk] for k, v in records.items()}
+                scene.propagate(d_o[a:a + chunk], d_d[a:a + chunk], d_l[a:a + chunk], seed=args.seed, photon_id_base=base + a,
+                                records=rec, hitmap=hitmap, counters=counters, stream=stream)
+        per_pass = (n // chunk) * chunk
+        passes = max(1, min(args.total // per_pass, 50))
+        hitmap.zero_(); counters.zero_()
+        one_pass(0)                                                    # warm-up
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = pkg.launch_count()
+        ev0.record(stream)
+        for p in range(passes):
+            one_pass((p + 1) * per_pass)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        ms = ev0.elapsed_time(ev1)
+        done = passes * per_pass
+        rows.append({"chunk": chunk, "photons": done, "calls": passes * (n // chunk), "ms": ms,
+                     "photons_per_s": done / (ms * 1e-3), "hbm_gbs_algorithmic": done * (BYTES_IN + BYTES_OUT + BYTES_BIN) / (ms * 1e-3) / 1e9,
+                     "gpu_launches": pkg.launch_count() - l0})
+    best = max(rows, key=lambda r: r["photons_per_s"])
+    print(json.dumps({"metric": METRIC, "value": best["photons_per_s"], "unit": UNIT, "n_gpus": 1, "higher_is_better": True,
+                      "dtype": "f32", "data": "synthetic", "scaling": "weak", "vs_baseline": None,
+                      "config": {"workload": f"{args.config} chunk-size sweep: {w.scene.n_triangles} triangles, resident batch of {n} photons "
+                                             f"streamed until {args.total} photons per chunk size", "best_chunk": best["chunk"]},
+                      "sweep": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -131,6 +169,11 @@ def main():
     ap.add_argument("--reference-sample", type=int, default=20000)
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="config C5 protocol: stream --total photons through the resident batch in chunks of 1e5..1e8 "
+                         "and report photons/s and HBM GB/s per chunk size instead of the default line")
+    ap.add_argument("--total", type=int, default=1_000_000_000, help="photons streamed per chunk size in --sweep")
+    ap.add_argument("--chunks", type=str, default="100000,1000000,10000000,100000000")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "opx" else args.warmup
     if args.impl == "reference":
@@ -181,6 +224,9 @@ def main():
 
     records = scene.alloc_records(n, dev)
     hitmap, counters = scene.alloc_accumulators(dev)
+
+    if args.sweep:
+        return run_sweep(args, scene, (d_o, d_d, d_l), records, hitmap, counters, n, stream, w, pkg)
 
     def step():
         hitmap.zero_(); counters.zero_()
@@ -274,14 +320,19 @@ def main():
         "alu_tflops": alu_achieved, "alu_frac": alu_achieved / fp32_peak_tflops,
         "hbm_gbs": hbm_achieved, "hbm_frac": hbm_achieved / peaks["hbm_gbs"],
         "photons_per_s_alu_bound": n / t_alu_bound, "photons_per_s_hbm_bound": n / t_hbm_bound})
+    fma = pkg.measure_fp32_peak(dev)          # FMA micro-benchmark on this device
+    roof.update({"fp32_peak_measured_tflops": fma, "alu_frac_of_measured_peak": alu_achieved / fma if fma else None})
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         n_sample = min(n, args.cpu_sample)
         v, threads, secs, segs = time_oracle(w, n_sample, args.seed)
+        n1 = max(1000, n_sample // max(2, threads))
+        v1, _, secs1, _ = time_oracle(w, n1, args.seed, n_threads=1)
         cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
-               "sample": f"first {n_sample} photon ids of {args.config}, brute force over {w.scene.n_triangles} triangles, {secs:.1f} s",
-               "ray_triangle_tests_per_s": segs * w.scene.n_triangles / secs}
+               "sample": f"first {n_sample} photon ids of {args.config}, brute force over {w.scene.n_triangles} triangles, {secs:.1f} s "
+                         f"on all cores; first {n1} ids, {secs1:.1f} s on one thread",
+               "single_thread_value": v1, "ray_triangle_tests_per_s": segs * w.scene.n_triangles / secs}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -203,6 +203,13 @@ opx_status opx_propagate_stats(const opx_scene* scene, uint64_t n, uint64_t phot
                                const float* d_origins, const float* d_dirs, const float* d_wavelengths,
                                uint64_t seed, uint64_t* d_stats, void* cuda_stream);
 
+/* FP32 FMA micro-benchmark (8 independent chains per thread, 8 blocks of 256 threads per SM, no memory
+ * traffic): writes the best of three timed launches, in TFLOP/s (FMA = 2), to *tflops.  It is the
+ * measured counterpart of the derived peak SMs x 128 lanes x 2 x clock that the roofline of the
+ * ALU-bound propagation kernel is quoted against.  d_scratch: >= 4 device bytes.
+ * Synchronises the stream. */
+opx_status opx_measure_fp32_peak(double* tflops, void* d_scratch, void* cuda_stream);
+
 opx_status opx_scene_info(const opx_scene* scene, uint64_t* n_triangles, uint64_t* n_nodes,
                           uint64_t* n_pixels, uint64_t* n_surfaces);
 opx_status opx_scene_get_layout(const opx_scene* scene, opx_scene_layout* out);

@@ -43,6 +43,7 @@ struct PacketSmem {
     float red[kPktWarps][2];
     float bcast[2];
     uint32_t scan_tot[kPktWarps];
+    int next_group;              // dynamic hand-out of packet groups to warps
 };
 static_assert(sizeof(int) * kStackSmem >= sizeof(uint32_t) * kRadix, "radix counters alias the stack overflow area");
 
@@ -193,6 +194,7 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const uint64_t tile_base = (uint64_t)blockIdx.x * kTile;
     const int m = (int)min((uint64_t)kTile, n - tile_base);
+    if (threadIdx.x == 0) sm.next_group = 0;
 
     // 1. stage the tile (coalesced, streaming: read once); 16-byte loads for full, aligned tiles
     const bool vec = m == kTile && ((reinterpret_cast<uintptr_t>(origins) | reinterpret_cast<uintptr_t>(dirs) |
@@ -249,8 +251,13 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
     }
 
     // 3. each warp takes groups of 32 neighbouring photons and walks them as a packet
+    //    (groups are handed out dynamically so that a slow packet does not hold up its warp's share)
     const int groups = (m + 31) >> 5;
-    for (int gidx = w; gidx < groups; gidx += kPktWarps) {
+    for (;;) {
+        int gidx = 0;
+        if (lane == 0) gidx = atomicAdd(&sm.next_group, 1);
+        gidx = __shfl_sync(0xffffffffu, gidx, 0);
+        if (gidx >= groups) break;
         const int slot = gidx * 32 + lane;
         bool alive = slot < m;
         const bool valid = alive;

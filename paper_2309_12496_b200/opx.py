@@ -20,7 +20,8 @@ OPX_OK, OPX_ERR_INVALID_ARG, OPX_ERR_BAD_STATE, OPX_ERR_WORKSPACE_TOO_SMALL, OPX
 
 EXPORTS = ("opx_scene_create", "opx_scene_workspace_bytes", "opx_bvh_build", "opx_propagate",
            "opx_propagate_brute", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
-           "opx_profile_begin", "opx_profile_end", "opx_propagate_stats", "opx_scene_info", "opx_scene_get_layout", "opx_launch_count", "opx_scene_destroy",
+           "opx_profile_begin", "opx_profile_end", "opx_propagate_stats", "opx_measure_fp32_peak",
+           "opx_scene_info", "opx_scene_get_layout", "opx_launch_count", "opx_scene_destroy",
            "opx_last_error", "opx_version")
 
 
@@ -86,6 +87,7 @@ def load_library(path=LIB_PATH):
     lib.opx_profile_begin.argtypes = [vp, u32]
     lib.opx_profile_end.argtypes = [vp, vp, vp, vp]
     lib.opx_propagate_stats.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp]
+    lib.opx_measure_fp32_peak.argtypes = [vp, vp, vp]
     lib.opx_scene_info.argtypes = [vp, vp, vp, vp, vp]
     lib.opx_scene_get_layout.argtypes = [vp, vp]
     lib.opx_scene_destroy.argtypes = [vp]
@@ -96,6 +98,16 @@ def load_library(path=LIB_PATH):
 def _check(status):
     if status != OPX_OK:
         raise OpxError(status, load_library().opx_last_error().decode())
+
+
+def measure_fp32_peak(device="cuda"):
+    """opx_measure_fp32_peak -> TFLOP/s of the FP32 FMA micro-benchmark on the current device."""
+    import torch
+    scratch = torch.zeros(4, dtype=torch.float32, device=device)
+    out = C.c_double()
+    _check(load_library().opx_measure_fp32_peak(C.byref(out), scratch.data_ptr(),
+                                                C.c_void_p(torch.cuda.current_stream(device).cuda_stream)))
+    return out.value
 
 
 def launch_count():

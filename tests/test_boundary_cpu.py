@@ -24,7 +24,7 @@ def lib():
 
 def test_every_declared_symbol_is_exported(lib):
     header = open(os.path.join(ROOT, "include", "opx.h")).read()
-    declared = set(re.findall(r"\b(opx_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(opx_[a-z0-9_]+)\s*\(", header))
     assert declared == set(pkg.EXPORTS)
     for name in declared:
         assert hasattr(lib, name), name
