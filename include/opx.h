@@ -123,6 +123,8 @@ typedef struct {
     uint64_t frames;      /* (n_frames) x 64 B                                                  */
     uint64_t sorted_keys; /* (n_triangles) x 8 B Morton keys in leaf order (kept for checking)  */
     uint64_t parents;     /* (2 n_triangles - 1) x 4 B: parent of internal node i / leaf T-1+i  */
+    uint64_t wide_nodes;  /* (wide_node_capacity) x 896 B: 32-wide nodes collapsed from `nodes`  */
+    uint64_t wide_node_capacity;
     uint64_t total_bytes;
 } opx_scene_layout;
 
@@ -202,6 +204,20 @@ opx_status opx_profile_end(opx_scene* scene, float* ms_propagate, float* ms_bin,
 opx_status opx_propagate_stats(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,
                                const float* d_origins, const float* d_dirs, const float* d_wavelengths,
                                uint64_t seed, uint64_t* d_stats, void* cuda_stream);
+
+/* Work counters of the PRODUCT kernel (k_propagate_packet, instrumented instantiation): same records
+ * as opx_propagate into `out` (DEVICE arrays of n), no binning, and ADDS to d_stats (8 uint64, DEVICE):
+ * [0] packet-segments (one closest-hit query of a 32-photon packet) answered by beam traversal of the
+ * 32-wide tree, [1] packet-segments answered by the binary packet walk (incoherent packets, stack
+ * overflow, no wide tree), [2] wide nodes visited, [3] triangles handed to the lanes by beam traversal
+ * (each is tested by every live lane), [4] beam-stack overflows, [5..7] reserved.  Never timed. */
+opx_status opx_propagate_packet_stats(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,
+                                      const float* d_origins, const float* d_dirs, const float* d_wavelengths,
+                                      uint64_t seed, const opx_hits* out, uint64_t* d_stats, void* cuda_stream);
+
+/* Number of 32-wide nodes the last opx_bvh_build produced (0: the collapse did not fit its capacity and
+ * packets walk the binary tree only) and the capacity reserved in the scene workspace. */
+opx_status opx_scene_wide_info(const opx_scene* scene, uint64_t* n_wide_nodes, uint64_t* capacity);
 
 /* FP32 FMA micro-benchmark (8 independent chains per thread, 8 blocks of 256 threads per SM, no memory
  * traffic): writes the best of three timed launches, in TFLOP/s (FMA = 2), to *tflops.  It is the

@@ -329,6 +329,26 @@ opx_status opx_propagate_stats(const opx_scene* scene, uint64_t n, uint64_t phot
     return launch_stats(*scene, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, d_stats, (cudaStream_t)cuda_stream);
 }
 
+opx_status opx_propagate_packet_stats(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
+                                      const float* d_dirs, const float* d_wavelengths, uint64_t seed, const opx_hits* out,
+                                      uint64_t* d_stats, void* cuda_stream) {
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate_packet_stats before opx_bvh_build");
+    if (n == 0) return OPX_OK;
+    if (!d_origins || !d_dirs || !d_wavelengths || !d_stats || !out) return fail(OPX_ERR_INVALID_ARG, "NULL pointer");
+    if (!out->pos || !out->dir || !out->pixel || !out->surface || !out->state || !out->bounces)
+        return fail(OPX_ERR_INVALID_ARG, "NULL hit-record array");
+    return launch_packet_stats(*scene, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, *out, d_stats, (cudaStream_t)cuda_stream);
+}
+
+opx_status opx_scene_wide_info(const opx_scene* scene, uint64_t* n_wide_nodes, uint64_t* capacity) {
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_scene_wide_info before opx_bvh_build");
+    if (n_wide_nodes) *n_wide_nodes = scene->dev.n_wnodes;
+    if (capacity) *capacity = scene->layout.wide_node_capacity;
+    return OPX_OK;
+}
+
 opx_status opx_scene_info(const opx_scene* scene, uint64_t* n_triangles, uint64_t* n_nodes, uint64_t* n_pixels,
                           uint64_t* n_surfaces) {
     if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");

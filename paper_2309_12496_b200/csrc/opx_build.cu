@@ -8,6 +8,7 @@
 // The BVH is not part of the parity contract (the oracle has none); what is, is that traversal
 // never culls a triangle the contract test of DESIGN.md 3.3 accepts -- hence the padding here.
 #include <cfloat>
+#include <cmath>
 
 #include "opx_internal.cuh"
 
@@ -15,6 +16,7 @@ namespace opx {
 
 namespace {
 
+constexpr float kBeamWidthInTriangles = 8.f;    // beam_max_width = this x the typical triangle size
 constexpr int kSortBlock = 256;
 constexpr int kSortItems = 8;
 constexpr int kSortTile = kSortBlock * kSortItems;  // 2048 keys per block per pass
@@ -28,6 +30,8 @@ struct BuildTmp {
     uint32_t* hist;       // 256 x n_sort_blocks
     uint32_t* bounds;     // 6 ordered-int floats: min xyz, max xyz
     uint32_t* flags;      // T-1 arrival counters
+    int2* queue[2];       // collapse tasks (binary node, wide node), ping-pong per level
+    uint32_t* wcount;     // collapse counters: n_in, n_out, n_wide_nodes, overflow
 };
 
 __host__ __device__ inline size_t sort_blocks(size_t T) { return (T + kSortTile - 1) / kSortTile; }
@@ -222,7 +226,7 @@ __global__ void __launch_bounds__(256) k_hierarchy(const uint64_t* __restrict__ 
     const int lo = min(i, j), hi = max(i, j);
     const int left = (lo == gamma) ? ~gamma : gamma;
     const int right = (hi == gamma + 1) ? ~(gamma + 1) : gamma + 1;
-    nodes[i].q3 = make_int4(left, right, 0, 0);
+    nodes[i].q3 = make_int4(left, right, l + 1, 0);      // .z: leaves below this node
     parents[left >= 0 ? left : (T - 1 + ~left)] = i;
     parents[right >= 0 ? right : (T - 1 + ~right)] = i;
     if (i == 0) parents[0] = -1;
@@ -257,7 +261,104 @@ __global__ void __launch_bounds__(256) k_refit(const float4* __restrict__ tris, 
     }
 }
 
+// ------------------------------------------------------------------- collapse to the 32-wide tree
+// One warp per wide node, one launch per level.  A task (b, w) turns the binary subtree rooted at b
+// into wide node w: lane k holds child k; the child with the largest box (among those with more
+// than 32 leaves -- smaller subtrees become full bottom nodes later) is replaced by its two
+// children until 32 slots are used; then the smallest remaining subtrees are expanded all the way to
+// their triangles while they fit.  Children that are still binary subtrees become tasks of the next
+// level.  A subtree of at most 32 leaves expands completely into triangle children.
+struct WEntry { int ref; int cnt; float lo[3], hi[3]; };
+
+__device__ inline void take_child(const NodeDev* __restrict__ bn, int node, int slot, WEntry& e) {
+    const NodeDev* nd = bn + node;
+    const float* f = reinterpret_cast<const float*>(nd) + slot * 6;
+    e.lo[0] = f[0]; e.lo[1] = f[1]; e.lo[2] = f[2]; e.hi[0] = f[3]; e.hi[1] = f[4]; e.hi[2] = f[5];
+    e.ref = slot == 0 ? nd->q3.x : nd->q3.y;
+    e.cnt = e.ref >= 0 ? bn[e.ref].q3.z : 1;
+}
+
+__global__ void __launch_bounds__(256) k_collapse(const NodeDev* __restrict__ bn, const int2* __restrict__ q_in,
+                                                  const uint32_t* __restrict__ n_in_ptr, int2* q_out, uint32_t* n_out,
+                                                  WNodeDev* wn, uint32_t* n_wn, uint32_t cap_wn, uint32_t* overflow) {
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const uint32_t n_in = *n_in_ptr;
+    const uint32_t warps = gridDim.x * (blockDim.x >> 5);
+    for (uint32_t task = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); task < n_in; task += warps) {
+        const int b = q_in[task].x, w = q_in[task].y;
+        WEntry e; e.ref = 0x7fffffff; e.cnt = 0;
+        bool valid = false;
+        if (lane < 2) { take_child(bn, b, lane, e); valid = true; }
+        const bool bottom = bn[b].q3.z <= kWide;
+        int count = 2;
+        while (count < kWide) {
+            uint32_t key = 0;
+            if (valid && e.ref >= 0 && e.ref != 0x7fffffff && (bottom || e.cnt > kWide)) {
+                const float ex = e.hi[0] - e.lo[0], ey = e.hi[1] - e.lo[1], ez = e.hi[2] - e.lo[2];
+                key = __float_as_uint(fmaxf(ex * ey + ey * ez + ez * ex, 0.f)) + 1u;
+            }
+            const uint32_t best = __reduce_max_sync(full, key);
+            if (best == 0) break;
+            const int L = __ffs(__ballot_sync(full, key == best)) - 1;
+            const int r = __shfl_sync(full, e.ref, L);
+            if (lane == L) take_child(bn, r, 0, e);
+            if (lane == count) { take_child(bn, r, 1, e); valid = true; }
+            ++count;
+        }
+        if (!bottom) {
+            for (;;) {   // fill: expand the smallest remaining subtree completely while it fits
+                const bool cand = valid && e.ref >= 0 && e.cnt <= kWide;
+                const int cmin = __reduce_min_sync(full, cand ? e.cnt : 0x7fffffff);
+                if (cmin == 0x7fffffff || count + cmin - 1 > kWide) break;
+                const int L = __ffs(__ballot_sync(full, cand && e.cnt == cmin)) - 1;
+                bool mine = lane == L;       // entries of the subtree being expanded
+                for (;;) {
+                    const unsigned m = __ballot_sync(full, mine && e.ref >= 0);
+                    if (!m) break;
+                    const int P = __ffs(m) - 1;
+                    const int r = __shfl_sync(full, e.ref, P);
+                    if (lane == P) take_child(bn, r, 0, e);
+                    if (lane == count) { take_child(bn, r, 1, e); valid = true; mine = true; }
+                    ++count;
+                }
+            }
+        }
+        // children that are still binary subtrees become wide nodes of the next level
+        const bool internal = valid && e.ref >= 0;
+        const unsigned m = __ballot_sync(full, internal);
+        const int k = __popc(m);
+        bool ok = true;
+        if (k) {
+            uint32_t base = 0, qbase = 0;
+            if (lane == 0) { base = atomicAdd(n_wn, (uint32_t)k); qbase = atomicAdd(n_out, (uint32_t)k); }
+            base = __shfl_sync(full, base, 0); qbase = __shfl_sync(full, qbase, 0);
+            if (base + k > cap_wn) { ok = false; if (lane == 0) *overflow = 1u; }
+            else if (internal) {
+                const int rank = __popc(m & ((1u << lane) - 1u));
+                q_out[qbase + rank] = make_int2(e.ref, (int)(base + rank));
+                e.ref = (int)(base + rank);
+            }
+        }
+        if (!ok) continue;
+        WNodeDev* o = wn + w;
+        const float inf = __int_as_float(0x7f800000);
+        for (int a = 0; a < 3; ++a) { o->lo[a][lane] = valid ? e.lo[a] : inf; o->hi[a][lane] = valid ? e.hi[a] : -inf; }
+        o->ref[lane] = valid ? e.ref : 0x7fffffff;
+    }
+}
+
+__global__ void k_collapse_init(int2* q, uint32_t* counters) {
+    // counters: [0] n_in, [1] n_out, [2] n_wn, [3] overflow
+    q[0] = make_int2(0, 0);
+    counters[0] = 1u; counters[1] = 0u; counters[2] = 1u; counters[3] = 0u;
+}
+
+__global__ void k_collapse_next(uint32_t* counters) { counters[0] = counters[1]; counters[1] = 0u; }
+
 }  // namespace
+
+size_t wide_node_capacity(size_t T) { return T >= 2 ? T / 8 + 64 : 1; }
 
 // ------------------------------------------------------------------------------------- layout
 void compute_layout(const SceneHost& s, opx_scene_layout* lay, size_t* tmp_bytes) {
@@ -274,6 +375,8 @@ void compute_layout(const SceneHost& s, opx_scene_layout* lay, size_t* tmp_bytes
     lay->frames = take(s.frames.size() * sizeof(FrameDev));
     lay->sorted_keys = take(T * 8);
     lay->parents = take((2 * T + 1) * 4);
+    lay->wide_node_capacity = wide_node_capacity(T);
+    lay->wide_nodes = take(lay->wide_node_capacity * sizeof(WNodeDev));
     lay->total_bytes = off;
     if (tmp_bytes) {
         size_t t = 0;
@@ -281,6 +384,7 @@ void compute_layout(const SceneHost& s, opx_scene_layout* lay, size_t* tmp_bytes
         tk(T * 36); tk(T * 4); tk(T * 12);
         tk(T * 8); tk(T * 4); tk(T * 4);            // second key buffer, two index buffers
         tk(256 * sort_blocks(T) * 4); tk(64); tk(T * 4);
+        tk(wide_node_capacity(T) * 8); tk(wide_node_capacity(T) * 8); tk(64);      // collapse queues + counters
         *tmp_bytes = t;
     }
 }
@@ -307,6 +411,8 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
         tmp.keys[0] = sorted_keys; tmp.keys[1] = (uint64_t*)take(T * 8);
         tmp.idx[0] = (uint32_t*)take(T * 4); tmp.idx[1] = (uint32_t*)take(T * 4);
         tmp.hist = (uint32_t*)take(256 * sort_blocks(T) * 4); tmp.bounds = (uint32_t*)take(64); tmp.flags = (uint32_t*)take(T * 4);
+        tmp.queue[0] = (int2*)take(wide_node_capacity(T) * 8); tmp.queue[1] = (int2*)take(wide_node_capacity(T) * 8);
+        tmp.wcount = (uint32_t*)take(64);
     }
     auto up = [&](void* dst, const void* src, size_t bytes) -> cudaError_t {
         if (!bytes) return cudaSuccess;
@@ -323,8 +429,25 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
     float maxabs = 0.f;
     for (float v : s.tri) { const float a = std::fabs(v); if (a > maxabs) maxabs = a; }
     const float pad = fmaxf(maxabs * (1.0f / 65536.0f), 1e-6f);
+    // typical triangle size (log-mean of the largest AABB extent) and scene extent: a beam much wider
+    // than the triangles it meets gains nothing over per-ray box tests
+    double logsum = 0.0;
+    float slo[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, shi[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
+    for (size_t t = 0; t < T; ++t) {
+        const float* v = &s.tri[9 * t];
+        float ext = 0.f;
+        for (int c = 0; c < 3; ++c) {
+            const float lo = std::fmin(v[c], std::fmin(v[3 + c], v[6 + c])), hi = std::fmax(v[c], std::fmax(v[3 + c], v[6 + c]));
+            ext = std::fmax(ext, hi - lo);
+            slo[c] = std::fmin(slo[c], lo); shi[c] = std::fmax(shi[c], hi);
+        }
+        logsum += std::log2((double)std::fmax(ext, 1e-20f));
+    }
+    const float tri_size = T ? (float)std::exp2(logsum / (double)T) : 0.f;
+    const float scene_ext = T ? std::fmax(shi[0] - slo[0], std::fmax(shi[1] - slo[1], shi[2] - slo[2])) : 0.f;
 
     const int Ti = (int)T;
+    uint32_t n_wide = 0;
     if (T >= 2) {
         const uint32_t nsb = (uint32_t)sort_blocks(T);
         const uint32_t g256 = (uint32_t)((T + 255) / 256);
@@ -347,6 +470,26 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
         if ((e = cudaMemsetAsync(tmp.flags, 0, T * 4, stream))) return check_cuda(e, "memset flags");
         k_refit<<<g256, 256, 0, stream>>>(tris, Ti, pad, nodes, parents, tmp.flags);
         count_launch(3);
+        // collapse into the 32-wide tree, level by level (the host reads the size of the next level)
+        WNodeDev* wnodes = (WNodeDev*)(ws + lay.wide_nodes);
+        const uint32_t cap = (uint32_t)lay.wide_node_capacity;
+        k_collapse_init<<<1, 1, 0, stream>>>(tmp.queue[0], tmp.wcount);
+        count_launch(1);
+        uint32_t h_cnt[4] = {1, 0, 1, 0};
+        int qi = 0;
+        for (int level = 0; level < 128 && h_cnt[0] > 0; ++level) {
+            const uint32_t blocks = (h_cnt[0] + 7) / 8;
+            k_collapse<<<blocks < 2368u ? blocks : 2368u, 256, 0, stream>>>(nodes, tmp.queue[qi], tmp.wcount, tmp.queue[qi ^ 1], tmp.wcount + 1,
+                                                                          wnodes, tmp.wcount + 2, cap, tmp.wcount + 3);
+            k_collapse_next<<<1, 1, 0, stream>>>(tmp.wcount);
+            count_launch(2);
+            if ((e = cudaMemcpyAsync(h_cnt, tmp.wcount, 16, cudaMemcpyDeviceToHost, stream)) || (e = cudaStreamSynchronize(stream)))
+                return check_cuda(e, "wide-tree collapse");
+            if (h_cnt[3]) break;
+            qi ^= 1;
+        }
+        // capacity exceeded (or a pathologically deep tree): no wide tree, packets walk the binary tree
+        n_wide = (h_cnt[3] || h_cnt[0] > 0) ? 0u : h_cnt[2];
     } else if (T == 1) {
         // a single triangle needs no hierarchy: propagate tests it directly (see launch_propagate)
         uint64_t zero_key = 0;
@@ -361,10 +504,13 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
     if ((e = cudaStreamSynchronize(stream))) return check_cuda(e, "BVH build");
 
     SceneDev& d = s.dev;
+    d.wnodes = (const WNodeDev*)(ws + lay.wide_nodes); d.n_wnodes = n_wide;
     d.nodes = nodes; d.tris = tris; d.normals = normals; d.surfaces = surfaces; d.mat_kinds = mat_kinds;
     d.tables = tables; d.frames = frames;
     d.n_tri = (uint32_t)T; d.n_nodes = (uint32_t)(T > 1 ? T - 1 : 1);
     d.n_lambda = s.params.n_lambda; d.max_bounces = s.params.max_bounces;
+    d.beam_max_width = kBeamWidthInTriangles * tri_size;
+    d.beam_max_spread = scene_ext > 0.f ? d.beam_max_width / (0.5f * scene_ext) : 0.f;
     d.lambda_min = s.params.lambda_min_nm; d.inv_dlambda = s.inv_dlambda; d.t_min = s.params.t_min_mm;
     return OPX_OK;
 }

@@ -24,19 +24,29 @@ struct alignas(16) FrameDev {  // 64 B
 //   q1 = (c0.hi.y, c0.hi.z, c1.lo.x, c1.lo.y)
 //   q2 = (c1.lo.z, c1.hi.x, c1.hi.y, c1.hi.z)
 //   q3 = (child0, child1, 0, 0) as int bits; child >= 0: internal node index; child < 0: leaf ~child
+//   q3.z = number of leaves (triangles) below this node
 struct alignas(16) NodeDev { float4 q0, q1, q2; int4 q3; };
+
+// Wide BVH node, 896 B: up to 32 children in SoA so that lane k of a warp reads child k with seven
+// coalesced 128-byte loads.  ref >= 0: wide node index; ref < 0: ~(leaf-order triangle index).
+// Unused slots hold an empty box (lo = +inf, hi = -inf) that no beam can enter.
+constexpr int kWide = 32;
+struct alignas(128) WNodeDev { float lo[3][kWide]; float hi[3][kWide]; int ref[kWide]; };
+constexpr int kWOffLo = 0, kWOffHi = 3 * kWide, kWOffRef = 6 * kWide;      // word offsets inside a WNodeDev
 
 // Everything the propagation kernels need, passed by value as a kernel parameter.
 struct SceneDev {
     const NodeDev* nodes;      // n_nodes
+    const WNodeDev* wnodes;    // n_wnodes (0: the wide tree is not available, packets walk the binary tree)
     const float4* tris;        // 3 per triangle, leaf order: (a.xyz, id bits) (b.xyz, surface bits) (c.xyz, 0)
     const float4* normals;     // leaf order: n.xyz, surface id bits
     const int2* surfaces;      // (material, frame)
     const uint32_t* mat_kinds;
     const float* tables;       // n_materials x n_lambda
     const FrameDev* frames;
-    uint32_t n_tri, n_nodes, n_lambda, max_bounces;
+    uint32_t n_tri, n_nodes, n_wnodes, n_lambda, max_bounces;
     float lambda_min, inv_dlambda, t_min;
+    float beam_max_width, beam_max_spread;   // packets wider than this (origins [mm] / directions) walk the binary tree
 };
 
 struct Layout : opx_scene_layout {};
@@ -80,6 +90,9 @@ opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, uint64_t
                             uint32_t* hitmap, uint64_t* counters, cudaStream_t stream);
 opx_status launch_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,
                         const float* wl, uint64_t seed, uint64_t* stats, cudaStream_t stream);
+opx_status launch_packet_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,
+                               const float* wl, uint64_t seed, const opx_hits& out, uint64_t* stats, cudaStream_t stream);
+size_t wide_node_capacity(size_t n_triangles);
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 

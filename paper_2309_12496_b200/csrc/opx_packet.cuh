@@ -14,6 +14,7 @@
 //   4. store   records are written back into the photon's own shared-memory slot and the tile is
 //              written out with coalesced streaming stores.
 #pragma once
+#include "opx_beam.cuh"
 #include "opx_device.cuh"
 
 namespace opx {
@@ -40,12 +41,14 @@ struct PacketSmem {
         int stack[kPktWarps][kStackSmem];        // traversal: stack entries >= 32 of each warp
         uint32_t cnt[kRadix][kPktWarps];         // sort: radix counters [digit][warp]
     };
-    float red[kPktWarps][2];
-    float bcast[2];
+    float beam_tn[kPktWarps][kBeamStack];        // beam traversal: entry bounds of the stacked wide nodes (refs alias `stack`)
+    float red[kPktWarps][3];
+    float bcast[3];
     uint32_t scan_tot[kPktWarps];
     int next_group;              // dynamic hand-out of packet groups to warps
 };
 static_assert(sizeof(int) * kStackSmem >= sizeof(uint32_t) * kRadix, "radix counters alias the stack overflow area");
+static_assert(kBeamStack <= kStackSmem, "the beam stack refs alias the binary walk's overflow area");
 
 // Octahedral map of a direction to [-1,1]^2 (NaN-safe: garbage maps to 0,0).
 __device__ __forceinline__ void octa(float dx, float dy, float dz, float& u, float& v) {
@@ -60,17 +63,19 @@ __device__ __forceinline__ void octa(float dx, float dy, float dz, float& u, flo
     if (!(fabsf(v) <= 1.f)) v = 0.f;
 }
 
-__device__ __forceinline__ void block_sum2(PacketSmem& sm, float x, float y, float& sx, float& sy) {
-    for (int off = 16; off > 0; off >>= 1) { x += __shfl_xor_sync(0xffffffffu, x, off); y += __shfl_xor_sync(0xffffffffu, y, off); }
-    if ((threadIdx.x & 31) == 0) { sm.red[threadIdx.x >> 5][0] = x; sm.red[threadIdx.x >> 5][1] = y; }
+__device__ __forceinline__ void block_sum3(PacketSmem& sm, float x, float y, float z, float& sx, float& sy, float& sz) {
+    for (int off = 16; off > 0; off >>= 1) {
+        x += __shfl_xor_sync(0xffffffffu, x, off); y += __shfl_xor_sync(0xffffffffu, y, off); z += __shfl_xor_sync(0xffffffffu, z, off);
+    }
+    if ((threadIdx.x & 31) == 0) { sm.red[threadIdx.x >> 5][0] = x; sm.red[threadIdx.x >> 5][1] = y; sm.red[threadIdx.x >> 5][2] = z; }
     __syncthreads();
-    if (threadIdx.x < 2) {
+    if (threadIdx.x < 3) {
         float r = 0.f;
         for (int w = 0; w < kPktWarps; ++w) r += sm.red[w][threadIdx.x];
         sm.bcast[threadIdx.x] = r;
     }
     __syncthreads();
-    sx = sm.bcast[0]; sy = sm.bcast[1];
+    sx = sm.bcast[0]; sy = sm.bcast[1]; sz = sm.bcast[2];
 }
 
 // One stable radix pass (kRadixBits bits) src -> dst over kTile packed keys.  Warp w owns the
@@ -185,10 +190,12 @@ __device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW
     return h;
 }
 
+template <bool kStats>
 __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const SceneDev sc, uint64_t n, uint64_t id_base,
                                                                      const float* __restrict__ origins,
                                                                      const float* __restrict__ dirs,
-                                                                     const float* __restrict__ wl, uint64_t seed, opx_hits out) {
+                                                                     const float* __restrict__ wl, uint64_t seed, opx_hits out,
+                                                                     unsigned long long* stats) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PacketSmem& sm = *reinterpret_cast<PacketSmem*>(smem_raw);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -218,29 +225,75 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
     }
     __syncthreads();
 
-    // 2. sort key: 12-bit pseudo-angle about the tile's mean direction in the octahedral plane
+    // 2. sort key: (run of the tile the photon belongs to, 10-bit pseudo-angle of its direction about
+    //    the run's mean direction in the octahedral plane).  A run is a stretch of consecutive photons
+    //    without a jump of the origin (> 16 x the tile's mean jump): photons arrive in generation order,
+    //    so a jump is where the next charged track starts, and its cone has a different axis.
     {
-        float u[kItems], v[kItems];
-        float su = 0.f, sv = 0.f;
+        float u[kItems], v[kItems], jump[kItems];
+        float su = 0.f, sv = 0.f, sj = 0.f;
 #pragma unroll
         for (int r = 0; r < kItems; ++r) {
             const int i = r * kPktThreads + threadIdx.x;
-            u[r] = 0.f; v[r] = 0.f;
-            if (i < m) { octa(sm.d[3 * i], sm.d[3 * i + 1], sm.d[3 * i + 2], u[r], v[r]); su += u[r]; sv += v[r]; }
+            u[r] = 0.f; v[r] = 0.f; jump[r] = 0.f;
+            if (i < m) {
+                octa(sm.d[3 * i], sm.d[3 * i + 1], sm.d[3 * i + 2], u[r], v[r]); su += u[r]; sv += v[r];
+                if (i > 0) {
+                    const float j = fmaxf(fmaxf(fabsf(sm.o[3 * i] - sm.o[3 * i - 3]), fabsf(sm.o[3 * i + 1] - sm.o[3 * i - 2])),
+                                          fabsf(sm.o[3 * i + 2] - sm.o[3 * i - 1]));
+                    if (j < kInf) { jump[r] = j; sj += j; }
+                }
+            }
         }
-        float cu, cv;
-        block_sum2(sm, su, sv, cu, cv);
-        cu /= (float)m; cv /= (float)m;
+        float cu, cv, cj;
+        block_sum3(sm, su, sv, sj, cu, cv, cj);
+        const float thr = 16.f * cj / (float)m;
+        bool flag[kItems];
+        bool any = false;
+#pragma unroll
+        for (int r = 0; r < kItems; ++r) { flag[r] = jump[r] > thr; any |= flag[r]; }
+        uint32_t run[kItems] = {};
+        float cur[kItems], cvr[kItems];
+#pragma unroll
+        for (int r = 0; r < kItems; ++r) { cur[r] = cu / (float)m; cvr[r] = cv / (float)m; }
+        if (__syncthreads_or(any)) {      // rare: the tile holds photons of more than one track
+            uint32_t* chunk = &sm.cnt[0][0];                       // kItems x kPktWarps jump counts, in tile order
+            float* rs = reinterpret_cast<float*>(chunk + 64);      // 4 runs x (sum u, sum v, count)
+            unsigned bal[kItems];
+#pragma unroll
+            for (int r = 0; r < kItems; ++r) {
+                bal[r] = __ballot_sync(0xffffffffu, flag[r]);
+                if (lane == 0) chunk[r * kPktWarps + w] = __popc(bal[r]);
+            }
+            if (threadIdx.x < 12) rs[threadIdx.x] = 0.f;
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < kItems; ++r) {
+                uint32_t before = 0;
+                for (int c = 0; c < r * kPktWarps + w; ++c) before += chunk[c];
+                run[r] = min(3u, before + __popc(bal[r] & (0xffffffffu >> (31 - lane))));
+                if (r * kPktThreads + (int)threadIdx.x < m) {
+                    atomicAdd(&rs[3 * run[r]], u[r]); atomicAdd(&rs[3 * run[r] + 1], v[r]); atomicAdd(&rs[3 * run[r] + 2], 1.f);
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < kItems; ++r) {
+                const float cnt = fmaxf(rs[3 * run[r] + 2], 1.f);
+                cur[r] = rs[3 * run[r]] / cnt; cvr[r] = rs[3 * run[r] + 1] / cnt;
+            }
+            __syncthreads();
+        }
 #pragma unroll
         for (int r = 0; r < kItems; ++r) {
             const int i = r * kPktThreads + threadIdx.x;
             uint32_t key = 0xfffu;
             if (i < m) {
-                const float du = u[r] - cu, dv = v[r] - cv;
+                const float du = u[r] - cur[r], dv = v[r] - cvr[r];
                 const float a = fabsf(du) + fabsf(dv);
                 const float pp = a > 0.f ? dv / a : 0.f;                     // diamond angle in [0,4)
                 const float ang = du >= 0.f ? (dv >= 0.f ? pp : 4.f + pp) : 2.f - pp;
-                key = min(4095u, (uint32_t)(ang * 1024.f));
+                key = (run[r] << 10) | min(1023u, (uint32_t)(ang * 256.f));
             }
             sm.key[i] = (key << 16) | (uint32_t)i;
         }
@@ -253,6 +306,7 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
     // 3. each warp takes groups of 32 neighbouring photons and walks them as a packet
     //    (groups are handed out dynamically so that a slow packet does not hold up its warp's share)
     const int groups = (m + 31) >> 5;
+    BeamStats bstats;
     for (;;) {
         int gidx = 0;
         if (lane == 0) gidx = atomicAdd(&sm.next_group, 1);
@@ -267,8 +321,34 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
                     id_base + tile_base + (uint64_t)i);
         while (__any_sync(0xffffffffu, alive)) {
             const RayW rw = ray_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz);
-            const Slab sl = slab_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz);
             const float tmin = p.b == 0 ? 0.f : sc.t_min;
+            if (sc.n_wnodes) {     // coherent packet: one beam through the 32-wide tree
+                Beam bm;
+                float s;
+                const unsigned tris_before = bstats.tris, visits_before = bstats.visits;
+                if (beam_setup(sc, p.ox, p.oy, p.oz, p.dx, p.dy, p.dz, tmin, alive, bm, s)) {
+                    Hit hb;
+                    const bool done = bm.mixed ? closest_hit_beam<true, kStats>(sc, rw, bm, s, tmin, p.last, alive, lane, sm.stack[w], sm.beam_tn[w], hb, bstats)
+                                               : closest_hit_beam<false, kStats>(sc, rw, bm, s, tmin, p.last, alive, lane, sm.stack[w], sm.beam_tn[w], hb, bstats);
+                    if (done) {
+                        if (kStats) {
+                            ++bstats.beam_segments;
+                            const unsigned dt = bstats.tris - tris_before, dv = bstats.visits - visits_before;
+                            const int bucket = min(15, 32 - __clz(dt));
+                            const int bb = min(3, (int)__shfl_sync(0xffffffffu, p.b, __ffs(__ballot_sync(0xffffffffu, alive)) - 1));
+                            if (lane == 0) {
+                                atomicAdd(&stats[8 + bucket], 1ull); atomicAdd(&stats[24 + bucket], (unsigned long long)dt);
+                                atomicAdd(&stats[40 + bb], 1ull); atomicAdd(&stats[44 + bb], (unsigned long long)dt);
+                                atomicAdd(&stats[48 + bb], (unsigned long long)dv);
+                            }
+                        }
+                        if (alive) alive = interact(sc, hb, p, seed);
+                        continue;
+                    }
+                }
+            }
+            if (kStats) ++bstats.fallback_segments;
+            const Slab sl = slab_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz);
             // sign octant of the packet: specialised traversal when all alive lanes agree
             const int oct = (p.dx < 0.f ? 1 : 0) | (p.dy < 0.f ? 2 : 0) | (p.dz < 0.f ? 4 : 0);
             const unsigned am = __ballot_sync(0xffffffffu, alive);
@@ -286,6 +366,13 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
         }
     }
     __syncthreads();
+    if (kStats) {
+        if (lane == 0) {
+            atomicAdd(&stats[0], (unsigned long long)bstats.beam_segments); atomicAdd(&stats[1], (unsigned long long)bstats.fallback_segments);
+            atomicAdd(&stats[2], (unsigned long long)bstats.visits); atomicAdd(&stats[3], (unsigned long long)bstats.tris);
+            atomicAdd(&stats[4], (unsigned long long)bstats.overflows);
+        }
+    }
 
     // 4. write the tile's records (coalesced, streaming)
     for (int k = threadIdx.x; k < 3 * m; k += kPktThreads) {

@@ -8,9 +8,9 @@
 
 namespace opx {
 
-opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, uint64_t id_base, const float* o, const float* d,
-                            const float* wl, uint64_t seed, const opx_hits& out, uint32_t* hitmap, uint64_t* counters,
-                            cudaStream_t stream) {
+static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t n, uint64_t id_base, const float* o, const float* d,
+                                        const float* wl, uint64_t seed, const opx_hits& out, uint32_t* hitmap, uint64_t* counters,
+                                        uint64_t* packet_stats, cudaStream_t stream) {
     cudaEvent_t* ev = nullptr;
     if (s.prof_used < s.prof_max) { ev = &s.prof_events[3 * (size_t)s.prof_used]; ++s.prof_used; }
     if (ev) cudaEventRecord(ev[0], stream);
@@ -22,13 +22,16 @@ opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, uint64_t
     } else {
         static bool configured = false;
         if (!configured) {
-            if (opx_status st = check_cuda(cudaFuncSetAttribute(k_propagate_packet, cudaFuncAttributeMaxDynamicSharedMemorySize,
+            if (opx_status st = check_cuda(cudaFuncSetAttribute(k_propagate_packet<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                                (int)sizeof(PacketSmem)), "cudaFuncSetAttribute")) return st;
+            if (opx_status st = check_cuda(cudaFuncSetAttribute(k_propagate_packet<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                                 (int)sizeof(PacketSmem)), "cudaFuncSetAttribute")) return st;
             configured = true;
         }
         const uint64_t tiles = (n + kTile - 1) / kTile;
         if (tiles > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
-        k_propagate_packet<<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(s.dev, n, id_base, o, d, wl, seed, out);
+        if (packet_stats) k_propagate_packet<true><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(s.dev, n, id_base, o, d, wl, seed, out, (unsigned long long*)packet_stats);
+        else k_propagate_packet<false><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(s.dev, n, id_base, o, d, wl, seed, out, nullptr);
     }
     count_launch(1);
     if (ev) cudaEventRecord(ev[1], stream);
@@ -40,6 +43,18 @@ opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, uint64_t
     }
     if (ev) cudaEventRecord(ev[2], stream);
     return check_cuda(cudaGetLastError(), "propagate launch");
+}
+
+opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, uint64_t id_base, const float* o, const float* d,
+                            const float* wl, uint64_t seed, const opx_hits& out, uint32_t* hitmap, uint64_t* counters,
+                            cudaStream_t stream) {
+    return launch_propagate_impl(s, brute, n, id_base, o, d, wl, seed, out, hitmap, counters, nullptr, stream);
+}
+
+opx_status launch_packet_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,
+                               const float* wl, uint64_t seed, const opx_hits& out, uint64_t* stats, cudaStream_t stream) {
+    if (s.dev.n_tri < 2) return fail(OPX_ERR_BAD_STATE, "no hierarchy to instrument (fewer than two triangles)");
+    return launch_propagate_impl(s, false, n, id_base, o, d, wl, seed, out, nullptr, nullptr, stats, stream);
 }
 
 opx_status launch_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d, const float* wl,

@@ -20,7 +20,8 @@ OPX_OK, OPX_ERR_INVALID_ARG, OPX_ERR_BAD_STATE, OPX_ERR_WORKSPACE_TOO_SMALL, OPX
 
 EXPORTS = ("opx_scene_create", "opx_scene_workspace_bytes", "opx_bvh_build", "opx_propagate",
            "opx_propagate_brute", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
-           "opx_profile_begin", "opx_profile_end", "opx_propagate_stats", "opx_measure_fp32_peak",
+           "opx_profile_begin", "opx_profile_end", "opx_propagate_stats", "opx_propagate_packet_stats",
+           "opx_scene_wide_info", "opx_measure_fp32_peak",
            "opx_scene_info", "opx_scene_get_layout", "opx_launch_count", "opx_scene_destroy",
            "opx_last_error", "opx_version")
 
@@ -58,7 +59,8 @@ class Hits(C.Structure):
 
 class SceneLayout(C.Structure):
     _fields_ = [(k, C.c_uint64) for k in ("nodes", "triangles", "normals", "surfaces", "mat_kinds", "tables",
-                                          "frames", "sorted_keys", "parents", "total_bytes")]
+                                          "frames", "sorted_keys", "parents", "wide_nodes", "wide_node_capacity",
+                                          "total_bytes")]
 
 
 _lib = None
@@ -87,6 +89,8 @@ def load_library(path=LIB_PATH):
     lib.opx_profile_begin.argtypes = [vp, u32]
     lib.opx_profile_end.argtypes = [vp, vp, vp, vp]
     lib.opx_propagate_stats.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp]
+    lib.opx_propagate_packet_stats.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp, vp]
+    lib.opx_scene_wide_info.argtypes = [vp, vp, vp]
     lib.opx_measure_fp32_peak.argtypes = [vp, vp, vp]
     lib.opx_scene_info.argtypes = [vp, vp, vp, vp, vp]
     lib.opx_scene_get_layout.argtypes = [vp, vp]
@@ -250,6 +254,30 @@ class Scene:
                                                   C.c_void_p(st.cuda_stream)))
         v = stats.cpu().tolist()
         return dict(segments=v[0], nodes=v[1], triangle_tests=v[2], interactions=v[3])
+
+    def propagate_packet_stats(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, records=None, stream=None):
+        """opx_propagate_packet_stats -> (records, dict(beam_segments, fallback_segments, wide_visits,
+        beam_triangles, stack_overflows)) of the instrumented product kernel."""
+        import torch
+        n = int(wavelengths.shape[0])
+        dev = wavelengths.device
+        if records is None:
+            records = self.alloc_records(n, dev)
+        stats = torch.zeros(64, dtype=torch.int64, device=dev)
+        h = Hits(*(records[k].data_ptr() for k in ("pos", "dir", "pixel", "surface", "state", "bounces")))
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        _check(load_library().opx_propagate_packet_stats(self._h, n, int(photon_id_base), origins.data_ptr(), dirs.data_ptr(),
+                                                         wavelengths.data_ptr(), int(seed), C.byref(h), stats.data_ptr(),
+                                                         C.c_void_p(st.cuda_stream)))
+        v = stats.cpu().tolist()
+        return records, dict(beam_segments=v[0], fallback_segments=v[1], wide_visits=v[2], beam_triangles=v[3],
+                             stack_overflows=v[4], raw=v)
+
+    def wide_info(self):
+        """opx_scene_wide_info -> (wide nodes built, capacity)."""
+        a, b = C.c_uint64(), C.c_uint64()
+        _check(load_library().opx_scene_wide_info(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def propagate_host(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, chunk=1 << 21, out=None,
                        stream=None, device="cuda"):
