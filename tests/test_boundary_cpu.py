@@ -34,7 +34,7 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_struct_sizes_match_header(lib):
     assert C.sizeof(opx.SceneParams) == 20 and C.sizeof(opx.PixelFrame) == 56
-    assert C.sizeof(opx.Mesh) == 40 and C.sizeof(opx.Hits) == 48 and C.sizeof(opx.SceneLayout) == 80
+    assert C.sizeof(opx.Mesh) == 40 and C.sizeof(opx.Hits) == 48 and C.sizeof(opx.SceneLayout) == 96
 
 
 def test_scene_create_and_info(lib):
@@ -45,7 +45,7 @@ def test_scene_create_and_info(lib):
     lay = s.layout()
     assert lay["total_bytes"] == scene_b and scene_b >= 20013 * 64 + 20014 * 64 and tmp_b > 20014 * 36
     offs = [lay[k] for k in ("nodes", "triangles", "normals", "surfaces", "mat_kinds", "tables", "frames",
-                             "sorted_keys", "parents")]
+                             "sorted_keys", "parents", "wide_nodes")]
     assert offs == sorted(offs) and all(o % 256 == 0 for o in offs)
     empty = pkg.Scene(Scene())
     assert (empty.n_triangles, empty.n_pixels) == (0, 0)
