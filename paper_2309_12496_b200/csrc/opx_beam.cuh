@@ -10,10 +10,16 @@
 //     [omin_a + t' dmin_a,  omax_a + t' dmax_a]        per axis a,
 // with omin/omax/dmin/dmax the (slightly widened) extremes of o'_i and d_i over the members.  A box
 // [lo, hi] can only be entered by a member while, on every axis,
-//     omax_a + t' dmax_a >= lo_a     and     omin_a + t' dmin_a <= hi_a,
+//     (1) omax_a + t' dmax_a >= lo_a     and     (2) omin_a + t' dmin_a <= hi_a,
 // each of which is a lower or an upper bound on t' depending on the sign of dmax_a / dmin_a.  The
 // interval they leave, clipped to [tlo, thi] with tlo = min_i(tmin - s_i) and thi = max_i(t_best_i - s_i),
 // is empty  =>  no member ray can hit anything in the box closer than its current best hit (ties kept).
+//
+// Per-lane cull.  When the beam enters many triangle boxes of a node (a packet's footprint covers more
+// facets than one ray crosses), every lane first slab-tests ITS OWN ray against those boxes (the planes
+// sit in the registers of the lane that owns the child and are broadcast by shuffle) and then tests
+// only the triangles whose box its ray enters: the leaf loop runs max-over-lanes instead of
+// sum-over-lanes iterations.
 #pragma once
 #include "opx_device.cuh"
 
@@ -21,101 +27,125 @@ namespace opx {
 namespace {
 
 constexpr int kBeamStack = 64;            // per warp, in shared memory; overflow => fall back to the binary walk
+#ifndef OPX_CULL_MIN
+#define OPX_CULL_MIN 4
+#endif
+constexpr int kCullMin = OPX_CULL_MIN;   // per-lane cull when the beam enters at least this many triangle boxes of a node
 
 struct Beam {
-    // entry bound per axis: fma(plane[offN_a], rn_a, cn_a); exit bound: fma(plane[offF_a], rf_a, cf_a).
+    // entry bound of axis a: fma(near_a, rn_a, cn_a); exit bound: fma(far_a, rf_a, cf_a), where
+    // (near, far) = (lo, hi) of the child box, swapped on an axis where all member directions are negative.
     // On an axis where the member directions have both signs (mixed), both planes give ENTRY bounds.
     float rn[3], cn[3], rf[3], cf[3];
-    int offN[3], offF[3];                 // word offsets of the two planes inside a WNodeDev (lane added by the caller)
+    unsigned neg;                         // bit a: near plane of axis a is hi
     unsigned mixed;                       // bit a: axis a is mixed
     float tlo;
 };
 
-struct BeamStats { unsigned visits = 0, tris = 0, beam_segments = 0, fallback_segments = 0, overflows = 0; };
+struct BeamStats { unsigned visits = 0, tris = 0, beam_segments = 0, fallback_segments = 0, overflows = 0, culls = 0; };
 
 __device__ __forceinline__ int f2ordi(float f) { const int i = __float_as_int(f); return i ^ ((i >> 31) & 0x7fffffff); }
 __device__ __forceinline__ float ordi2f(int i) { return __int_as_float(i ^ ((i >> 31) & 0x7fffffff)); }
 __device__ __forceinline__ float warp_min(float v) { return ordi2f(__reduce_min_sync(0xffffffffu, f2ordi(v))); }
 __device__ __forceinline__ float warp_max(float v) { return ordi2f(__reduce_max_sync(0xffffffffu, f2ordi(v))); }
+// min / max of floats known to be >= 0 (or +inf): their bit patterns order like the values
+__device__ __forceinline__ float warp_min_pos(float v) { return __int_as_float(__reduce_min_sync(0xffffffffu, __float_as_int(v))); }
+__device__ __forceinline__ float warp_max_pos(float v) { return __int_as_float(__reduce_max_sync(0xffffffffu, __float_as_int(v))); }
+__device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
 // Builds the beam of the alive lanes.  Returns false (warp-uniform) when the packet is not coherent
 // enough for a beam: some alive ray is non-finite, runs against the packet's dominant axis or nearly
-// perpendicular to it, or the re-based origins / the directions spread by more than the scene's limits
-// (SceneDev::beam_max_width, beam_max_spread).  `s` is the lane's re-basing offset (t = t' + s).
+// perpendicular to it, or a re-based origin / a direction lies further than the scene's limits
+// (SceneDev::beam_max_width, beam_max_spread) from the leader's.  `s` is the lane's re-basing offset
+// (t = t' + s).
+//
+// The extremes are taken on keys  k = x - (x_leader - W)  in [0, 2W]  (W = the limit): non-negative
+// floats order like their bit patterns, so each extreme is one integer warp reduction; a negative
+// key (bit pattern < 0), a key > 2W or a NaN (bit pattern > that of 2W) marks a packet that is too wide.
 __device__ __forceinline__ bool beam_setup(const SceneDev& sc, float ox, float oy, float oz, float dx, float dy, float dz, float tmin, bool alive,
                                            Beam& bm, float& s) {
     const unsigned full = 0xffffffffu;
     const unsigned am = __ballot_sync(full, alive);
     const int leader = __ffs(am) - 1;
-    // dominant axis of the leader's direction
+    const int src = alive ? (int)(threadIdx.x & 31) : leader;     // a lane without a ray stands in for the leader
+    dx = __shfl_sync(full, dx, src); dy = __shfl_sync(full, dy, src); dz = __shfl_sync(full, dz, src);
+    ox = __shfl_sync(full, ox, src); oy = __shfl_sync(full, oy, src); oz = __shfl_sync(full, oz, src);
     const float lx = __shfl_sync(full, dx, leader), ly = __shfl_sync(full, dy, leader), lz = __shfl_sync(full, dz, leader);
     int K = 0; float lk = lx;
     if (fabsf(ly) > fabsf(lk)) { K = 1; lk = ly; }
     if (fabsf(lz) > fabsf(lk)) { K = 2; lk = lz; }
     const float dK = K == 0 ? dx : (K == 1 ? dy : dz), oK = K == 0 ? ox : (K == 1 ? oy : oz);
     const float sumabs = fabsf(ox) + fabsf(oy) + fabsf(oz) + fabsf(dx) + fabsf(dy) + fabsf(dz);
-    const bool member = alive && sumabs < kInf && (lk > 0.f ? dK >= 0.25f : dK <= -0.25f);     // NaN fails both
-    if (__ballot_sync(full, alive && !member)) return false;
+    const bool member = sumabs < kInf && (lk > 0.f ? dK >= 0.25f : dK <= -0.25f);     // NaN fails both
+    if (!__all_sync(full, member)) return false;
     // rear-most origin along K
-    const float c = lk > 0.f ? warp_min(alive ? oK : kInf) : warp_max(alive ? oK : -kInf);
-    s = alive ? __fdividef(c - oK, dK) : 0.f;
-    s = fminf(s, 0.f);
+    const float c = lk > 0.f ? warp_min(oK) : warp_max(oK);
+    s = fminf((c - oK) * rcp_approx(dK), 0.f);
     const float px = __fmaf_rn(s, dx, ox), py = __fmaf_rn(s, dy, oy), pz = __fmaf_rn(s, dz, oz);
+    const float W = sc.beam_max_width, S = sc.beam_max_spread;
+    const float bx = __shfl_sync(full, px, leader) - W, by = __shfl_sync(full, py, leader) - W, bz = __shfl_sync(full, pz, leader) - W;
+    const float ex = lx - S, ey = ly - S, ez = lz - S;
+    const float kx = px - bx, ky = py - by, kz = pz - bz, jx = dx - ex, jy = dy - ey, jz = dz - ez;
     float omin[3], omax[3], dmin[3], dmax[3];
-    omin[0] = warp_min(alive ? px : kInf); omax[0] = warp_max(alive ? px : -kInf);
-    omin[1] = warp_min(alive ? py : kInf); omax[1] = warp_max(alive ? py : -kInf);
-    omin[2] = warp_min(alive ? pz : kInf); omax[2] = warp_max(alive ? pz : -kInf);
-    dmin[0] = warp_min(alive ? dx : kInf); dmax[0] = warp_max(alive ? dx : -kInf);
-    dmin[1] = warp_min(alive ? dy : kInf); dmax[1] = warp_max(alive ? dy : -kInf);
-    dmin[2] = warp_min(alive ? dz : kInf); dmax[2] = warp_max(alive ? dz : -kInf);
-    bm.tlo = fmaxf(warp_min(alive ? tmin - s : kInf), 0.f);
-    // widen: re-based origins carry a few ulp of rounding, directions a few ulp of 1
-    float scale = 0.f;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) scale = fmaxf(scale, fmaxf(fabsf(omin[a]), fabsf(omax[a])));
-    const float eo = scale * 1.9073486e-6f + 1e-30f;      // 2^-19 of the largest |coordinate|
+    omin[0] = warp_min_pos(kx); omax[0] = warp_max_pos(kx); omin[1] = warp_min_pos(ky); omax[1] = warp_max_pos(ky);
+    omin[2] = warp_min_pos(kz); omax[2] = warp_max_pos(kz);
+    dmin[0] = warp_min_pos(jx); dmax[0] = warp_max_pos(jx); dmin[1] = warp_min_pos(jy); dmax[1] = warp_max_pos(jy);
+    dmin[2] = warp_min_pos(jz); dmax[2] = warp_max_pos(jz);
+    const int lim_o = __float_as_int(2.f * W), lim_d = __float_as_int(2.f * S);
     bool ok = true;
-    bm.mixed = 0u;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        if (dmax[a] - dmin[a] > sc.beam_max_spread || omax[a] - omin[a] > sc.beam_max_width) ok = false;
-        const float lo_o = omin[a] - eo, hi_o = omax[a] + eo;
-        float lo_d = dmin[a] - 1e-6f, hi_d = dmax[a] + 1e-6f;
+        ok = ok && __float_as_int(omin[a]) >= 0 && __float_as_int(omax[a]) <= lim_o && __float_as_int(dmin[a]) >= 0 &&
+             __float_as_int(dmax[a]) <= lim_d;
+    }
+    if (!ok) return false;
+    bm.tlo = warp_min_pos(alive ? tmin - s : kInf);      // tmin >= 0 and s <= 0
+    const float base_o[3] = {bx, by, bz}, base_d[3] = {ex, ey, ez};
+    // widen: keys, re-based origins and their sums carry a few ulp of rounding, directions a few ulp of 1
+    const float scale = fmaxf(fmaxf(fabsf(bx), fabsf(by)), fmaxf(fabsf(bz), 4.f * W));
+    const float eo = scale * 3.8146973e-6f + 1e-30f;      // 2^-18 of the largest |coordinate|
+    bm.mixed = 0u; bm.neg = 0u;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const float lo_o = (omin[a] + base_o[a]) - eo, hi_o = (omax[a] + base_o[a]) + eo;
+        float lo_d = (dmin[a] + base_d[a]) - 2e-6f, hi_d = (dmax[a] + base_d[a]) + 2e-6f;
         if (fabsf(hi_d) < 1e-9f) hi_d = 1e-9f;             // widening only
         if (fabsf(lo_d) < 1e-9f) lo_d = -1e-9f;
-        const float r1 = 1.f / hi_d, r2 = 1.f / lo_d;      // constraint 1: omax + t dmax >= lo;  2: omin + t dmin <= hi
+        // constraint 1: hi_o + t hi_d >= lo  ->  bound fma(lo, r1, c1);  2: lo_o + t lo_d <= hi  ->  fma(hi, r2, c2).
+        // The approximate reciprocals are off by <= 2 ulp: far inside the padding of the boxes.
+        const float r1 = rcp_approx(hi_d), r2 = rcp_approx(lo_d);
         const float c1 = -hi_o * r1, c2 = -lo_o * r2;
-        if (lo_d > 0.f) {             // all positive: 1 bounds the entry (uses lo), 2 the exit (uses hi)
-            bm.rn[a] = r1; bm.cn[a] = c1; bm.offN[a] = kWOffLo + a * kWide;
-            bm.rf[a] = r2; bm.cf[a] = c2; bm.offF[a] = kWOffHi + a * kWide;
-        } else if (hi_d < 0.f) {      // all negative: 2 bounds the entry (uses hi), 1 the exit (uses lo)
-            bm.rn[a] = r2; bm.cn[a] = c2; bm.offN[a] = kWOffHi + a * kWide;
-            bm.rf[a] = r1; bm.cf[a] = c1; bm.offF[a] = kWOffLo + a * kWide;
-        } else {                      // mixed: both are entry bounds, no exit bound
-            bm.rn[a] = r1; bm.cn[a] = c1; bm.offN[a] = kWOffLo + a * kWide;
-            bm.rf[a] = r2; bm.cf[a] = c2; bm.offF[a] = kWOffHi + a * kWide;
-            bm.mixed |= 1u << a;
-        }
+        const bool neg = hi_d < 0.f;                       // all negative: 2 bounds the entry (plane hi), 1 the exit (plane lo)
+        bm.rn[a] = neg ? r2 : r1; bm.cn[a] = neg ? c2 : c1;
+        bm.rf[a] = neg ? r1 : r2; bm.cf[a] = neg ? c1 : c2;
+        if (neg) bm.neg |= 1u << a;
+        else if (!(lo_d > 0.f)) bm.mixed |= 1u << a;       // mixed: (lo, r1, c1) and (hi, r2, c2) are both entry bounds
     }
-    return ok;
+    return true;
 }
 
 // Closest hit of the packet by beam traversal.  Returns false (warp-uniform) if the shared-memory
 // stack overflowed: the caller then redoes the segment with the binary packet walk.
+// (so, sd) point at the lane's own segment in shared memory (origin, direction; not re-based): the per-lane cull
+// reads it back from there, so the segment does not occupy registers during the walk.
 template <bool kMixed, bool kStats>
 __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayW& rw, const Beam& bm, float s, float tmin, int last,
-                                                 bool alive, int lane, int* s_ref, float* s_tn, Hit& h, BeamStats& stats) {
+                                                 bool alive, int lane, const float* so, const float* sd,
+                                                 int* s_ref, float* s_tn, Hit& h, BeamStats& stats) {
     const unsigned full = 0xffffffffu;
     h = Hit{kInf, -1, 0x7fffffff};
     float thi = kInf;
     int sp = 0, ref = 0;
     const unsigned lt = (1u << lane) - 1u;
+    const bool ngx = bm.neg & 1u, ngy = bm.neg & 2u, ngz = bm.neg & 4u;
     for (;;) {
         if (kStats) ++stats.visits;
         const float* nd = reinterpret_cast<const float*>(sc.wnodes + ref) + lane;
-        const float nx = __ldg(nd + bm.offN[0]), ny = __ldg(nd + bm.offN[1]), nz = __ldg(nd + bm.offN[2]);
-        const float fx = __ldg(nd + bm.offF[0]), fy = __ldg(nd + bm.offF[1]), fz = __ldg(nd + bm.offF[2]);
+        const float lox = __ldg(nd + kWOffLo), loy = __ldg(nd + kWOffLo + kWide), loz = __ldg(nd + kWOffLo + 2 * kWide);
+        const float hix = __ldg(nd + kWOffHi), hiy = __ldg(nd + kWOffHi + kWide), hiz = __ldg(nd + kWOffHi + 2 * kWide);
         const int cref = __float_as_int(__ldg(nd + kWOffRef));
+        const float nx = ngx ? hix : lox, ny = ngy ? hiy : loy, nz = ngz ? hiz : loz;
+        const float fx = ngx ? lox : hix, fy = ngy ? loy : hiy, fz = ngz ? loz : hiz;
         const float ax = __fmaf_rn(nx, bm.rn[0], bm.cn[0]), ay = __fmaf_rn(ny, bm.rn[1], bm.cn[1]), az = __fmaf_rn(nz, bm.rn[2], bm.cn[2]);
         const float bx = __fmaf_rn(fx, bm.rf[0], bm.cf[0]), by = __fmaf_rn(fy, bm.rf[1], bm.cf[1]), bz = __fmaf_rn(fz, bm.rf[2], bm.cf[2]);
         float tn = fmaxf(fmaxf(ax, ay), fmaxf(az, bm.tlo)), tf = thi;
@@ -127,23 +157,45 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayW&
             tf = fminf(fminf(bx, by), fminf(bz, tf));
         }
         const bool hit = tn <= tf;
-        unsigned mt = __ballot_sync(full, hit && cref < 0);
+        const unsigned mt = __ballot_sync(full, hit && cref < 0);
         if (mt) {
-            do {
-                const int L = __ffs(mt) - 1;
-                mt &= mt - 1;
+            unsigned mine = mt;                      // the triangle children this lane still has to test
+            if (!kMixed && __popc(mt) >= kCullMin) {
+                // per-lane cull: own ray against the candidate boxes (all member rays share the beam's sign octant, so
+                // near/far are the same planes for every lane).  Approximate reciprocals: see slab_setup.
+                if (kStats) ++stats.culls;
+                const float ix = rcp_approx(sd[0]), iy = rcp_approx(sd[1]), iz = rcp_approx(sd[2]);
+                const float qx = -so[0] * ix, qy = -so[1] * iy, qz = -so[2] * iz;
+                const float cap = alive ? h.t : -1.f;
+                mine = 0u;
+                unsigned m = mt;
+                do {
+                    const int L = __ffs(m) - 1;
+                    m &= m - 1;
+                    const float e0 = __fmaf_rn(__shfl_sync(full, nx, L), ix, qx), e1 = __fmaf_rn(__shfl_sync(full, ny, L), iy, qy),
+                                e2 = __fmaf_rn(__shfl_sync(full, nz, L), iz, qz);
+                    const float x0 = __fmaf_rn(__shfl_sync(full, fx, L), ix, qx), x1 = __fmaf_rn(__shfl_sync(full, fy, L), iy, qy),
+                                x2 = __fmaf_rn(__shfl_sync(full, fz, L), iz, qz);
+                    const float en = fmaxf(fmaxf(e0, e1), fmaxf(e2, 0.f)), exi = fminf(fminf(x0, x1), fminf(x2, cap));
+                    if (en <= exi) mine |= 1u << L;
+                } while (m);
+            }
+            while (__any_sync(full, mine != 0u)) {
+                const bool has = mine != 0u;
+                const int L = has ? __ffs(mine) - 1 : 0;
+                mine &= mine - 1u;
                 const int j = ~__shfl_sync(full, cref, L);
                 if (kStats) ++stats.tris;
-                if (alive) consider(sc, rw, j, tmin, last, h);
-            } while (mt);
+                if (alive && has) consider(sc, rw, j, tmin, last, h);
+            }
             thi = warp_max(alive ? h.t - s : -kInf);
         }
         const bool go = hit && cref >= 0 && tn <= thi;
         const unsigned mn = __ballot_sync(full, go);
         if (mn) {
-            // nearest child next, the others onto the stack with their entry bounds
-            const int kmin = __reduce_min_sync(full, go ? f2ordi(tn) : 0x7fffffff);
-            const int L = __ffs(__ballot_sync(full, go && f2ordi(tn) == kmin)) - 1;
+            // nearest child next, the others onto the stack with their entry bounds (tn >= 0: bit patterns order like values)
+            const int kmin = __reduce_min_sync(full, go ? __float_as_int(tn) : 0x7fffffff);
+            const int L = __ffs(__ballot_sync(full, go && __float_as_int(tn) == kmin)) - 1;
             const unsigned rest = mn & ~(1u << L);
             if (rest) {
                 const int k = __popc(rest);

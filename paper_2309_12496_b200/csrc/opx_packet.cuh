@@ -314,55 +314,69 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
         if (gidx >= groups) break;
         const int slot = gidx * 32 + lane;
         bool alive = slot < m;
-        const bool valid = alive;
         const int i = alive ? (int)(sm.key[slot] & 0xffffu) : 0;
-        Photon p;
-        photon_init(p, sm.o[3 * i], sm.o[3 * i + 1], sm.o[3 * i + 2], sm.d[3 * i], sm.d[3 * i + 1], sm.d[3 * i + 2], sm.wl[i],
-                    id_base + tile_base + (uint64_t)i);
+        // Only the bounce count and the triangle just left stay in registers across the traversal: the segment
+        // (origin, direction) lives in the photon's own shared-memory slot (rewritten after each reflection; nobody
+        // else reads or writes that slot), wavelength and id are re-read at each interaction, and the record
+        // replaces the segment in the slot the moment the photon terminates.
+        const float* so = sm.o + 3 * i;
+        const float* sd = sm.d + 3 * i;
+        uint32_t nb = 0;
+        int last = -1;
         while (__any_sync(0xffffffffu, alive)) {
-            const RayW rw = ray_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz);
-            const float tmin = p.b == 0 ? 0.f : sc.t_min;
-            if (sc.n_wnodes) {     // coherent packet: one beam through the 32-wide tree
+            const float tmin = nb == 0 ? 0.f : sc.t_min;
+            Hit h;
+            RayW rw;
+            bool done = false;
+            {
+                const float ox = so[0], oy = so[1], oz = so[2], dx = sd[0], dy = sd[1], dz = sd[2];
+                rw = ray_setup(ox, oy, oz, dx, dy, dz);
                 Beam bm;
                 float s;
                 const unsigned tris_before = bstats.tris, visits_before = bstats.visits;
-                if (beam_setup(sc, p.ox, p.oy, p.oz, p.dx, p.dy, p.dz, tmin, alive, bm, s)) {
-                    Hit hb;
-                    const bool done = bm.mixed ? closest_hit_beam<true, kStats>(sc, rw, bm, s, tmin, p.last, alive, lane, sm.stack[w], sm.beam_tn[w], hb, bstats)
-                                               : closest_hit_beam<false, kStats>(sc, rw, bm, s, tmin, p.last, alive, lane, sm.stack[w], sm.beam_tn[w], hb, bstats);
-                    if (done) {
-                        if (kStats) {
-                            ++bstats.beam_segments;
-                            const unsigned dt = bstats.tris - tris_before, dv = bstats.visits - visits_before;
-                            const int bucket = min(15, 32 - __clz(dt));
-                            const int bb = min(3, (int)__shfl_sync(0xffffffffu, p.b, __ffs(__ballot_sync(0xffffffffu, alive)) - 1));
-                            if (lane == 0) {
-                                atomicAdd(&stats[8 + bucket], 1ull); atomicAdd(&stats[24 + bucket], (unsigned long long)dt);
-                                atomicAdd(&stats[40 + bb], 1ull); atomicAdd(&stats[44 + bb], (unsigned long long)dt);
-                                atomicAdd(&stats[48 + bb], (unsigned long long)dv);
-                            }
+                if (sc.n_wnodes && beam_setup(sc, ox, oy, oz, dx, dy, dz, tmin, alive, bm, s)) {     // coherent packet: one beam through the 32-wide tree
+                    done = bm.mixed ? closest_hit_beam<true, kStats>(sc, rw, bm, s, tmin, last, alive, lane, so, sd, sm.stack[w], sm.beam_tn[w], h, bstats)
+                                    : closest_hit_beam<false, kStats>(sc, rw, bm, s, tmin, last, alive, lane, so, sd, sm.stack[w], sm.beam_tn[w], h, bstats);
+                    if (kStats && done) {
+                        ++bstats.beam_segments;
+                        const unsigned dt = bstats.tris - tris_before, dv = bstats.visits - visits_before;
+                        const int bucket = min(15, 32 - __clz(dt));
+                        const int bb = min(3, (int)__shfl_sync(0xffffffffu, nb, __ffs(__ballot_sync(0xffffffffu, alive)) - 1));
+                        if (lane == 0) {
+                            atomicAdd(&stats[8 + bucket], 1ull); atomicAdd(&stats[24 + bucket], (unsigned long long)dt);
+                            atomicAdd(&stats[40 + bb], 1ull); atomicAdd(&stats[44 + bb], (unsigned long long)dt);
+                            atomicAdd(&stats[48 + bb], (unsigned long long)dv);
                         }
-                        if (alive) alive = interact(sc, hb, p, seed);
-                        continue;
                     }
                 }
             }
-            if (kStats) ++bstats.fallback_segments;
-            const Slab sl = slab_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz);
-            // sign octant of the packet: specialised traversal when all alive lanes agree
-            const int oct = (p.dx < 0.f ? 1 : 0) | (p.dy < 0.f ? 2 : 0) | (p.dz < 0.f ? 4 : 0);
-            const unsigned am = __ballot_sync(0xffffffffu, alive);
-            const int oct0 = __shfl_sync(0xffffffffu, oct, __ffs(am) - 1);
-            const bool uni = __all_sync(0xffffffffu, !alive || oct == oct0);
-            const Hit h = closest_hit_packet(sc, rw, sl, tmin, p.last, alive, lane, sm.stack[w], uni ? oct0 : 8);
-            if (alive) alive = interact(sc, h, p, seed);
-        }
-        if (valid) {      // the photon's own slot: nobody else reads or writes it
-            sm.o[3 * i] = p.px; sm.o[3 * i + 1] = p.py; sm.o[3 * i + 2] = p.pz;
-            sm.d[3 * i] = p.dx; sm.d[3 * i + 1] = p.dy; sm.d[3 * i + 2] = p.dz;
-            sm.wl[i] = __int_as_float(p.pixel);
-            sm.surface[i] = p.surface;
-            sm.state[i] = (uint8_t)p.state; sm.bounces[i] = (uint8_t)p.b;
+            if (!done) {
+                if (kStats) ++bstats.fallback_segments;
+                const float ox = so[0], oy = so[1], oz = so[2], dx = sd[0], dy = sd[1], dz = sd[2];
+                const Slab sl = slab_setup(ox, oy, oz, dx, dy, dz);
+                // sign octant of the packet: specialised traversal when all alive lanes agree
+                const int oct = (dx < 0.f ? 1 : 0) | (dy < 0.f ? 2 : 0) | (dz < 0.f ? 4 : 0);
+                const unsigned am = __ballot_sync(0xffffffffu, alive);
+                const int oct0 = __shfl_sync(0xffffffffu, oct, __ffs(am) - 1);
+                const bool uni = __all_sync(0xffffffffu, !alive || oct == oct0);
+                h = closest_hit_packet(sc, rw, sl, tmin, last, alive, lane, sm.stack[w], uni ? oct0 : 8);
+            }
+            if (alive) {
+                Photon p;
+                photon_init(p, so[0], so[1], so[2], sd[0], sd[1], sd[2], sm.wl[i], id_base + tile_base + (uint64_t)i);
+                p.b = nb; p.last = last;
+                alive = interact(sc, h, p, seed);
+                sm.d[3 * i] = p.dx; sm.d[3 * i + 1] = p.dy; sm.d[3 * i + 2] = p.dz;
+                if (alive) {
+                    sm.o[3 * i] = p.ox; sm.o[3 * i + 1] = p.oy; sm.o[3 * i + 2] = p.oz;
+                    nb = p.b; last = p.last;
+                } else {
+                    sm.o[3 * i] = p.px; sm.o[3 * i + 1] = p.py; sm.o[3 * i + 2] = p.pz;
+                    sm.wl[i] = __int_as_float(p.pixel);
+                    sm.surface[i] = p.surface;
+                    sm.state[i] = (uint8_t)p.state; sm.bounces[i] = (uint8_t)p.b;
+                }
+            }
         }
     }
     __syncthreads();
@@ -370,7 +384,7 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
         if (lane == 0) {
             atomicAdd(&stats[0], (unsigned long long)bstats.beam_segments); atomicAdd(&stats[1], (unsigned long long)bstats.fallback_segments);
             atomicAdd(&stats[2], (unsigned long long)bstats.visits); atomicAdd(&stats[3], (unsigned long long)bstats.tris);
-            atomicAdd(&stats[4], (unsigned long long)bstats.overflows);
+            atomicAdd(&stats[4], (unsigned long long)bstats.overflows); atomicAdd(&stats[5], (unsigned long long)bstats.culls);
         }
     }
 

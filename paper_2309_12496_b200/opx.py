@@ -271,7 +271,7 @@ class Scene:
                                                          C.c_void_p(st.cuda_stream)))
         v = stats.cpu().tolist()
         return records, dict(beam_segments=v[0], fallback_segments=v[1], wide_visits=v[2], beam_triangles=v[3],
-                             stack_overflows=v[4], raw=v)
+                             stack_overflows=v[4], lane_culls=v[5], raw=v)
 
     def wide_info(self):
         """opx_scene_wide_info -> (wide nodes built, capacity)."""
