@@ -36,6 +36,11 @@ def lib():
         _lib.oracle_table_lerp.argtypes = [C.c_int, C.c_void_p, C.c_uint32, C.c_float, C.c_float, C.c_float]
         _lib.oracle_hit_triangle.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         _lib.oracle_pixel_map.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        _lib.oracle_table_value.restype = C.c_double
+        _lib.oracle_table_value.argtypes = [C.c_int, C.c_void_p, C.c_uint32, C.c_uint32, C.c_float, C.c_float, C.c_float]
+        _lib.oracle_uniform_stream.restype = C.c_float
+        _lib.oracle_uniform_stream.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32]
+        _lib.oracle_prefilter.restype = C.c_uint64
     return _lib
 
 
@@ -67,6 +72,40 @@ def uniform(seed, g, b):
 def table_lerp(table, lam, lmin=200.0, lmax=600.0, fp64=False):
     t = _f32(table)
     return float(lib().oracle_table_lerp(int(fp64), _p(t), len(t), lmin, lmax, float(lam)))
+
+
+NO_EFFICIENCY = 1          # trace flag: efficiencies were applied by prefilter(), surfaces act with probability 1
+LINEAR, HISTOGRAM = 0, 1   # table forms
+
+
+def uniform_stream(seed, g, b, stream):
+    return float(lib().oracle_uniform_stream(int(seed), int(g), int(b), int(stream)))
+
+
+def table_value(table, lam, interp=LINEAR, lmin=200.0, lmax=600.0, fp64=False):
+    t = _f32(table)
+    return float(lib().oracle_table_value(int(fp64), _p(t), len(t), int(interp), lmin, lmax, float(lam)))
+
+
+def _mat_interp(scene):
+    return np.ascontiguousarray([m.get("interp", LINEAR) for m in scene.materials], dtype=np.uint32)
+
+
+def prefilter(scene, wavelengths, factors, seed=0, id_base=0):
+    """Pre-propagation efficiency filter: one accept-reject per photon on the product of the
+    efficiencies of the materials listed in `factors`.  Returns keep (n,) uint8, index (n_kept,) uint32, prob (n,)."""
+    wl = _f32(wavelengths).reshape(-1)
+    n = len(wl)
+    mat_table = np.ascontiguousarray(np.stack([m["table"] for m in scene.materials]), dtype=np.float32)
+    interp = _mat_interp(scene)
+    fac = np.ascontiguousarray(factors, dtype=np.uint32)
+    keep, index, prob = np.zeros(n, np.uint8), np.zeros(n, np.uint32), np.zeros(n, np.float32)
+    kept = lib().oracle_prefilter(_p(mat_table), _p(interp), C.c_uint32(len(interp)), C.c_uint32(mat_table.shape[1]),
+                                  C.c_float(scene.lambda_min), C.c_float(scene.lambda_max), _p(fac), C.c_uint32(len(fac)),
+                                  C.c_uint64(n), C.c_uint64(id_base), _p(wl), C.c_uint64(seed), _p(keep), _p(index), _p(prob))
+    if kept == 2 ** 64 - 1:
+        raise ValueError("oracle_prefilter: factor is not a material index")
+    return Result(keep=keep, index=index[:kept], prob=prob)
 
 
 def reflect(d, n, fp64=False):
@@ -112,7 +151,7 @@ class Result(dict):
 
 
 def trace_mesh(scene, origins, dirs, wavelengths, seed=0, id_base=0, ids=None, fp64=False,
-               n_threads=None):
+               n_threads=None, flags=0):
     """Brute-force trace of `scene` (a workloads.Scene-like object: meshes, materials, frames,
     lambda_min/max, n_lambda, max_bounces, t_min)."""
     o, d, wl = _f32(origins).reshape(-1, 3), _f32(dirs).reshape(-1, 3), _f32(wavelengths).reshape(-1)
@@ -127,12 +166,12 @@ def trace_mesh(scene, origins, dirs, wavelengths, seed=0, id_base=0, ids=None, f
     return trace_mesh_arrays(tri, tri_surface, surf_mat, surf_frame, mat_kind, mat_table,
                              scene.lambda_min, scene.lambda_max, frames, len(scene.frames),
                              scene.max_bounces, scene.t_min, scene.n_pixels, o, d, wl, seed, id_base,
-                             ids, fp64, n_threads)
+                             ids, fp64, n_threads, mat_interp=_mat_interp(scene), flags=flags)
 
 
 def trace_mesh_arrays(tri, tri_surface, surf_mat, surf_frame, mat_kind, mat_table, lmin, lmax, frames,
                       n_frames, max_bounces, t_min, n_pixels, o, d, wl, seed=0, id_base=0, ids=None,
-                      fp64=False, n_threads=None):
+                      fp64=False, n_threads=None, mat_interp=None, flags=0):
     n = len(wl)
     if n_threads is None:
         n_threads = os.cpu_count() or 1
@@ -141,8 +180,9 @@ def trace_mesh_arrays(tri, tri_surface, surf_mat, surf_frame, mat_kind, mat_tabl
                surface=np.zeros(n, np.int32), tri=np.zeros(n, np.int32), state=np.zeros(n, np.uint8),
                bounces=np.zeros(n, np.uint8), segments=np.zeros(n, np.uint32),
                hitmap=np.zeros(max(1, n_pixels), np.uint32), counters=np.zeros(8, np.uint64))
-    rc = lib().oracle_trace_mesh(
-        C.c_int(int(fp64)), _p(tri), _p(tri_surface), C.c_uint64(len(tri_surface)),
+    interp_arr = None if mat_interp is None else np.ascontiguousarray(mat_interp, dtype=np.uint32)
+    rc = lib().oracle_trace_mesh_ex(
+        C.c_int(int(fp64)), _p(interp_arr), C.c_uint32(flags), _p(tri), _p(tri_surface), C.c_uint64(len(tri_surface)),
         _p(surf_mat), _p(surf_frame), C.c_uint32(len(surf_mat)),
         _p(mat_kind), _p(mat_table), C.c_uint32(len(mat_kind)), C.c_uint32(mat_table.shape[1]),
         C.c_float(lmin), C.c_float(lmax), frames, C.c_uint32(n_frames),

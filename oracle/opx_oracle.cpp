@@ -63,9 +63,11 @@ void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]
 }
 
 // u(seed, g, b) in [0,1): 24 high bits of word 0, exactly representable in fp32.
-float uniform_draw(uint64_t seed, uint64_t g, uint32_t b) {
+// Counter word 3 names the stream: 0 = in-flight draws of the propagation, 1 = the pre-propagation filter
+// (DESIGN.md 3.9), so the two never share a random number.
+float uniform_draw(uint64_t seed, uint64_t g, uint32_t b, uint32_t stream = 0u) {
     const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
-    const uint32_t ctr[4] = {(uint32_t)g, (uint32_t)(g >> 32), b, 0u};
+    const uint32_t ctr[4] = {(uint32_t)g, (uint32_t)(g >> 32), b, stream};
     uint32_t r[4];
     philox4x32_10(ctr, key, r);
     return (float)(r[0] >> 8) * 0x1.0p-24f;
@@ -95,6 +97,30 @@ R table_lerp(const float* y, uint32_t n_lambda, R lambda_min, R inv_dlambda, R l
     if (f > (R)1) f = (R)1;
     const R y0 = (R)y[j], y1 = (R)y[j + 1];
     return rfma<R>(f, y1 - y0, y0);
+}
+
+// DESIGN.md 3.8.  The paper's own table form: "histograms of 33 nm bin width" (QE) and
+// "bins of 25 nm" (reflectivity).  The n_lambda values are the contents of n_lambda equal bins that tile
+// [lambda_min, lambda_max]; a wavelength takes the content of its bin, the end bins extend outwards.
+template <typename R>
+R table_histogram(const float* y, uint32_t n_lambda, R lambda_min, R inv_bin, R lambda) {
+    const R xf = std::floor((lambda - lambda_min) * inv_bin);
+    int j;                                                     // j = clamp(floor(x), 0, n_lambda-1)
+    if (!(xf >= (R)0)) j = 0;                                  // also catches NaN
+    else if (xf > (R)(n_lambda - 1)) j = (int)n_lambda - 1;
+    else j = (int)xf;
+    return (R)y[j];
+}
+
+enum TableInterp : uint32_t { TABLE_LINEAR = 0, TABLE_HISTOGRAM = 1 };
+
+// Efficiency of one material at lambda in its own table form.  The grid constants are computed in double and
+// rounded once to Real: inv_dlambda = (n-1)/(max-min) for the linear form, inv_bin = n/(max-min) for bins.
+template <typename R>
+R table_value(const float* y, uint32_t n_lambda, uint32_t interp, float lambda_min, float lambda_max, R lambda) {
+    const double span = (double)lambda_max - (double)lambda_min;
+    if (interp == TABLE_HISTOGRAM) return table_histogram<R>(y, n_lambda, (R)lambda_min, (R)((double)n_lambda / span), lambda);
+    return table_lerp<R>(y, n_lambda, (R)lambda_min, (R)((double)(n_lambda - 1) / span), lambda);
 }
 
 // ------------------------------------------------------------------------ ray / triangle test
@@ -215,7 +241,10 @@ struct SceneView {
     float lambda_min, lambda_max;
     const Frame* frames; uint32_t n_frames;
     uint32_t max_bounces; float t_min;
+    const uint32_t* mat_interp;    // M table forms (TableInterp), NULL = all linear
+    uint32_t flags;                // FLAG_NO_EFFICIENCY: surfaces act with probability 1, no random draws
 };
+enum : uint32_t { FLAG_NO_EFFICIENCY = 1u };
 
 struct Record { double pos[3], dir[3]; int32_t pixel, surface, tri; uint8_t state, bounces; uint32_t segments; };
 
@@ -226,7 +255,7 @@ Record trace_photon(const SceneView& sc, const std::vector<Vec3<R>>& normals, ui
                     uint64_t g, const float* o_in, const float* d_in, float lambda_in) {
     Vec3<R> o{(R)o_in[0], (R)o_in[1], (R)o_in[2]}, d{(R)d_in[0], (R)d_in[1], (R)d_in[2]};
     const R lambda = (R)lambda_in;
-    const R inv_dl = (R)((double)(sc.n_lambda - 1) / ((double)sc.lambda_max - (double)sc.lambda_min));
+    const bool draw = !(sc.flags & FLAG_NO_EFFICIENCY);        // efficiencies already applied (3.9)
     uint32_t b = 0;
     int64_t last = -1;
     Record rec{};
@@ -260,10 +289,13 @@ Record trace_photon(const SceneView& sc, const std::vector<Vec3<R>>& normals, ui
         rec.pos[0] = p.x; rec.pos[1] = p.y; rec.pos[2] = p.z;
         rec.dir[0] = d.x; rec.dir[1] = d.y; rec.dir[2] = d.z;
         if (kind == MAT_ABSORBER) { rec.state = ABSORBED_SURFACE; break; }
+        const uint32_t interp = sc.mat_interp ? sc.mat_interp[m] : (uint32_t)TABLE_LINEAR;
         if (kind == MAT_MIRROR) {
-            const R u = (R)uniform_draw(seed, g, b);
-            if (!(u < table_lerp<R>(table, sc.n_lambda, (R)sc.lambda_min, inv_dl, lambda))) {
-                rec.state = ABSORBED_MIRROR; break;
+            if (draw) {
+                const R u = (R)uniform_draw(seed, g, b);
+                if (!(u < table_value<R>(table, sc.n_lambda, interp, sc.lambda_min, sc.lambda_max, lambda))) {
+                    rec.state = ABSORBED_MIRROR; break;
+                }
             }
             d = reflect<R>(d, normals[k_best]);
             o = p; last = k_best; b++;
@@ -277,8 +309,9 @@ Record trace_photon(const SceneView& sc, const std::vector<Vec3<R>>& normals, ui
         const Frame& f = sc.frames[sc.surf_frame[s]];
         if (!pixel_map<R>(f, p, &iu, &iv)) { rec.state = DETECTOR_DEAD; rec.pixel = -1; break; }
         rec.pixel = (int32_t)(f.pixel_base + (uint32_t)iv * f.nu + (uint32_t)iu);
+        if (!draw) { rec.state = DETECTED; break; }
         const R u = (R)uniform_draw(seed, g, b);
-        rec.state = (u < table_lerp<R>(table, sc.n_lambda, (R)sc.lambda_min, inv_dl, lambda)) ? DETECTED : QE_REJECTED;
+        rec.state = (u < table_value<R>(table, sc.n_lambda, interp, sc.lambda_min, sc.lambda_max, lambda)) ? DETECTED : QE_REJECTED;
         break;
     }
     rec.bounces = (uint8_t)b;
@@ -363,7 +396,7 @@ int oracle_hit_triangle(int fp64, const float* o, const float* d, const float* v
 // Trace n photons through a triangle scene.  counters: 8 uint64 (+=): one per terminal state 0..6,
 // [7] = closest-hit queries (segments).  hitmap: n_pixels uint32 (+=).  ids == NULL => global id =
 // id_base + i.
-int oracle_trace_mesh(int fp64,
+int oracle_trace_mesh_ex(int fp64, const uint32_t* mat_interp, uint32_t flags,
                       const float* tri, const int32_t* tri_surface, uint64_t n_tri,
                       const uint32_t* surf_material, const int32_t* surf_frame, uint32_t n_surf,
                       const uint32_t* mat_kind, const float* mat_table, uint32_t n_mat, uint32_t n_lambda,
@@ -380,12 +413,67 @@ int oracle_trace_mesh(int fp64,
         if (surf_material[s] >= n_mat) return 3;
         if (mat_kind[surf_material[s]] == MAT_DETECTOR && (surf_frame[s] < 0 || (uint32_t)surf_frame[s] >= n_frames)) return 4;
     }
+    if (mat_interp) for (uint32_t m = 0; m < n_mat; ++m) if (mat_interp[m] > TABLE_HISTOGRAM) return 5;
     SceneView sc{tri, tri_surface, n_tri, surf_material, surf_frame, n_surf, mat_kind, mat_table, n_mat,
-                 n_lambda, lambda_min, lambda_max, frames, n_frames, max_bounces, t_min};
+                 n_lambda, lambda_min, lambda_max, frames, n_frames, max_bounces, t_min, mat_interp, flags};
     Outputs out{pos, dir, pixel, surface, tri_out, state, bounces, segments, hitmap, counters};
     if (fp64) trace_all<double>(sc, n, ids, id_base, origins, dirs, wl, seed, out, n_threads);
     else trace_all<float>(sc, n, ids, id_base, origins, dirs, wl, seed, out, n_threads);
     return 0;
+}
+
+// The form every test written before the table forms and flags existed calls: linear tables, in-flight draws.
+int oracle_trace_mesh(int fp64,
+                      const float* tri, const int32_t* tri_surface, uint64_t n_tri,
+                      const uint32_t* surf_material, const int32_t* surf_frame, uint32_t n_surf,
+                      const uint32_t* mat_kind, const float* mat_table, uint32_t n_mat, uint32_t n_lambda,
+                      float lambda_min, float lambda_max, const Frame* frames, uint32_t n_frames,
+                      uint32_t max_bounces, float t_min,
+                      uint64_t n, const uint64_t* ids, uint64_t id_base,
+                      const float* origins, const float* dirs, const float* wl, uint64_t seed,
+                      double* pos, double* dir, int32_t* pixel, int32_t* surface, int32_t* tri_out,
+                      uint8_t* state, uint8_t* bounces, uint32_t* segments, uint32_t* hitmap,
+                      uint64_t* counters, int n_threads) {
+    return oracle_trace_mesh_ex(fp64, nullptr, 0u, tri, tri_surface, n_tri, surf_material, surf_frame, n_surf, mat_kind,
+                                mat_table, n_mat, n_lambda, lambda_min, lambda_max, frames, n_frames, max_bounces, t_min,
+                                n, ids, id_base, origins, dirs, wl, seed, pos, dir, pixel, surface, tri_out, state,
+                                bounces, segments, hitmap, counters, n_threads);
+}
+
+double oracle_table_value(int fp64, const float* y, uint32_t n_lambda, uint32_t interp, float lmin, float lmax, float lambda) {
+    if (fp64) return table_value<double>(y, n_lambda, interp, lmin, lmax, (double)lambda);
+    return (double)table_value<float>(y, n_lambda, interp, lmin, lmax, lambda);
+}
+float oracle_uniform_stream(uint64_t seed, uint64_t g, uint32_t b, uint32_t stream) { return uniform_draw(seed, g, b, stream); }
+
+// Pre-propagation efficiency filter, the paper's own method ("For each photon, with its
+// specific wavelength, an accept-reject algorithm was used to model the three efficiencies before propagation
+// ... any discarded photons would not be detected").  DESIGN.md 3.9: ONE draw per photon,
+// u = U(seed, g, 0; stream 1), against the product of the listed materials' efficiencies at the photon's
+// wavelength, p = (..(e_0 * e_1) * e_2 ..) multiplied left to right in fp32; the photon is kept iff u < p.
+// keep[i] = 1/0; kept_index receives the indices of the kept photons in input order (stable compaction);
+// returns their number.  prob (may be NULL) receives p per photon.
+uint64_t oracle_prefilter(const float* mat_table, const uint32_t* mat_interp, uint32_t n_mat, uint32_t n_lambda,
+                          float lambda_min, float lambda_max, const uint32_t* factors, uint32_t n_factors,
+                          uint64_t n, uint64_t id_base, const float* wl, uint64_t seed,
+                          uint8_t* keep, uint32_t* kept_index, float* prob) {
+    uint64_t kept = 0;
+    for (uint64_t i = 0; i < n; ++i) {
+        float p = 1.0f;
+        for (uint32_t k = 0; k < n_factors; ++k) {
+            const uint32_t m = factors[k];
+            if (m >= n_mat) return ~0ull;
+            const float e = table_value<float>(mat_table + (size_t)m * n_lambda, n_lambda,
+                                               mat_interp ? mat_interp[m] : (uint32_t)TABLE_LINEAR, lambda_min, lambda_max, wl[i]);
+            p = (k == 0) ? e : p * e;
+        }
+        const float u = uniform_draw(seed, id_base + i, 0u, 1u);
+        const bool k = u < p;
+        if (prob) prob[i] = p;
+        keep[i] = k ? 1 : 0;
+        if (k) kept_index[kept++] = (uint32_t)i;
+    }
+    return kept;
 }
 
 // ------------------------------------------------------------------- analytic toy RICH (fp64)

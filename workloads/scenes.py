@@ -19,6 +19,9 @@ N_LAMBDA = 64                   # BASELINE.json config 1: 64-point tables
 LAMBDA_MIN_NM, LAMBDA_MAX_NM = 200.0, 600.0
 
 
+TABLE_LINEAR, TABLE_HISTOGRAM = 0, 1     # opx_table_interp (include/opx.h)
+
+
 @dataclass
 class Scene:
     """Plain container; field names follow include/opx.h."""
@@ -47,10 +50,10 @@ class Scene:
                                 frame=int(frame)))
         return len(self.meshes) - 1
 
-    def add_material(self, kind, table):
+    def add_material(self, kind, table, interp=TABLE_LINEAR):
         t = np.ascontiguousarray(np.asarray(table, dtype=np.float64).astype(np.float32))
         assert t.shape == (self.n_lambda,)
-        self.materials.append(dict(kind=int(kind), table=t))
+        self.materials.append(dict(kind=int(kind), table=t, interp=int(interp)))
         return len(self.materials) - 1
 
     def add_frame(self, A, u, v, pitch_u, pitch_v, nu, nv, pixel_base):
@@ -88,6 +91,19 @@ def c2_tables():
     lam = lambda_grid()
     refl = 0.85 + 0.10 * np.arange(N_LAMBDA) / (N_LAMBDA - 1)
     qe = 0.30 * np.exp(-0.5 * ((lam - 400.0) / 90.0) ** 2)
+    return refl, qe
+
+
+def paper_histogram_tables():
+    """The paper's table form: QE as a histogram of 33 nm bins, reflectivity in bins of
+    25 nm, both written on ONE grid of 400 bins of 1 nm over 200-600 nm (every bin edge is a whole nm, so the
+    1 nm grid holds both binnings exactly).  Shapes only (QE peaking 35 % near 450 nm, R falling from 94 % to
+    89 %): the measured curves of Ref. [14] are not in the container."""
+    lam = LAMBDA_MIN_NM + 0.5 + np.arange(400)                       # centres of the 1 nm bins
+    centre33 = LAMBDA_MIN_NM + 33.0 * (np.floor((lam - LAMBDA_MIN_NM) / 33.0) + 0.5)
+    centre25 = LAMBDA_MIN_NM + 25.0 * (np.floor((lam - LAMBDA_MIN_NM) / 25.0) + 0.5)
+    qe = 0.35 * np.exp(-0.5 * ((centre33 - 450.0) / 110.0) ** 2)
+    refl = 0.94 - 0.05 * (centre25 - 212.5) / 375.0
     return refl, qe
 
 
@@ -162,10 +178,15 @@ def toy_rich_scene(tables="c2", cells=100, enclosure=True):
     dv = np.cross(-r, du)
 
     sc = Scene()
-    refl, qe = flat_tables() if tables == "flat" else c2_tables()
-    m_abs = sc.add_material(MAT_ABSORBER, np.zeros(N_LAMBDA))
-    m_mir = sc.add_material(MAT_MIRROR, refl)
-    m_det = sc.add_material(MAT_DETECTOR, qe)
+    interp = TABLE_LINEAR
+    if tables == "paper_hist":
+        sc.n_lambda, interp = 400, TABLE_HISTOGRAM
+        refl, qe = paper_histogram_tables()
+    else:
+        refl, qe = flat_tables() if tables == "flat" else c2_tables()
+    m_abs = sc.add_material(MAT_ABSORBER, np.zeros(sc.n_lambda))
+    m_mir = sc.add_material(MAT_MIRROR, refl, interp)
+    m_det = sc.add_material(MAT_DETECTOR, qe, interp)
 
     step = 2 * half / cells
     sag = lambda X, Y: (R - np.sqrt(R * R - (X - half) ** 2 - (Y - half) ** 2))[..., None] * a
@@ -186,7 +207,8 @@ def toy_rich_scene(tables="c2", cells=100, enclosure=True):
         bv, bt = _box(lo, hi)
         sc.add_mesh("enclosure", bv, bt, m_abs)
 
-    sc.info = dict(R=R, tilt=tilt, V=V, C=C, a=a, ex=ex, ey=ey, half=half, r=r, D=D, du=du, dv=dv,
+    sc.info = dict(m_abs=m_abs, m_mir=m_mir, m_det=m_det,
+                   R=R, tilt=tilt, V=V, C=C, a=a, ex=ex, ey=ey, half=half, r=r, D=D, du=du, dv=dv,
                    facet_circumradius=step * np.sqrt(2) / 2, pixel_grid=npix)
     return sc
 
