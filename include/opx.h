@@ -69,11 +69,25 @@ typedef struct {
     float t_min_mm;                     /* minimum hit distance after a bounce (1e-3), >= 0   */
 } opx_scene_params;
 
+/* Form of a material's efficiency table.
+ *   LINEAR     n_lambda points on the uniform grid lambda_min..lambda_max, piecewise linear, clamped;
+ *   HISTOGRAM  the paper's form ("histograms of 33 nm bin width", "bins of 25 nm"): the
+ *              n_lambda values are the contents of n_lambda equal bins tiling [lambda_min, lambda_max]; lower
+ *              bin edges inclusive, the end bins extend outwards. */
+typedef enum { OPX_TABLE_LINEAR = 0, OPX_TABLE_HISTOGRAM = 1 } opx_table_interp;
+
 typedef struct {
     uint32_t kind;      /* opx_mat_kind                                                        */
+    uint32_t interp;    /* opx_table_interp                                                    */
     const float* table; /* HOST, n_lambda values in [0,1]: reflectivity (mirror) or QE         */
                         /* (detector); ignored (may be NULL) for an absorber                   */
 } opx_material;
+
+/* Flags of opx_propagate_flags. */
+typedef enum {
+    OPX_FLAG_NO_EFFICIENCY = 1 /* efficiencies were applied before propagation (opx_prefilter): every mirror
+                                  reflects, every detector pixel detects, no random number is drawn */
+} opx_flags;
 
 /* Detector pixel grid: a point p maps to a = (p-A).u, b = (p-A).v,
  * iu = floor(a / pitch_u), iv = floor(b / pitch_v); inside iff 0 <= iu < nu and 0 <= iv < nv;
@@ -165,6 +179,34 @@ opx_status opx_propagate(const opx_scene* scene, uint64_t n, uint64_t photon_id_
                          const float* d_origins, const float* d_dirs, const float* d_wavelengths,
                          uint64_t seed, const opx_hits* out, uint32_t* d_hitmap, uint64_t* d_counters,
                          void* cuda_stream);
+
+/* opx_propagate with `flags` (opx_flags, 0 = opx_propagate) and an optional photon count that lives on the
+ * device: if d_n is not NULL the kernels propagate min(n, *d_n) photons (read when the kernels run, so the count
+ * written by opx_prefilter on the same stream is used without a host round trip); records beyond it are left
+ * untouched.  n then only bounds the launch and the arrays. */
+opx_status opx_propagate_flags(const opx_scene* scene, uint64_t n, const uint64_t* d_n, uint64_t photon_id_base,
+                               const float* d_origins, const float* d_dirs, const float* d_wavelengths,
+                               uint64_t seed, uint32_t flags, const opx_hits* out, uint32_t* d_hitmap,
+                               uint64_t* d_counters, void* cuda_stream);
+
+/* Pre-propagation efficiency filter, the paper's own method ("it is advantageous to apply any
+ * quantum efficiency and reflectivity effects prior to propagation and discard the associated photons ... For
+ * each photon, with its specific wavelength, an accept-reject algorithm was used to model the three
+ * efficiencies before propagation").  DESIGN.md 3.9: photon i is kept iff
+ *     U(seed, photon_id_base + i, 0; stream 1)  <  e_0(lambda_i) * e_1(lambda_i) * ... (left to right, fp32),
+ * e_k = the table of material factors[k] (HOST array of n_factors <= 8 material indices, e.g. detector, mirror 1,
+ * mirror 2; a material may repeat; n_factors = 0 keeps everything).  The kept photons are written in input
+ * order (stable compaction) to d_out_origins / d_out_dirs (x3) / d_out_wavelengths, their index i to
+ * d_out_index (may be NULL), and their number to *d_n_kept (DEVICE uint64, overwritten).  All out arrays hold
+ * n entries; they must not alias the inputs.  n <= 2^32 - 1.  Trace the survivors with
+ * opx_propagate_flags(..., n, d_n_kept, ..., OPX_FLAG_NO_EFFICIENCY, ...).
+ * d_workspace: opx_prefilter_workspace_bytes(n) device bytes, 256-byte aligned. */
+opx_status opx_prefilter_workspace_bytes(uint64_t n, size_t* bytes);
+opx_status opx_prefilter(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
+                         const float* d_dirs, const float* d_wavelengths, uint64_t seed,
+                         const uint32_t* factors, uint32_t n_factors,
+                         float* d_out_origins, float* d_out_dirs, float* d_out_wavelengths, uint32_t* d_out_index,
+                         uint64_t* d_n_kept, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* Same computation with the closest hit found by testing EVERY triangle on the GPU (no BVH
  * traversal).  A debugging aid that separates the arithmetic of DESIGN.md section 3 from the BVH;

@@ -72,13 +72,15 @@ opx_status opx_scene_create(const opx_scene_params* params, const opx_mesh* mesh
     auto* s = new opx_scene();
     s->params = *params;
     s->inv_dlambda = (float)((double)(params->n_lambda - 1) / ((double)params->lambda_max_nm - (double)params->lambda_min_nm));
+    s->inv_bin = (float)((double)params->n_lambda / ((double)params->lambda_max_nm - (double)params->lambda_min_nm));
     auto bail = [&](const std::string& m) { delete s; return fail(OPX_ERR_INVALID_ARG, m); };
 
     s->mat_kinds.resize(n_materials);
     s->tables.assign((size_t)n_materials * params->n_lambda, 0.f);
     for (uint32_t m = 0; m < n_materials; ++m) {
         if (materials[m].kind > OPX_MAT_DETECTOR) return bail("material kind out of range");
-        s->mat_kinds[m] = materials[m].kind;
+        if (materials[m].interp > OPX_TABLE_HISTOGRAM) return bail("material table form out of range");
+        s->mat_kinds[m] = materials[m].kind | (materials[m].interp << 8);
         if (materials[m].kind == OPX_MAT_ABSORBER) continue;
         if (!materials[m].table) return bail("mirror/detector material without a table");
         for (uint32_t j = 0; j < params->n_lambda; ++j) {
@@ -112,7 +114,7 @@ opx_status opx_scene_create(const opx_scene_params* params, const opx_mesh* mesh
     for (uint32_t k = 0; k < n_meshes; ++k) {
         const opx_mesh& m = meshes[k];
         if (m.material >= n_materials) return bail("mesh material index out of range");
-        const bool det = s->mat_kinds[m.material] == OPX_MAT_DETECTOR;
+        const bool det = (s->mat_kinds[m.material] & 0xffu) == OPX_MAT_DETECTOR;
         if (det && (m.pixel_frame < 0 || (uint32_t)m.pixel_frame >= n_frames)) return bail("detector mesh needs a valid pixel frame");
         s->surfaces[k] = make_int2((int)m.material, det ? m.pixel_frame : -1);
         if (m.n_triangles && (!m.vertices || !m.indices)) return bail("mesh vertices/indices is NULL");
@@ -161,8 +163,8 @@ opx_status opx_bvh_build(opx_scene* scene, void* d_scene_ws, size_t scene_bytes,
     return OPX_OK;
 }
 
-static opx_status propagate_common(const opx_scene* scene, bool brute, uint64_t n, uint64_t base,
-                                   const float* o, const float* d, const float* wl, uint64_t seed,
+static opx_status propagate_common(const opx_scene* scene, bool brute, uint64_t n, const uint64_t* d_n, uint64_t base,
+                                   const float* o, const float* d, const float* wl, uint64_t seed, uint32_t flags,
                                    const opx_hits* out, uint32_t* hitmap, uint64_t* counters, void* stream) {
     if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
     if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate before opx_bvh_build");
@@ -175,21 +177,66 @@ static opx_status propagate_common(const opx_scene* scene, bool brute, uint64_t 
         misaligned(out->pixel, 4) || misaligned(out->surface, 4) || misaligned(hitmap, 4) || misaligned(counters, 8))
         return fail(OPX_ERR_INVALID_ARG, "misaligned pointer");
     if (n > (1ull << 40)) return fail(OPX_ERR_INVALID_ARG, "n too large for one call");
+    if (flags & ~(uint32_t)OPX_FLAG_NO_EFFICIENCY) return fail(OPX_ERR_INVALID_ARG, "unknown flag");
+    if (misaligned(d_n, 8)) return fail(OPX_ERR_INVALID_ARG, "misaligned d_n");
     if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_propagate")) return st;
-    return launch_propagate(*scene, brute, n, base, o, d, wl, seed, *out, hitmap, counters, (cudaStream_t)stream);
+    return launch_propagate(*scene, brute, n, d_n, base, o, d, wl, seed, flags, *out, hitmap, counters, (cudaStream_t)stream);
 }
 
 opx_status opx_propagate(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
                          const float* d_dirs, const float* d_wavelengths, uint64_t seed, const opx_hits* out,
                          uint32_t* d_hitmap, uint64_t* d_counters, void* cuda_stream) {
-    return propagate_common(scene, false, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, out, d_hitmap,
+    return propagate_common(scene, false, n, nullptr, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, 0u, out, d_hitmap,
                             d_counters, cuda_stream);
+}
+
+opx_status opx_propagate_flags(const opx_scene* scene, uint64_t n, const uint64_t* d_n, uint64_t photon_id_base,
+                               const float* d_origins, const float* d_dirs, const float* d_wavelengths,
+                               uint64_t seed, uint32_t flags, const opx_hits* out, uint32_t* d_hitmap,
+                               uint64_t* d_counters, void* cuda_stream) {
+    return propagate_common(scene, false, n, d_n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, flags, out, d_hitmap,
+                            d_counters, cuda_stream);
+}
+
+opx_status opx_prefilter_workspace_bytes(uint64_t n, size_t* bytes) {
+    if (!bytes) return fail(OPX_ERR_INVALID_ARG, "bytes is NULL");
+    if (n > 0xffffffffull) return fail(OPX_ERR_INVALID_ARG, "n must be <= 2^32 - 1");
+    *bytes = prefilter_workspace_bytes(n);
+    return OPX_OK;
+}
+
+opx_status opx_prefilter(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
+                         const float* d_dirs, const float* d_wavelengths, uint64_t seed,
+                         const uint32_t* factors, uint32_t n_factors,
+                         float* d_out_origins, float* d_out_dirs, float* d_out_wavelengths, uint32_t* d_out_index,
+                         uint64_t* d_n_kept, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_prefilter before opx_bvh_build");
+    if (!d_n_kept || misaligned(d_n_kept, 8)) return fail(OPX_ERR_INVALID_ARG, "d_n_kept is NULL or misaligned");
+    if (n > 0xffffffffull) return fail(OPX_ERR_INVALID_ARG, "n must be <= 2^32 - 1");
+    if (n_factors > 8 || (n_factors && !factors)) return fail(OPX_ERR_INVALID_ARG, "n_factors must be <= 8 and factors non-NULL");
+    for (uint32_t k = 0; k < n_factors; ++k) {
+        if (factors[k] >= scene->mat_kinds.size()) return fail(OPX_ERR_INVALID_ARG, "factor material index out of range");
+        if ((scene->mat_kinds[factors[k]] & 0xffu) == OPX_MAT_ABSORBER) return fail(OPX_ERR_INVALID_ARG, "an absorber has no efficiency table");
+    }
+    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_prefilter")) return st;
+    if (n == 0) return check_cuda(cudaMemsetAsync(d_n_kept, 0, 8, (cudaStream_t)cuda_stream), "cudaMemsetAsync");
+    if (!d_origins || !d_dirs || !d_wavelengths || !d_out_origins || !d_out_dirs || !d_out_wavelengths || !d_workspace)
+        return fail(OPX_ERR_INVALID_ARG, "NULL photon/workspace pointer");
+    if (misaligned(d_origins, 4) || misaligned(d_dirs, 4) || misaligned(d_wavelengths, 4) || misaligned(d_out_origins, 4) ||
+        misaligned(d_out_dirs, 4) || misaligned(d_out_wavelengths, 4) || misaligned(d_out_index, 4) || misaligned(d_workspace, 256))
+        return fail(OPX_ERR_INVALID_ARG, "misaligned pointer");
+    if (d_out_origins == d_origins || d_out_dirs == d_dirs || d_out_wavelengths == d_wavelengths)
+        return fail(OPX_ERR_INVALID_ARG, "out arrays must not alias the inputs");
+    if (workspace_bytes < prefilter_workspace_bytes(n)) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_prefilter_workspace_bytes)");
+    return launch_prefilter(*scene, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, factors, n_factors, d_out_origins,
+                            d_out_dirs, d_out_wavelengths, d_out_index, d_n_kept, d_workspace, (cudaStream_t)cuda_stream);
 }
 
 opx_status opx_propagate_brute(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
                                const float* d_dirs, const float* d_wavelengths, uint64_t seed, const opx_hits* out,
                                uint32_t* d_hitmap, uint64_t* d_counters, void* cuda_stream) {
-    return propagate_common(scene, true, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, out, d_hitmap,
+    return propagate_common(scene, true, n, nullptr, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, 0u, out, d_hitmap,
                             d_counters, cuda_stream);
 }
 
@@ -262,7 +309,7 @@ opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photo
         cudaMemcpyAsync(s.d, h_dirs + 3 * done, m * 12, cudaMemcpyHostToDevice, s.st);
         cudaMemcpyAsync(s.wl, h_wavelengths + done, m * 4, cudaMemcpyHostToDevice, s.st);
         opx_hits dev_out{s.pos, s.dir, s.pixel, s.surface, s.state, s.bounces};
-        st = launch_propagate(*scene, false, m, photon_id_base + done, s.o, s.d, s.wl, seed, dev_out, d_hitmap,
+        st = launch_propagate(*scene, false, m, nullptr, photon_id_base + done, s.o, s.d, s.wl, seed, 0u, dev_out, d_hitmap,
                               d_counters, s.st);
         cudaMemcpyAsync(h_out->pos + 3 * done, s.pos, m * 12, cudaMemcpyDeviceToHost, s.st);
         cudaMemcpyAsync(h_out->dir + 3 * done, s.dir, m * 12, cudaMemcpyDeviceToHost, s.st);

@@ -10,12 +10,14 @@ namespace {
 // __match_any_sync so that a ring concentrated on a few hundred pixels costs one atomic per
 // distinct pixel per warp.  Integer adds only, so the result does not depend on the order.
 __global__ void __launch_bounds__(256) k_bin(const uint8_t* __restrict__ state, const uint8_t* __restrict__ bounces,
-                                             const int32_t* __restrict__ pixel, uint64_t n, uint32_t* hitmap,
+                                             const int32_t* __restrict__ pixel, uint64_t n,
+                                             const unsigned long long* __restrict__ d_n, uint32_t* hitmap,
                                              unsigned long long* counters) {
     __shared__ unsigned int s_cnt[8];
     if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0;
     __syncthreads();
     const int lane = threadIdx.x & 31;
+    if (d_n) n = min(n, (uint64_t)__ldg(d_n));
     unsigned int seg_local = 0;
     for (uint64_t base = (blockIdx.x * (uint64_t)blockDim.x + threadIdx.x) - lane; base < n; base += (uint64_t)gridDim.x * blockDim.x) {
         const uint64_t i = base + lane;

@@ -512,6 +512,7 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
     d.beam_max_width = kBeamWidthInTriangles * tri_size;
     d.beam_max_spread = scene_ext > 0.f ? d.beam_max_width / (0.5f * scene_ext) : 0.f;
     d.lambda_min = s.params.lambda_min_nm; d.inv_dlambda = s.inv_dlambda; d.t_min = s.params.t_min_mm;
+    d.inv_bin = s.inv_bin; d.flags = 0; d.d_n = nullptr;
     return OPX_OK;
 }
 

@@ -9,9 +9,10 @@ namespace opx {
 __device__ constexpr float kInf = __builtin_huge_valf();
 
 // ---------------------------------------------------------------------------- Philox4x32-10 (3.1)
-__device__ __forceinline__ float philox_uniform(uint64_t seed, uint64_t g, uint32_t b) {
+// `stream` is counter word 3: 0 = in-flight draws (3.1), 1 = the pre-propagation filter (3.9).
+__device__ __forceinline__ float philox_uniform(uint64_t seed, uint64_t g, uint32_t b, uint32_t stream = 0u) {
     const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
-    uint32_t c0 = (uint32_t)g, c1 = (uint32_t)(g >> 32), c2 = b, c3 = 0u;
+    uint32_t c0 = (uint32_t)g, c1 = (uint32_t)(g >> 32), c2 = b, c3 = stream;
     uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
@@ -39,6 +40,24 @@ __device__ __forceinline__ float table_lerp(const float* __restrict__ y, uint32_
     if (f > 1.f) f = 1.f;
     const float y0 = __ldg(y + j), y1 = __ldg(y + j + 1);
     return __fmaf_rn(f, __fsub_rn(y1, y0), y0);
+}
+
+// ------------------------------------------------------------------------ histogram lookup (3.8)
+__device__ __forceinline__ float table_hist(const float* __restrict__ y, uint32_t n_lambda, float lambda_min,
+                                            float inv_bin, float lambda) {
+    const float xf = floorf(__fmul_rn(__fsub_rn(lambda, lambda_min), inv_bin));
+    int j;
+    if (!(xf >= 0.f)) j = 0;
+    else if (xf > (float)(n_lambda - 1)) j = (int)n_lambda - 1;
+    else j = (int)xf;
+    return __ldg(y + j);
+}
+
+// e_m(lambda): efficiency of material m in its own table form; mk = mat_kinds[m] (kind | interp << 8).
+__device__ __forceinline__ float table_value(const SceneDev& sc, uint32_t m, uint32_t mk, float lambda) {
+    const float* y = sc.tables + (size_t)m * sc.n_lambda;
+    if ((mk >> 8) == OPX_TABLE_HISTOGRAM) return table_hist(y, sc.n_lambda, sc.lambda_min, sc.inv_bin, lambda);
+    return table_lerp(y, sc.n_lambda, sc.lambda_min, sc.inv_dlambda, lambda);
 }
 
 // ------------------------------------------------------------------------------- ray set-up (3.3)
@@ -143,12 +162,11 @@ __device__ __forceinline__ bool interact(const SceneDev& sc, const Hit& h, Photo
     const float4 nrm = __ldg(sc.normals + h.j);
     p.surface = __float_as_int(nrm.w);
     const int2 sf = __ldg(sc.surfaces + p.surface);
-    const uint32_t kind = __ldg(sc.mat_kinds + sf.x);
-    const float* table = sc.tables + (size_t)sf.x * sc.n_lambda;
+    const uint32_t mk = __ldg(sc.mat_kinds + sf.x), kind = mk & 0xffu;
+    const bool draw = !(sc.flags & OPX_FLAG_NO_EFFICIENCY);                                       // 3.10
     if (kind == OPX_MAT_ABSORBER) { p.state = OPX_ABSORBED_SURFACE; return false; }
     if (kind == OPX_MAT_MIRROR) {
-        const float u = philox_uniform(seed, p.g, p.b);
-        if (!(u < table_lerp(table, sc.n_lambda, sc.lambda_min, sc.inv_dlambda, p.lambda))) { p.state = OPX_ABSORBED_MIRROR; return false; }
+        if (draw && !(philox_uniform(seed, p.g, p.b) < table_value(sc, (uint32_t)sf.x, mk, p.lambda))) { p.state = OPX_ABSORBED_MIRROR; return false; }
         const float c = __fmaf_rn(p.dz, nrm.z, __fmaf_rn(p.dy, nrm.y, __fmul_rn(p.dx, nrm.x)));   // 3.5
         const float m2c = __fmul_rn(-2.f, c);
         p.dx = __fmaf_rn(m2c, nrm.x, p.dx); p.dy = __fmaf_rn(m2c, nrm.y, p.dy); p.dz = __fmaf_rn(m2c, nrm.z, p.dz);
@@ -166,8 +184,7 @@ __device__ __forceinline__ bool interact(const SceneDev& sc, const Hit& h, Photo
     const float fu = floorf(__fmul_rn(ca, f2.y)), fv = floorf(__fmul_rn(cb, f2.z));
     if (!(fu >= 0.f) || !(fv >= 0.f) || !(fu < (float)f3.x) || !(fv < (float)f3.y)) { p.state = OPX_DETECTOR_DEAD; return false; }
     p.pixel = (int)(f3.z + (uint32_t)fv * f3.x + (uint32_t)fu);
-    const float u = philox_uniform(seed, p.g, p.b);
-    p.state = (u < table_lerp(table, sc.n_lambda, sc.lambda_min, sc.inv_dlambda, p.lambda)) ? OPX_DETECTED : OPX_QE_REJECTED;
+    p.state = (!draw || philox_uniform(seed, p.g, p.b) < table_value(sc, (uint32_t)sf.x, mk, p.lambda)) ? OPX_DETECTED : OPX_QE_REJECTED;
     return false;
 }
 

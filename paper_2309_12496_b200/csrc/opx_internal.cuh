@@ -41,11 +41,14 @@ struct SceneDev {
     const float4* tris;        // 3 per triangle, leaf order: (a.xyz, id bits) (b.xyz, surface bits) (c.xyz, 0)
     const float4* normals;     // leaf order: n.xyz, surface id bits
     const int2* surfaces;      // (material, frame)
-    const uint32_t* mat_kinds;
+    const uint32_t* mat_kinds; // opx_mat_kind | opx_table_interp << 8
     const float* tables;       // n_materials x n_lambda
     const FrameDev* frames;
     uint32_t n_tri, n_nodes, n_wnodes, n_lambda, max_bounces;
     float lambda_min, inv_dlambda, t_min;
+    float inv_bin;             // histogram tables: n_lambda / (lambda_max - lambda_min)
+    uint32_t flags;            // opx_flags of this launch (set per call, 0 in the stored copy)
+    const unsigned long long* d_n;   // optional device-side photon count of this launch (min(n, *d_n) photons), else NULL
     float beam_max_width, beam_max_spread;   // packets wider than this (origins [mm] / directions) walk the binary tree
 };
 
@@ -62,7 +65,7 @@ struct SceneHost {
     std::vector<float> tables;       // M x n_lambda
     std::vector<FrameDev> frames;
     uint64_t n_pixels = 0;
-    float inv_dlambda = 0.f;
+    float inv_dlambda = 0.f, inv_bin = 0.f;
     // set by opx_bvh_build
     bool built = false;
     void* d_scene_ws = nullptr;
@@ -85,9 +88,14 @@ void compute_layout(const SceneHost& s, opx_scene_layout* lay, size_t* tmp_bytes
 opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_t stream);
 
 // propagate (opx_propagate.cu)
-opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, uint64_t id_base, const float* o,
-                            const float* d, const float* wl, uint64_t seed, const opx_hits& out,
+opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
+                            const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_hits& out,
                             uint32_t* hitmap, uint64_t* counters, cudaStream_t stream);
+// pre-propagation filter (opx_prefilter.cu)
+size_t prefilter_workspace_bytes(uint64_t n);
+opx_status launch_prefilter(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d, const float* wl,
+                            uint64_t seed, const uint32_t* factors, uint32_t n_factors, float* oo, float* od, float* owl,
+                            uint32_t* oidx, uint64_t* d_n_kept, void* ws, cudaStream_t stream);
 opx_status launch_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,
                         const float* wl, uint64_t seed, uint64_t* stats, cudaStream_t stream);
 opx_status launch_packet_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,

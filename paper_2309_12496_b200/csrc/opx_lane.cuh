@@ -64,6 +64,7 @@ __global__ void __launch_bounds__(128) k_propagate_lane(const SceneDev sc, uint6
                                                         const float* __restrict__ wl, uint64_t seed, opx_hits out,
                                                         unsigned long long* stats) {
     const uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
+    if (sc.d_n) n = min(n, (uint64_t)__ldg(sc.d_n));
     if (i >= n) return;
     Photon p;
     photon_init(p, origins[3 * i], origins[3 * i + 1], origins[3 * i + 2], dirs[3 * i], dirs[3 * i + 1], dirs[3 * i + 2], wl[i], id_base + i);

@@ -200,6 +200,8 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
     PacketSmem& sm = *reinterpret_cast<PacketSmem*>(smem_raw);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const uint64_t tile_base = (uint64_t)blockIdx.x * kTile;
+    if (sc.d_n) n = min(n, (uint64_t)__ldg(sc.d_n));       // photon count left on the device by opx_prefilter
+    if (tile_base >= n) return;
     const int m = (int)min((uint64_t)kTile, n - tile_base);
     if (threadIdx.x == 0) sm.next_group = 0;
 

@@ -8,9 +8,12 @@
 
 namespace opx {
 
-static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t n, uint64_t id_base, const float* o, const float* d,
-                                        const float* wl, uint64_t seed, const opx_hits& out, uint32_t* hitmap, uint64_t* counters,
-                                        uint64_t* packet_stats, cudaStream_t stream) {
+static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
+                                        const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_hits& out,
+                                        uint32_t* hitmap, uint64_t* counters, uint64_t* packet_stats, cudaStream_t stream) {
+    SceneDev dev = s.dev;          // per-launch copy: flags and the optional device-side count ride in the kernel parameter
+    dev.flags = flags;
+    dev.d_n = (const unsigned long long*)d_n;
     cudaEvent_t* ev = nullptr;
     if (s.prof_used < s.prof_max) { ev = &s.prof_events[3 * (size_t)s.prof_used]; ++s.prof_used; }
     if (ev) cudaEventRecord(ev[0], stream);
@@ -18,7 +21,7 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
         // debug mode, or a scene with fewer than two triangles (no hierarchy): test the triangle list directly
         const uint64_t blocks = (n + 127) / 128;
         if (blocks > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
-        k_propagate_lane<true, false><<<(unsigned)blocks, 128, 0, stream>>>(s.dev, n, id_base, o, d, wl, seed, out, nullptr);
+        k_propagate_lane<true, false><<<(unsigned)blocks, 128, 0, stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr);
     } else {
         static bool configured = false;
         if (!configured) {
@@ -30,31 +33,31 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
         }
         const uint64_t tiles = (n + kTile - 1) / kTile;
         if (tiles > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
-        if (packet_stats) k_propagate_packet<true><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(s.dev, n, id_base, o, d, wl, seed, out, (unsigned long long*)packet_stats);
-        else k_propagate_packet<false><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(s.dev, n, id_base, o, d, wl, seed, out, nullptr);
+        if (packet_stats) k_propagate_packet<true><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(dev, n, id_base, o, d, wl, seed, out, (unsigned long long*)packet_stats);
+        else k_propagate_packet<false><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr);
     }
     count_launch(1);
     if (ev) cudaEventRecord(ev[1], stream);
     if (hitmap || counters) {
         const uint64_t bb = (n + 255) / 256;
         const unsigned grid = (unsigned)(bb < 148ull * 8 ? bb : 148ull * 8);
-        k_bin<<<grid, 256, 0, stream>>>(out.state, out.bounces, out.pixel, n, hitmap, (unsigned long long*)counters);
+        k_bin<<<grid, 256, 0, stream>>>(out.state, out.bounces, out.pixel, n, (const unsigned long long*)d_n, hitmap, (unsigned long long*)counters);
         count_launch(1);
     }
     if (ev) cudaEventRecord(ev[2], stream);
     return check_cuda(cudaGetLastError(), "propagate launch");
 }
 
-opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, uint64_t id_base, const float* o, const float* d,
-                            const float* wl, uint64_t seed, const opx_hits& out, uint32_t* hitmap, uint64_t* counters,
-                            cudaStream_t stream) {
-    return launch_propagate_impl(s, brute, n, id_base, o, d, wl, seed, out, hitmap, counters, nullptr, stream);
+opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
+                            const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_hits& out, uint32_t* hitmap,
+                            uint64_t* counters, cudaStream_t stream) {
+    return launch_propagate_impl(s, brute, n, d_n, id_base, o, d, wl, seed, flags, out, hitmap, counters, nullptr, stream);
 }
 
 opx_status launch_packet_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,
                                const float* wl, uint64_t seed, const opx_hits& out, uint64_t* stats, cudaStream_t stream) {
     if (s.dev.n_tri < 2) return fail(OPX_ERR_BAD_STATE, "no hierarchy to instrument (fewer than two triangles)");
-    return launch_propagate_impl(s, false, n, id_base, o, d, wl, seed, out, nullptr, nullptr, stats, stream);
+    return launch_propagate_impl(s, false, n, nullptr, id_base, o, d, wl, seed, 0u, out, nullptr, nullptr, stats, stream);
 }
 
 opx_status launch_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d, const float* wl,

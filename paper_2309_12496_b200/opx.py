@@ -18,8 +18,11 @@ STATE_NAMES = ("DETECTED", "QE_REJECTED", "ABSORBED_SURFACE", "ABSORBED_MIRROR",
 OPX_OK, OPX_ERR_INVALID_ARG, OPX_ERR_BAD_STATE, OPX_ERR_WORKSPACE_TOO_SMALL, OPX_ERR_CUDA, \
     OPX_ERR_UNSUPPORTED_DEVICE = range(6)
 
+FLAG_NO_EFFICIENCY = 1                   # opx_flags
+TABLE_LINEAR, TABLE_HISTOGRAM = 0, 1     # opx_table_interp
+
 EXPORTS = ("opx_scene_create", "opx_scene_workspace_bytes", "opx_bvh_build", "opx_propagate",
-           "opx_propagate_brute", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
+           "opx_propagate_flags", "opx_prefilter_workspace_bytes", "opx_prefilter", "opx_propagate_brute", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
            "opx_profile_begin", "opx_profile_end", "opx_propagate_stats", "opx_propagate_packet_stats",
            "opx_scene_wide_info", "opx_measure_fp32_peak",
            "opx_scene_info", "opx_scene_get_layout", "opx_launch_count", "opx_scene_destroy",
@@ -38,7 +41,7 @@ class SceneParams(C.Structure):
 
 
 class Material(C.Structure):
-    _fields_ = [("kind", C.c_uint32), ("table", C.c_void_p)]
+    _fields_ = [("kind", C.c_uint32), ("interp", C.c_uint32), ("table", C.c_void_p)]
 
 
 class PixelFrame(C.Structure):
@@ -84,6 +87,9 @@ def load_library(path=LIB_PATH):
     lib.opx_bvh_build.argtypes = [vp, vp, C.c_size_t, vp, C.c_size_t, vp]
     for f in (lib.opx_propagate, lib.opx_propagate_brute):
         f.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp, vp, vp]
+    lib.opx_propagate_flags.argtypes = [vp, u64, vp, u64, vp, vp, vp, u64, u32, vp, vp, vp, vp]
+    lib.opx_prefilter_workspace_bytes.argtypes = [u64, vp]
+    lib.opx_prefilter.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, u32, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
     lib.opx_propagate_host_workspace_bytes.argtypes = [vp, u64, vp]
     lib.opx_propagate_host.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp, vp, vp, C.c_size_t, u64, vp]
     lib.opx_profile_begin.argtypes = [vp, u32]
@@ -133,7 +139,7 @@ class Scene:
         for k, m in enumerate(scene.materials):
             t = np.ascontiguousarray(m["table"], dtype=np.float32)
             keep.append(t)
-            mats[k].kind, mats[k].table = int(m["kind"]), t.ctypes.data
+            mats[k].kind, mats[k].interp, mats[k].table = int(m["kind"]), int(m.get("interp", TABLE_LINEAR)), t.ctypes.data
         frames = (PixelFrame * max(1, len(scene.frames)))()
         for k, f in enumerate(scene.frames):
             frames[k].A[:] = [float(x) for x in f["A"]]
@@ -206,9 +212,11 @@ class Scene:
                 torch.zeros(8, dtype=torch.int64, device=device))
 
     def propagate(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, records=None, hitmap=None,
-                  counters=None, stream=None, brute=False):
+                  counters=None, stream=None, brute=False, flags=0, n_dev=None):
         """opx_propagate on device tensors.  hitmap (int32 view of uint32) and counters (int64 view of
-        uint64) are accumulated into; pass zeroed tensors or None to have them created."""
+        uint64) are accumulated into; pass zeroed tensors or None to have them created.
+        flags / n_dev (int64 CUDA tensor of one element: photon count left on the device by prefilter)
+        select opx_propagate_flags."""
         import torch
         n = int(wavelengths.shape[0])
         for t, shape in ((origins, (n, 3)), (dirs, (n, 3)), (wavelengths, (n,))):
@@ -223,11 +231,47 @@ class Scene:
             counters = ct if counters is None else counters
         h = Hits(*(records[k].data_ptr() for k in ("pos", "dir", "pixel", "surface", "state", "bounces")))
         st = stream if stream is not None else torch.cuda.current_stream(dev)
-        fn = load_library().opx_propagate_brute if brute else load_library().opx_propagate
-        _check(fn(self._h, n, int(photon_id_base), origins.data_ptr(), dirs.data_ptr(), wavelengths.data_ptr(),
-                  int(seed), C.byref(h), hitmap.data_ptr(), counters.data_ptr(), C.c_void_p(st.cuda_stream)))
+        if flags or n_dev is not None:
+            if brute:
+                raise OpxError(OPX_ERR_INVALID_ARG, "opx_propagate_brute takes no flags")
+            _check(load_library().opx_propagate_flags(
+                self._h, n, None if n_dev is None else n_dev.data_ptr(), int(photon_id_base), origins.data_ptr(),
+                dirs.data_ptr(), wavelengths.data_ptr(), int(seed), int(flags), C.byref(h), hitmap.data_ptr(),
+                counters.data_ptr(), C.c_void_p(st.cuda_stream)))
+        else:
+            fn = load_library().opx_propagate_brute if brute else load_library().opx_propagate
+            _check(fn(self._h, n, int(photon_id_base), origins.data_ptr(), dirs.data_ptr(), wavelengths.data_ptr(),
+                      int(seed), C.byref(h), hitmap.data_ptr(), counters.data_ptr(), C.c_void_p(st.cuda_stream)))
         out = dict(records)
         out["hitmap"], out["counters"] = hitmap[:self.n_pixels], counters
+        return out
+
+    def prefilter(self, origins, dirs, wavelengths, factors, seed=0, photon_id_base=0, out=None, stream=None):
+        """opx_prefilter on device tensors -> dict(origins, dirs, wavelengths, index (int32 view of uint32),
+        n_kept (int64 CUDA tensor of one element)); the first n_kept entries of the arrays are the survivors in
+        input order.  No host synchronisation: pass out["n_kept"] as `n_dev` to propagate()."""
+        import torch
+        n = int(wavelengths.shape[0])
+        dev = wavelengths.device
+        if out is None:
+            out = dict(origins=torch.empty((n, 3), dtype=torch.float32, device=dev),
+                       dirs=torch.empty((n, 3), dtype=torch.float32, device=dev),
+                       wavelengths=torch.empty(n, dtype=torch.float32, device=dev),
+                       index=torch.empty(n, dtype=torch.int32, device=dev),
+                       n_kept=torch.zeros(1, dtype=torch.int64, device=dev))
+        need = C.c_size_t()
+        _check(load_library().opx_prefilter_workspace_bytes(n, C.byref(need)))
+        ws = out.get("workspace")
+        if ws is None or ws.numel() < need.value + 256:
+            ws = out["workspace"] = torch.empty(need.value + 256, dtype=torch.uint8, device=dev)
+        fac = (C.c_uint32 * max(1, len(factors)))(*[int(f) for f in factors])
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        idx = out.get("index")
+        _check(load_library().opx_prefilter(
+            self._h, n, int(photon_id_base), origins.data_ptr(), dirs.data_ptr(), wavelengths.data_ptr(), int(seed),
+            fac, len(factors), out["origins"].data_ptr(), out["dirs"].data_ptr(), out["wavelengths"].data_ptr(),
+            None if idx is None else idx.data_ptr(), out["n_kept"].data_ptr(), _aligned(ws), need.value,
+            C.c_void_p(st.cuda_stream)))
         return out
 
     def profile_begin(self, max_calls):
