@@ -323,6 +323,45 @@ def main():
     fma = pkg.measure_fp32_peak(dev)          # FMA micro-benchmark on this device
     roof.update({"fp32_peak_measured_tflops": fma, "alu_frac_of_measured_peak": alu_achieved / fma if fma else None})
 
+    # ---- the paper's own pipeline: filter on the efficiencies first, trace
+    #      the survivors with efficiencies switched off; the survivor count never leaves the device
+    paper = None
+    if world == 1:
+        kinds = [m["kind"] for m in w.scene.materials]
+        m_mir, m_det = kinds.index(1), kinds.index(2)
+        factors = [m_det] + [m_mir] * (2 if args.config in ("C4", "C5") else 1)
+        pre = scene.prefilter(d_o, d_d, d_l, factors, seed=args.seed, photon_id_base=id_base, stream=stream)
+        hm2, ct2 = scene.alloc_accumulators(dev)
+
+        def paper_step(trace=True):
+            hm2.zero_(); ct2.zero_()
+            scene.prefilter(d_o, d_d, d_l, factors, seed=args.seed, photon_id_base=id_base, out=pre, stream=stream)
+            if trace:
+                scene.propagate(pre["origins"], pre["dirs"], pre["wavelengths"], seed=args.seed, records=records, hitmap=hm2,
+                                counters=ct2, stream=stream, flags=pkg.FLAG_NO_EFFICIENCY, n_dev=pre["n_kept"])
+        times = {}
+        for name, trace in (("pipeline", True), ("prefilter", False)):
+            for _ in range(args.warmup):
+                paper_step(trace)
+            torch.cuda.synchronize()
+            ev0.record(stream)
+            for _ in range(args.steps):
+                paper_step(trace)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            times[name] = ev0.elapsed_time(ev1) / args.steps * 1e-3
+        kept = int(pre["n_kept"].item())
+        paper_step(True)
+        torch.cuda.synchronize()
+        pf_bytes = 4 * n + 2 * (n // 8) + kept * (BYTES_IN + BYTES_IN + 4)      # lambda in, mask out + in, survivors in + out + index
+        paper = {"what": "opx_prefilter on QE x R" + (" x R" if len(factors) == 3 else "") + " then opx_propagate_flags(NO_EFFICIENCY) on the survivors",
+                 "value": n / times["pipeline"], "unit": UNIT, "ms_per_step": 1e3 * times["pipeline"],
+                 "prefilter_ms": 1e3 * times["prefilter"], "kept_fraction": kept / n, "detected": int(ct2[0].item()),
+                 "detected_in_flight": int(cnt[0]),
+                 "prefilter_roofline": {"bound": "hbm", "achieved": pf_bytes / times["prefilter"] / 1e9, "peak": peaks["hbm_gbs"],
+                                        "unit": "GB/s", "frac": pf_bytes / times["prefilter"] / 1e9 / peaks["hbm_gbs"],
+                                        "bytes_per_photon": pf_bytes / n}}
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         n_sample = min(n, args.cpu_sample)
@@ -344,7 +383,7 @@ def main():
                    "photons_per_gpu": n, "triangles": w.scene.n_triangles, "pixels": scene.n_pixels, "seed": args.seed,
                    "id_partition": "contiguous global photon-id range per rank; scene + BVH replicated"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
-        "bvh_build_ms": min(t_build), "bvh_build_launches": int(build_launches),
+        "paper_pipeline": paper, "bvh_build_ms": min(t_build), "bvh_build_launches": int(build_launches),
         "states": dict(zip(pkg.STATE_NAMES, (int(x) for x in cnt[:7]))),
         "context_paper": "paper: 1.2e6 photons/s per Tesla T4 and 2e5 per Xeon thread, end to end (PAPER.md:9); other hardware, not the target",
     }
