@@ -91,6 +91,28 @@ def _mat_interp(scene):
     return np.ascontiguousarray([m.get("interp", LINEAR) for m in scene.materials], dtype=np.uint32)
 
 
+def _tri_vnormals(scene):
+    """(T, 3, 3) vertex normals per triangle in global triangle order, zeros for a mesh without the optional
+    "vertex_normals" (V, 3) entry; None when no mesh of the scene has one."""
+    if not any(m.get("vertex_normals") is not None for m in scene.meshes):
+        return None
+    out = []
+    for m in scene.meshes:
+        idx = m["indices"].astype(np.int64)
+        vn = m.get("vertex_normals")
+        out.append(np.zeros((len(idx), 3, 3), np.float32) if vn is None else _f32(vn)[idx])
+    return np.ascontiguousarray(np.concatenate(out, axis=0))
+
+
+def shading_normal(o, d, tri, vnormals, fp64=False):
+    """Shading normal where the ray meets the triangle -> (n (3,), uvw (3,)) or None on a miss."""
+    o, d, v, n9 = _f32(o), _f32(d), _f32(tri).reshape(9), _f32(vnormals).reshape(9)
+    out, uvw = np.zeros(3), np.zeros(3)
+    if not lib().oracle_shading_normal(int(fp64), _p(o), _p(d), _p(v), _p(n9), _p(out), _p(uvw)):
+        return None
+    return out, uvw
+
+
 def prefilter(scene, wavelengths, factors, seed=0, id_base=0):
     """Pre-propagation efficiency filter: one accept-reject per photon on the product of the
     efficiencies of the materials listed in `factors`.  Returns keep (n,) uint8, index (n_kept,) uint32, prob (n,)."""
@@ -166,12 +188,13 @@ def trace_mesh(scene, origins, dirs, wavelengths, seed=0, id_base=0, ids=None, f
     return trace_mesh_arrays(tri, tri_surface, surf_mat, surf_frame, mat_kind, mat_table,
                              scene.lambda_min, scene.lambda_max, frames, len(scene.frames),
                              scene.max_bounces, scene.t_min, scene.n_pixels, o, d, wl, seed, id_base,
-                             ids, fp64, n_threads, mat_interp=_mat_interp(scene), flags=flags)
+                             ids, fp64, n_threads, mat_interp=_mat_interp(scene), flags=flags,
+                             tri_vnormal=_tri_vnormals(scene))
 
 
 def trace_mesh_arrays(tri, tri_surface, surf_mat, surf_frame, mat_kind, mat_table, lmin, lmax, frames,
                       n_frames, max_bounces, t_min, n_pixels, o, d, wl, seed=0, id_base=0, ids=None,
-                      fp64=False, n_threads=None, mat_interp=None, flags=0):
+                      fp64=False, n_threads=None, mat_interp=None, flags=0, tri_vnormal=None):
     n = len(wl)
     if n_threads is None:
         n_threads = os.cpu_count() or 1
@@ -181,8 +204,10 @@ def trace_mesh_arrays(tri, tri_surface, surf_mat, surf_frame, mat_kind, mat_tabl
                bounces=np.zeros(n, np.uint8), segments=np.zeros(n, np.uint32),
                hitmap=np.zeros(max(1, n_pixels), np.uint32), counters=np.zeros(8, np.uint64))
     interp_arr = None if mat_interp is None else np.ascontiguousarray(mat_interp, dtype=np.uint32)
-    rc = lib().oracle_trace_mesh_ex(
-        C.c_int(int(fp64)), _p(interp_arr), C.c_uint32(flags), _p(tri), _p(tri_surface), C.c_uint64(len(tri_surface)),
+    vn_arr = None if tri_vnormal is None else np.ascontiguousarray(tri_vnormal, dtype=np.float32).reshape(-1, 9)
+    assert vn_arr is None or len(vn_arr) == len(tri_surface)
+    rc = lib().oracle_trace_mesh_ex2(
+        C.c_int(int(fp64)), _p(interp_arr), C.c_uint32(flags), _p(vn_arr), _p(tri), _p(tri_surface), C.c_uint64(len(tri_surface)),
         _p(surf_mat), _p(surf_frame), C.c_uint32(len(surf_mat)),
         _p(mat_kind), _p(mat_table), C.c_uint32(len(mat_kind)), C.c_uint32(mat_table.shape[1]),
         C.c_float(lmin), C.c_float(lmax), frames, C.c_uint32(n_frames),

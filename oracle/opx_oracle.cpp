@@ -148,9 +148,11 @@ template <typename R> RaySetup<R> ray_setup(const Vec3<R>& o, const Vec3<R>& d) 
 }
 
 // Returns true and t when the ray hits triangle (a,b,c) with t > tmin and t finite.
+// uvw (optional) receives the edge functions U, V, W as computed in Real: the unnormalised barycentric
+// weights of a, b, c at the hit (they sum to det), used by the shading normal of DESIGN.md 3.11.
 template <typename R>
 bool hit_triangle(const RaySetup<R>& rs, const Vec3<R>& a, const Vec3<R>& b, const Vec3<R>& c,
-                  R tmin, R* t_out) {
+                  R tmin, R* t_out, R* uvw = nullptr) {
     const Vec3<R> A{a.x - rs.o.x, a.y - rs.o.y, a.z - rs.o.z};
     const Vec3<R> B{b.x - rs.o.x, b.y - rs.o.y, b.z - rs.o.z};
     const Vec3<R> C{c.x - rs.o.x, c.y - rs.o.y, c.z - rs.o.z};
@@ -184,6 +186,7 @@ bool hit_triangle(const RaySetup<R>& rs, const Vec3<R>& a, const Vec3<R>& b, con
     }
     if (!std::isfinite(t) || !(t > tmin)) return false;
     *t_out = t;
+    if (uvw) { uvw[0] = U; uvw[1] = V; uvw[2] = W; }
     return true;
 }
 
@@ -204,6 +207,24 @@ template <typename R> Vec3<R> face_normal(const float* v /*9*/) {
     const double len = std::sqrt((nx * nx + ny * ny) + nz * nz);
     if (!(len > 0.0)) return Vec3<R>{(R)0, (R)0, (R)0};
     return Vec3<R>{(R)(nx / len), (R)(ny / len), (R)(nz / len)};
+}
+
+// DESIGN.md 3.11.  Shading normal of a mesh that carries vertex normals (an OBJ file's `vn` records; the paper
+// exports its mirrors as OBJ meshes, whose facets blur the ring): the vertex
+// normals na, nb, nc weighted by the edge functions of the hit (U weighs a, V weighs b, W weighs c; their common
+// factor 1/det drops out of the normalisation, and the sign it may carry does not matter to a reflection),
+//     m = fma(W, nc, fma(V, nb, U na)),   n = m * (1 / sqrt(fma(mz, mz, fma(my, my, mx mx)))).
+// A zero or non-finite length (a mesh without vertex normals has them all zero) falls back to the face normal.
+template <typename R>
+Vec3<R> shading_normal(const R* uvw, const float* vn /*9: na, nb, nc*/, const Vec3<R>& face) {
+    const R U = uvw[0], V = uvw[1], W = uvw[2];
+    const R mx = rfma<R>(W, (R)vn[6], rfma<R>(V, (R)vn[3], U * (R)vn[0]));
+    const R my = rfma<R>(W, (R)vn[7], rfma<R>(V, (R)vn[4], U * (R)vn[1]));
+    const R mz = rfma<R>(W, (R)vn[8], rfma<R>(V, (R)vn[5], U * (R)vn[2]));
+    const R len2 = rfma<R>(mz, mz, rfma<R>(my, my, mx * mx));
+    if (!(len2 > (R)0) || !std::isfinite(len2)) return face;
+    const R inv = (R)1 / std::sqrt(len2);
+    return Vec3<R>{mx * inv, my * inv, mz * inv};
 }
 
 // ---------------------------------------------------------------------------------- pixel map
@@ -243,6 +264,7 @@ struct SceneView {
     uint32_t max_bounces; float t_min;
     const uint32_t* mat_interp;    // M table forms (TableInterp), NULL = all linear
     uint32_t flags;                // FLAG_NO_EFFICIENCY: surfaces act with probability 1, no random draws
+    const float* tri_vnormal;      // T x 9 vertex normals (na, nb, nc) or NULL: mirrors reflect about the face normal
 };
 enum : uint32_t { FLAG_NO_EFFICIENCY = 1u };
 
@@ -266,13 +288,17 @@ Record trace_photon(const SceneView& sc, const std::vector<Vec3<R>>& normals, ui
         const R tmin = (b == 0) ? (R)0 : (R)sc.t_min;
         R t_best = std::numeric_limits<R>::infinity();
         int64_t k_best = -1;
+        R uvw_best[3] = {(R)0, (R)0, (R)0};
         for (uint64_t k = 0; k < sc.n_tri; ++k) {
             if ((int64_t)k == last) continue;
             const float* v = sc.tri + 9 * k;
-            R t;
+            R t, uvw[3];
             if (!hit_triangle<R>(rs, Vec3<R>{(R)v[0], (R)v[1], (R)v[2]}, Vec3<R>{(R)v[3], (R)v[4], (R)v[5]},
-                                 Vec3<R>{(R)v[6], (R)v[7], (R)v[8]}, tmin, &t)) continue;
-            if (t < t_best) { t_best = t; k_best = (int64_t)k; }   // ascending k: ties keep the lower id
+                                 Vec3<R>{(R)v[6], (R)v[7], (R)v[8]}, tmin, &t, uvw)) continue;
+            if (t < t_best) {                                      // ascending k: ties keep the lower id
+                t_best = t; k_best = (int64_t)k;
+                uvw_best[0] = uvw[0]; uvw_best[1] = uvw[1]; uvw_best[2] = uvw[2];
+            }
         }
         rec.segments++;
         if (k_best < 0) {
@@ -297,7 +323,8 @@ Record trace_photon(const SceneView& sc, const std::vector<Vec3<R>>& normals, ui
                     rec.state = ABSORBED_MIRROR; break;
                 }
             }
-            d = reflect<R>(d, normals[k_best]);
+            d = reflect<R>(d, sc.tri_vnormal ? shading_normal<R>(uvw_best, sc.tri_vnormal + 9 * k_best, normals[k_best])
+                                             : normals[k_best]);
             o = p; last = k_best; b++;
             if (b == sc.max_bounces) {
                 rec.state = BOUNCE_LIMIT; rec.dir[0] = d.x; rec.dir[1] = d.y; rec.dir[2] = d.z; break;
@@ -396,7 +423,7 @@ int oracle_hit_triangle(int fp64, const float* o, const float* d, const float* v
 // Trace n photons through a triangle scene.  counters: 8 uint64 (+=): one per terminal state 0..6,
 // [7] = closest-hit queries (segments).  hitmap: n_pixels uint32 (+=).  ids == NULL => global id =
 // id_base + i.
-int oracle_trace_mesh_ex(int fp64, const uint32_t* mat_interp, uint32_t flags,
+int oracle_trace_mesh_ex2(int fp64, const uint32_t* mat_interp, uint32_t flags, const float* tri_vnormal,
                       const float* tri, const int32_t* tri_surface, uint64_t n_tri,
                       const uint32_t* surf_material, const int32_t* surf_frame, uint32_t n_surf,
                       const uint32_t* mat_kind, const float* mat_table, uint32_t n_mat, uint32_t n_lambda,
@@ -415,11 +442,50 @@ int oracle_trace_mesh_ex(int fp64, const uint32_t* mat_interp, uint32_t flags,
     }
     if (mat_interp) for (uint32_t m = 0; m < n_mat; ++m) if (mat_interp[m] > TABLE_HISTOGRAM) return 5;
     SceneView sc{tri, tri_surface, n_tri, surf_material, surf_frame, n_surf, mat_kind, mat_table, n_mat,
-                 n_lambda, lambda_min, lambda_max, frames, n_frames, max_bounces, t_min, mat_interp, flags};
+                 n_lambda, lambda_min, lambda_max, frames, n_frames, max_bounces, t_min, mat_interp, flags, tri_vnormal};
     Outputs out{pos, dir, pixel, surface, tri_out, state, bounces, segments, hitmap, counters};
     if (fp64) trace_all<double>(sc, n, ids, id_base, origins, dirs, wl, seed, out, n_threads);
     else trace_all<float>(sc, n, ids, id_base, origins, dirs, wl, seed, out, n_threads);
     return 0;
+}
+
+// The form written before vertex normals existed: every mirror reflects about its face normal.
+int oracle_trace_mesh_ex(int fp64, const uint32_t* mat_interp, uint32_t flags,
+                      const float* tri, const int32_t* tri_surface, uint64_t n_tri,
+                      const uint32_t* surf_material, const int32_t* surf_frame, uint32_t n_surf,
+                      const uint32_t* mat_kind, const float* mat_table, uint32_t n_mat, uint32_t n_lambda,
+                      float lambda_min, float lambda_max, const Frame* frames, uint32_t n_frames,
+                      uint32_t max_bounces, float t_min,
+                      uint64_t n, const uint64_t* ids, uint64_t id_base,
+                      const float* origins, const float* dirs, const float* wl, uint64_t seed,
+                      double* pos, double* dir, int32_t* pixel, int32_t* surface, int32_t* tri_out,
+                      uint8_t* state, uint8_t* bounces, uint32_t* segments, uint32_t* hitmap,
+                      uint64_t* counters, int n_threads) {
+    return oracle_trace_mesh_ex2(fp64, mat_interp, flags, nullptr, tri, tri_surface, n_tri, surf_material, surf_frame, n_surf,
+                                 mat_kind, mat_table, n_mat, n_lambda, lambda_min, lambda_max, frames, n_frames, max_bounces,
+                                 t_min, n, ids, id_base, origins, dirs, wl, seed, pos, dir, pixel, surface, tri_out, state,
+                                 bounces, segments, hitmap, counters, n_threads);
+}
+
+// Shading normal at the point where the ray (o, d) meets triangle v9 with vertex normals n9.
+// Returns 0 on a miss; uvw (3, may be NULL) receives the edge functions.
+int oracle_shading_normal(int fp64, const float* o, const float* d, const float* v9, const float* n9, double* out, double* uvw_out) {
+    if (fp64) {
+        auto rs = ray_setup<double>({o[0], o[1], o[2]}, {d[0], d[1], d[2]});
+        double t, uvw[3];
+        if (!hit_triangle<double>(rs, {v9[0], v9[1], v9[2]}, {v9[3], v9[4], v9[5]}, {v9[6], v9[7], v9[8]}, 0.0, &t, uvw)) return 0;
+        const auto nn = shading_normal<double>(uvw, n9, face_normal<double>(v9));
+        out[0] = nn.x; out[1] = nn.y; out[2] = nn.z;
+        if (uvw_out) { uvw_out[0] = uvw[0]; uvw_out[1] = uvw[1]; uvw_out[2] = uvw[2]; }
+        return 1;
+    }
+    auto rs = ray_setup<float>({o[0], o[1], o[2]}, {d[0], d[1], d[2]});
+    float t, uvw[3];
+    if (!hit_triangle<float>(rs, {v9[0], v9[1], v9[2]}, {v9[3], v9[4], v9[5]}, {v9[6], v9[7], v9[8]}, 0.f, &t, uvw)) return 0;
+    const auto nn = shading_normal<float>(uvw, n9, face_normal<float>(v9));
+    out[0] = nn.x; out[1] = nn.y; out[2] = nn.z;
+    if (uvw_out) { uvw_out[0] = uvw[0]; uvw_out[1] = uvw[1]; uvw_out[2] = uvw[2]; }
+    return 1;
 }
 
 // The form every test written before the table forms and flags existed calls: linear tables, in-flight draws.

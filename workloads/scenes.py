@@ -43,11 +43,17 @@ class Scene:
     def n_pixels(self):
         return int(max((f["pixel_base"] + f["nu"] * f["nv"] for f in self.frames), default=0))
 
-    def add_mesh(self, name, vertices, indices, material, frame=-1):
+    def add_mesh(self, name, vertices, indices, material, frame=-1, vertex_normals=None):
+        """vertex_normals: optional (V, 3) unit normals (an OBJ file's `vn` records): a mirror mesh that carries
+        them reflects about the interpolated normal."""
         v = np.ascontiguousarray(np.asarray(vertices, dtype=np.float64).astype(np.float32))
         i = np.ascontiguousarray(np.asarray(indices, dtype=np.uint32).reshape(-1, 3))
+        vn = None
+        if vertex_normals is not None:
+            vn = np.ascontiguousarray(np.asarray(vertex_normals, dtype=np.float64).astype(np.float32))
+            assert vn.shape == v.shape
         self.meshes.append(dict(name=name, vertices=v, indices=i, material=int(material),
-                                frame=int(frame)))
+                                frame=int(frame), vertex_normals=vn))
         return len(self.meshes) - 1
 
     def add_material(self, kind, table, interp=TABLE_LINEAR):
@@ -159,12 +165,14 @@ def _box(lo, hi, nx=1, ny=1, nz=1):
 
 
 # ---------------------------------------------------------------------------- toy RICH
-def toy_rich_scene(tables="c2", cells=100, enclosure=True):
+def toy_rich_scene(tables="c2", cells=100, enclosure=True, smooth=False):
     """BASELINE.json configs 0-2: one spherical mirror cap (R = 2400 mm, square 800 mm
     aperture, vertex at z = 1200 mm, tilted 0.25 rad about +x) tessellated into
     2*cells^2 triangles, a 600x600 mm detector quad perpendicular to the reflected axis at
     R/2 from the mirror vertex with a 208x208 grid of 2.88 mm pixels, and an absorbing
     axis-aligned box around everything ("everything else is absorbing").
+    smooth=True gives the mirror mesh vertex normals (the unit vectors from each vertex towards the
+    centre of curvature, what an OBJ export of the sphere carries as `vn`): SURVEY.md 8(f) row f3.
     """
     R, tilt, zv, half = 2400.0, 0.25, 1200.0, 400.0
     V = np.array([0.0, 0.0, zv])
@@ -191,7 +199,7 @@ def toy_rich_scene(tables="c2", cells=100, enclosure=True):
     step = 2 * half / cells
     sag = lambda X, Y: (R - np.sqrt(R * R - (X - half) ** 2 - (Y - half) ** 2))[..., None] * a
     mv, mt = _grid_patch(V - half * ex - half * ey, ex, ey, cells, cells, step, step, lift=sag)
-    sc.add_mesh("mirror", mv, mt, m_mir)
+    sc.add_mesh("mirror", mv, mt, m_mir, vertex_normals=(C[None, :] - mv) / R if smooth else None)
 
     npix = int(np.floor(600.0 / PIXEL_PITCH_MM))              # 208
     halfgrid = 0.5 * npix * PIXEL_PITCH_MM                    # 299.52
