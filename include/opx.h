@@ -108,6 +108,10 @@ typedef struct {
     uint32_t material;       /* index into `materials`                                         */
     int32_t pixel_frame;     /* index into `frames`; required (>= 0) iff the material is a     */
                              /* detector, ignored otherwise                                    */
+    const float* vertex_normals; /* HOST, n_vertices x 3 unit normals (an OBJ file's `vn`), or NULL.  A mirror */
+                             /* mesh that carries them reflects about the normal interpolated with the hit's  */
+                             /* edge functions instead of the face    */
+                             /* normal; components must be finite.  Ignored by detectors and absorbers.       */
 } opx_mesh;
 
 /* Per-photon hit records, DEVICE pointers, each of length n (pos, dir: n x 3 packed).
@@ -139,6 +143,7 @@ typedef struct {
     uint64_t parents;     /* (2 n_triangles - 1) x 4 B: parent of internal node i / leaf T-1+i  */
     uint64_t wide_nodes;  /* (wide_node_capacity) x 896 B: 32-wide nodes collapsed from `nodes`  */
     uint64_t wide_node_capacity;
+    uint64_t vertex_normals; /* (n_triangles) x 36 B: na, nb, nc in GLOBAL triangle-id order; 16 B if no mesh has any */
     uint64_t total_bytes;
 } opx_scene_layout;
 

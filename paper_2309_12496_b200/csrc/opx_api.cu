@@ -111,6 +111,9 @@ opx_status opx_scene_create(const opx_scene_params* params, const opx_mesh* mesh
     s->tri.reserve(total * 9);
     s->tri_surface.reserve(total);
     s->surfaces.resize(n_meshes);
+    bool any_vn = false;
+    for (uint32_t k = 0; k < n_meshes; ++k) any_vn = any_vn || (meshes[k].vertex_normals && meshes[k].n_triangles);
+    if (any_vn) s->tri_vnormals.reserve(total * 9);
     for (uint32_t k = 0; k < n_meshes; ++k) {
         const opx_mesh& m = meshes[k];
         if (m.material >= n_materials) return bail("mesh material index out of range");
@@ -124,6 +127,13 @@ opx_status opx_scene_create(const opx_scene_params* params, const opx_mesh* mesh
                 if (vi >= m.n_vertices) return bail("vertex index out of range");
                 const float* v = m.vertices + 3 * (size_t)vi;
                 s->tri.push_back(v[0]); s->tri.push_back(v[1]); s->tri.push_back(v[2]);
+                if (any_vn) {
+                    for (int a = 0; a < 3; ++a) {
+                        const float x = m.vertex_normals ? m.vertex_normals[3 * (size_t)vi + a] : 0.f;
+                        if (!std::isfinite(x)) return bail("vertex normal component is not finite");
+                        s->tri_vnormals.push_back(x);
+                    }
+                }
             }
             s->tri_surface.push_back((int32_t)k);
         }

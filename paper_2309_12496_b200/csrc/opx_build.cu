@@ -377,6 +377,7 @@ void compute_layout(const SceneHost& s, opx_scene_layout* lay, size_t* tmp_bytes
     lay->parents = take((2 * T + 1) * 4);
     lay->wide_node_capacity = wide_node_capacity(T);
     lay->wide_nodes = take(lay->wide_node_capacity * sizeof(WNodeDev));
+    lay->vertex_normals = take(s.tri_vnormals.size() * 4);
     lay->total_bytes = off;
     if (tmp_bytes) {
         size_t t = 0;
@@ -422,7 +423,8 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
     if ((e = up(tmp.tri_in, s.tri.data(), T * 36)) || (e = up(tmp.surf_in, s.tri_surface.data(), T * 4)) ||
         (e = up(tmp.normals_in, s.normals.data(), T * 12)) || (e = up(surfaces, s.surfaces.data(), s.surfaces.size() * 8)) ||
         (e = up(mat_kinds, s.mat_kinds.data(), s.mat_kinds.size() * 4)) || (e = up(tables, s.tables.data(), s.tables.size() * 4)) ||
-        (e = up(frames, s.frames.data(), s.frames.size() * sizeof(FrameDev))))
+        (e = up(frames, s.frames.data(), s.frames.size() * sizeof(FrameDev))) ||
+        (e = up(ws + lay.vertex_normals, s.tri_vnormals.data(), s.tri_vnormals.size() * 4)))
         return check_cuda(e, "scene upload");
 
     // padding of the leaf boxes: 2^-16 of the largest |coordinate| (>= 128 ulp there), at least 1e-6
@@ -507,6 +509,7 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
     d.wnodes = (const WNodeDev*)(ws + lay.wide_nodes); d.n_wnodes = n_wide;
     d.nodes = nodes; d.tris = tris; d.normals = normals; d.surfaces = surfaces; d.mat_kinds = mat_kinds;
     d.tables = tables; d.frames = frames;
+    d.vnormals = s.tri_vnormals.empty() ? nullptr : (const float*)(ws + lay.vertex_normals);
     d.n_tri = (uint32_t)T; d.n_nodes = (uint32_t)(T > 1 ? T - 1 : 1);
     d.n_lambda = s.params.n_lambda; d.max_bounces = s.params.max_bounces;
     d.beam_max_width = kBeamWidthInTriangles * tri_size;

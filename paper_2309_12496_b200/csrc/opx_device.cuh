@@ -138,6 +138,32 @@ __device__ __forceinline__ void consider(const SceneDev& sc, const RayW& rw, int
     if (tt < h.t || (tt == h.t && gid < h.gid)) { h.t = tt; h.j = j; h.gid = gid; }
 }
 
+// Shading normal of DESIGN.md 3.11 for the hit on leaf-order triangle j (global id gid): the vertex normals weighted by
+// the fp32 edge functions U, V, W of 3.3, recomputed here for the one winning triangle (same operations on the same
+// inputs as tri_test, hence the same bits) so that the traversal loop does not have to carry them.  Returns false when
+// the face normal applies (no vertex normals on this triangle, or a degenerate sum).
+__device__ __forceinline__ bool shading_normal(const SceneDev& sc, const RayW& r, int j, int gid, float& nx, float& ny, float& nz) {
+    const float* t = reinterpret_cast<const float*>(sc.tris + 3 * (size_t)j);
+    const float Akx = __fsub_rn(__ldg(t + r.kx), r.okx), Aky = __fsub_rn(__ldg(t + r.ky), r.oky), Akz = __fsub_rn(__ldg(t + r.kz), r.okz);
+    const float Bkx = __fsub_rn(__ldg(t + 4 + r.kx), r.okx), Bky = __fsub_rn(__ldg(t + 4 + r.ky), r.oky), Bkz = __fsub_rn(__ldg(t + 4 + r.kz), r.okz);
+    const float Ckx = __fsub_rn(__ldg(t + 8 + r.kx), r.okx), Cky = __fsub_rn(__ldg(t + 8 + r.ky), r.oky), Ckz = __fsub_rn(__ldg(t + 8 + r.kz), r.okz);
+    const float Ax = __fmaf_rn(-r.Sx, Akz, Akx), Ay = __fmaf_rn(-r.Sy, Akz, Aky);
+    const float Bx = __fmaf_rn(-r.Sx, Bkz, Bkx), By = __fmaf_rn(-r.Sy, Bkz, Bky);
+    const float Cx = __fmaf_rn(-r.Sx, Ckz, Ckx), Cy = __fmaf_rn(-r.Sy, Ckz, Cky);
+    const float U = __fsub_rn(__fmul_rn(Cx, By), __fmul_rn(Cy, Bx));
+    const float V = __fsub_rn(__fmul_rn(Ax, Cy), __fmul_rn(Ay, Cx));
+    const float W = __fsub_rn(__fmul_rn(Bx, Ay), __fmul_rn(By, Ax));
+    const float* vn = sc.vnormals + 9 * (size_t)gid;
+    const float mx = __fmaf_rn(W, __ldg(vn + 6), __fmaf_rn(V, __ldg(vn + 3), __fmul_rn(U, __ldg(vn + 0))));
+    const float my = __fmaf_rn(W, __ldg(vn + 7), __fmaf_rn(V, __ldg(vn + 4), __fmul_rn(U, __ldg(vn + 1))));
+    const float mz = __fmaf_rn(W, __ldg(vn + 8), __fmaf_rn(V, __ldg(vn + 5), __fmul_rn(U, __ldg(vn + 2))));
+    const float len2 = __fmaf_rn(mz, mz, __fmaf_rn(my, my, __fmul_rn(mx, mx)));
+    if (!(len2 > 0.f) || !(len2 < kInf)) return false;
+    const float inv = __fdiv_rn(1.f, __fsqrt_rn(len2));
+    nx = __fmul_rn(mx, inv); ny = __fmul_rn(my, inv); nz = __fmul_rn(mz, inv);
+    return true;
+}
+
 // ------------------------------------------------------------------- photon state + interaction
 struct Photon {
     float ox, oy, oz, dx, dy, dz;      // current segment
@@ -156,7 +182,8 @@ __device__ __forceinline__ void photon_init(Photon& p, float ox, float oy, float
 
 // Applies the outcome of one closest-hit query.  Returns true when the photon
 // was reflected and continues with a new segment; otherwise p.state holds the terminal state.
-__device__ __forceinline__ bool interact(const SceneDev& sc, const Hit& h, Photon& p, uint64_t seed) {
+// rw: the watertight-test constants of the segment that produced h (needed for the shading normal only).
+__device__ __forceinline__ bool interact(const SceneDev& sc, const Hit& h, const RayW& rw, Photon& p, uint64_t seed) {
     if (h.j < 0) { p.state = OPX_ESCAPED; p.px = p.ox; p.py = p.oy; p.pz = p.oz; p.surface = -1; return false; }
     p.px = __fmaf_rn(h.t, p.dx, p.ox); p.py = __fmaf_rn(h.t, p.dy, p.oy); p.pz = __fmaf_rn(h.t, p.dz, p.oz);   // 3.7
     const float4 nrm = __ldg(sc.normals + h.j);
@@ -167,9 +194,11 @@ __device__ __forceinline__ bool interact(const SceneDev& sc, const Hit& h, Photo
     if (kind == OPX_MAT_ABSORBER) { p.state = OPX_ABSORBED_SURFACE; return false; }
     if (kind == OPX_MAT_MIRROR) {
         if (draw && !(philox_uniform(seed, p.g, p.b) < table_value(sc, (uint32_t)sf.x, mk, p.lambda))) { p.state = OPX_ABSORBED_MIRROR; return false; }
-        const float c = __fmaf_rn(p.dz, nrm.z, __fmaf_rn(p.dy, nrm.y, __fmul_rn(p.dx, nrm.x)));   // 3.5
+        float nx = nrm.x, ny = nrm.y, nz = nrm.z;
+        if (sc.vnormals) shading_normal(sc, rw, h.j, h.gid, nx, ny, nz);                           // 3.11 (face normal kept on false)
+        const float c = __fmaf_rn(p.dz, nz, __fmaf_rn(p.dy, ny, __fmul_rn(p.dx, nx)));             // 3.5
         const float m2c = __fmul_rn(-2.f, c);
-        p.dx = __fmaf_rn(m2c, nrm.x, p.dx); p.dy = __fmaf_rn(m2c, nrm.y, p.dy); p.dz = __fmaf_rn(m2c, nrm.z, p.dz);
+        p.dx = __fmaf_rn(m2c, nx, p.dx); p.dy = __fmaf_rn(m2c, ny, p.dy); p.dz = __fmaf_rn(m2c, nz, p.dz);
         p.ox = p.px; p.oy = p.py; p.oz = p.pz; p.last = h.gid; ++p.b;
         if (p.b == sc.max_bounces) { p.state = OPX_BOUNCE_LIMIT; return false; }
         return true;

@@ -40,6 +40,7 @@ struct SceneDev {
     const WNodeDev* wnodes;    // n_wnodes (0: the wide tree is not available, packets walk the binary tree)
     const float4* tris;        // 3 per triangle, leaf order: (a.xyz, id bits) (b.xyz, surface bits) (c.xyz, 0)
     const float4* normals;     // leaf order: n.xyz, surface id bits
+    const float* vnormals;     // 9 per triangle (na, nb, nc), GLOBAL id order; NULL when no mesh carries vertex normals (3.11)
     const int2* surfaces;      // (material, frame)
     const uint32_t* mat_kinds; // opx_mat_kind | opx_table_interp << 8
     const float* tables;       // n_materials x n_lambda
@@ -60,6 +61,7 @@ struct SceneHost {
     std::vector<float> tri;          // T x 9, global id order
     std::vector<int32_t> tri_surface;
     std::vector<float> normals;      // T x 3, contract 3.4
+    std::vector<float> tri_vnormals; // T x 9 (zeros for meshes without vertex normals), empty when no mesh has any
     std::vector<int2> surfaces;      // material, frame
     std::vector<uint32_t> mat_kinds;
     std::vector<float> tables;       // M x n_lambda

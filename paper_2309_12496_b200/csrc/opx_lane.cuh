@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(128) k_propagate_lane(const SceneDev sc, uint6
         if (kBrute) h = closest_hit_brute(sc, rw, tmin, p.last);
         else h = closest_hit_lane<kStats>(sc, rw, slab_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz), tmin, p.last, work);
         if (kStats) { ++segments; if (h.j >= 0) ++interactions; }
-        if (!interact(sc, h, p, seed)) break;
+        if (!interact(sc, h, rw, p, seed)) break;
     }
     if (kStats) {
         const unsigned int mask = __activemask();

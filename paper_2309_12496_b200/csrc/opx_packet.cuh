@@ -367,7 +367,7 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
                 Photon p;
                 photon_init(p, so[0], so[1], so[2], sd[0], sd[1], sd[2], sm.wl[i], id_base + tile_base + (uint64_t)i);
                 p.b = nb; p.last = last;
-                alive = interact(sc, h, p, seed);
+                alive = interact(sc, h, rw, p, seed);
                 sm.d[3 * i] = p.dx; sm.d[3 * i + 1] = p.dy; sm.d[3 * i + 2] = p.dz;
                 if (alive) {
                     sm.o[3 * i] = p.ox; sm.o[3 * i + 1] = p.oy; sm.o[3 * i + 2] = p.oz;

@@ -52,7 +52,8 @@ class PixelFrame(C.Structure):
 
 class Mesh(C.Structure):
     _fields_ = [("vertices", C.c_void_p), ("n_vertices", C.c_uint32), ("indices", C.c_void_p),
-                ("n_triangles", C.c_uint32), ("material", C.c_uint32), ("pixel_frame", C.c_int32)]
+                ("n_triangles", C.c_uint32), ("material", C.c_uint32), ("pixel_frame", C.c_int32),
+                ("vertex_normals", C.c_void_p)]
 
 
 class Hits(C.Structure):
@@ -63,7 +64,7 @@ class Hits(C.Structure):
 class SceneLayout(C.Structure):
     _fields_ = [(k, C.c_uint64) for k in ("nodes", "triangles", "normals", "surfaces", "mat_kinds", "tables",
                                           "frames", "sorted_keys", "parents", "wide_nodes", "wide_node_capacity",
-                                          "total_bytes")]
+                                          "vertex_normals", "total_bytes")]
 
 
 _lib = None
@@ -155,6 +156,12 @@ class Scene:
             meshes[k].vertices, meshes[k].n_vertices = v.ctypes.data, len(v)
             meshes[k].indices, meshes[k].n_triangles = i.ctypes.data, len(i)
             meshes[k].material, meshes[k].pixel_frame = int(m["material"]), int(m["frame"])
+            if m.get("vertex_normals") is not None:
+                vn = np.ascontiguousarray(m["vertex_normals"], dtype=np.float32)
+                if vn.shape != v.shape:
+                    raise OpxError(OPX_ERR_INVALID_ARG, "vertex_normals must have the shape of vertices")
+                keep.append(vn)
+                meshes[k].vertex_normals = vn.ctypes.data
         params = SceneParams(scene.lambda_min, scene.lambda_max, scene.n_lambda, scene.max_bounces, scene.t_min)
         handle = C.c_void_p()
         _check(lib.opx_scene_create(C.byref(params), meshes, len(scene.meshes), mats, len(scene.materials),
