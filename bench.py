@@ -112,7 +112,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{args.config}: {w.scene.n_triangles} triangles, {w.n} photons (sampled)"},
+        "config": {"workload": f"{args.config}{' + mirror vertex normals' if args.smooth else ''}: {w.scene.n_triangles} triangles, {w.n} photons (sampled)"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -169,6 +169,9 @@ def main():
     ap.add_argument("--reference-sample", type=int, default=20000)
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--smooth", action="store_true",
+                    help="toy-scene configs (C1-C3) with vertex normals on the mirror (SURVEY.md 8(f) row f3): a variant "
+                         "of the workload, named in config.workload; not the default line")
     ap.add_argument("--sweep", action="store_true",
                     help="config C5 protocol: stream --total photons through the resident batch in chunks of 1e5..1e8 "
                          "and report photons/s and HBM GB/s per chunk size instead of the default line")
@@ -199,6 +202,11 @@ def main():
     w = workloads.make_config(args.config, n=None)
     n = args.photons if args.photons else min(w.n, 100_000_000)       # per GPU per step (weak scaling)
     w = workloads.make_config(args.config, n=max(w.n, n * world))     # the job: world * n photons, ids 0..world*n
+    if args.smooth:
+        if args.config not in ("C1", "C2", "C3"):
+            raise SystemExit("--smooth: only the toy scene (C1-C3) has an analytic vertex-normal field")
+        from workloads.scenes import toy_rich_scene
+        w.scene = toy_rich_scene("flat" if args.config == "C1" else "c2", smooth=True)
     id_base, n = shard_range(n * world, rank, world)                  # contiguous global id range of this rank
     pin = [torch.empty((n, 3), dtype=torch.float32).pin_memory(), torch.empty((n, 3), dtype=torch.float32).pin_memory(),
            torch.empty(n, dtype=torch.float32).pin_memory()]
@@ -377,7 +385,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": f"{args.config}: {w.scene.n_triangles} triangles, {n} photons per GPU per step "
+        "config": {"workload": f"{args.config}{' + mirror vertex normals' if args.smooth else ''}: {w.scene.n_triangles} triangles, {n} photons per GPU per step "
                                f"({BYTES_IN + BYTES_OUT} B/photon = {(BYTES_IN + BYTES_OUT) * n / 1e6:.0f} MB per step)",
                    "l2": "inputs + outputs per step exceed the 126 MB L2" if (BYTES_IN + BYTES_OUT) * n > 126e6 else "fits in L2",
                    "photons_per_gpu": n, "triangles": w.scene.n_triangles, "pixels": scene.n_pixels, "seed": args.seed,
