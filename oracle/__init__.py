@@ -113,6 +113,21 @@ def shading_normal(o, d, tri, vnormals, fp64=False):
     return out, uvw
 
 
+def emit_cherenkov(steps, n, id_base=0, seed=0, n_index=1.0014, lambda1=200.0, lambda2=600.0):
+    """Cherenkov photons id_base .. id_base+n-1 from track steps.  `steps`: dict with x (S,3),
+    w (S,3), length (S,), beta (S,) float32 and first (S+1,) uint64.  Returns origins, dirs (n,3), wavelengths (n,)."""
+    x, w, ln, be = _f32(steps["x"]).reshape(-1, 3), _f32(steps["w"]).reshape(-1, 3), _f32(steps["length"]), _f32(steps["beta"])
+    first = np.ascontiguousarray(steps["first"], dtype=np.uint64)
+    assert len(first) == len(ln) + 1 == len(be) + 1 == len(x) + 1 == len(w) + 1
+    o, d, lam = np.zeros((n, 3), np.float32), np.zeros((n, 3), np.float32), np.zeros(n, np.float32)
+    rc = lib().oracle_emit_cherenkov(C.c_uint64(len(ln)), _p(x), _p(w), _p(ln), _p(be), _p(first), C.c_float(n_index),
+                                     C.c_float(lambda1), C.c_float(lambda2), C.c_uint64(n), C.c_uint64(id_base),
+                                     C.c_uint64(seed), _p(o), _p(d), _p(lam))
+    if rc != 0:
+        raise ValueError("oracle_emit_cherenkov: a photon id lies beyond the last step")
+    return o, d, lam
+
+
 def prefilter(scene, wavelengths, factors, seed=0, id_base=0):
     """Pre-propagation efficiency filter: one accept-reject per photon on the product of the
     efficiencies of the materials listed in `factors`.  Returns keep (n,) uint8, index (n_kept,) uint32, prob (n,)."""

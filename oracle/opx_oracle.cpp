@@ -542,6 +542,62 @@ uint64_t oracle_prefilter(const float* mat_table, const uint32_t* mat_interp, ui
     return kept;
 }
 
+// ------------------------------------------------------- Cherenkov emission from track steps (row f4)
+// DESIGN.md 3.12.  "The Cherenkov angle theta_c ... cos(theta_c) = 1/(n beta)"; photons are emitted
+// uniformly along the step, uniformly in azimuth about the track, with a wavelength density ~ 1/lambda^2.  The paper
+// leaves this to Geant4 and wants it memory-resident; here it is step by step in fp32, with the
+// azimuth drawn by Marsaglia's disc method so that no transcendental function is involved.
+// Step s: x (3), w (3, unit), L, beta; first (S+1) = exclusive prefix sum of the photon counts.
+// Photon g = id_base + i for i in [0, n) -> origins, dirs (n x 3), wl (n).  Returns 0, or 1 if some g has no step.
+int oracle_emit_cherenkov(uint64_t n_steps, const float* step_x, const float* step_w, const float* step_len,
+                          const float* step_beta, const uint64_t* first, float n_index, float lambda1, float lambda2,
+                          uint64_t n, uint64_t id_base, uint64_t seed, float* origins, float* dirs, float* wl) {
+    const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    for (uint64_t i = 0; i < n; ++i) {
+        const uint64_t g = id_base + i;
+        if (n_steps == 0 || g >= first[n_steps]) return 1;
+        // the step with first[s] <= g < first[s+1]: the LAST s with first[s] <= g (steps without photons are skipped)
+        uint64_t lo = 0, hi = n_steps;                           // invariant: first[lo] <= g < first[hi]
+        while (hi - lo > 1) { const uint64_t mid = lo + (hi - lo) / 2; if (first[mid] <= g) lo = mid; else hi = mid; }
+        const uint64_t s = lo;
+        const float* x = step_x + 3 * s;
+        const float* w = step_w + 3 * s;
+        auto block = [&](uint32_t a, float* u) {
+            const uint32_t ctr[4] = {(uint32_t)g, (uint32_t)(g >> 32), a, 2u};
+            uint32_t r[4];
+            philox4x32_10(ctr, key, r);
+            for (int k = 0; k < 4; ++k) u[k] = (float)(r[k] >> 8) * 0x1.0p-24f;
+        };
+        float u[4];
+        block(0u, u);
+        const float t = u[0] * step_len[s];
+        for (int a = 0; a < 3; ++a) origins[3 * i + a] = __builtin_fmaf(t, w[a], x[a]);
+        wl[i] = (lambda1 * lambda2) / __builtin_fmaf(-u[1], lambda2 - lambda1, lambda2);
+        float c = 1.0f / (n_index * step_beta[s]);
+        if (!(c < 1.0f)) c = 1.0f;
+        const float sn = std::sqrt(std::fmax(__builtin_fmaf(-c, c, 1.0f), 0.0f));
+        float cphi = 1.0f, sphi = 0.0f;
+        for (uint32_t a = 0; a < 64u; ++a) {
+            if (a > 0) block(a, u);
+            const float X = __builtin_fmaf(2.0f, u[2], -1.0f), Y = __builtin_fmaf(2.0f, u[3], -1.0f);
+            const float q = __builtin_fmaf(Y, Y, X * X);
+            if (q > 0.0f && q <= 1.0f) { cphi = (X * X - Y * Y) / q; sphi = ((2.0f * X) * Y) / q; break; }
+        }
+        const float sg = (w[2] >= 0.0f) ? 1.0f : -1.0f;
+        const float k = -1.0f / (sg + w[2]);
+        const float b = (w[0] * w[1]) * k;
+        const float e1[3] = {__builtin_fmaf(sg * w[0], w[0] * k, 1.0f), sg * b, -sg * w[0]};
+        const float e2[3] = {b, __builtin_fmaf(w[1], w[1] * k, sg), -w[1]};
+        const float A = sn * cphi, B = sn * sphi;
+        float m[3];
+        for (int a = 0; a < 3; ++a) m[a] = __builtin_fmaf(A, e1[a], __builtin_fmaf(B, e2[a], c * w[a]));
+        const float len2 = __builtin_fmaf(m[2], m[2], __builtin_fmaf(m[1], m[1], m[0] * m[0]));
+        const float inv = 1.0f / std::sqrt(len2);
+        for (int a = 0; a < 3; ++a) dirs[3 * i + a] = m[a] * inv;
+    }
+    return 0;
+}
+
 // ------------------------------------------------------------------- analytic toy RICH (fp64)
 // Config 0 of BASELINE.json with the mirror as an exact sphere: cap of the sphere (centre C, radius
 // R) whose points P satisfy |(P-V).ex| <= half, |(P-V).ey| <= half and (P-V).a < R (the hemisphere

@@ -26,8 +26,9 @@ def _scene(kind):
 class Workload:
     """name, scene, n (photons), seed, and photons(ids) -> (origins, dirs, wavelengths)."""
 
-    def __init__(self, name, scene, n, seed, source):
+    def __init__(self, name, scene, n, seed, source, track_source=None):
         self.name, self.scene, self.n, self.seed, self._source = name, scene, int(n), int(seed), source
+        self.track_source = track_source       # C3-C5: the TrackSource (its .steps() feeds on-device generation)
 
     def photons(self, ids):
         return self._source(np.asarray(ids, dtype=np.uint64))
@@ -45,11 +46,11 @@ def make_config(name, n=None, seed=0):
         return Workload(name, _scene("toy"), n, seed, lambda ids: cone_point_source(ids, seed))
     if name == "C3":
         src = TrackSource(n, seed)
-        return Workload(name, _scene("toy"), n, seed, src.photons)
+        return Workload(name, _scene("toy"), n, seed, src.photons, src)
     if name == "C4":
         src = TrackSource(n, seed)
-        return Workload(name, _scene("lhcb"), n, seed, src.photons)
+        return Workload(name, _scene("lhcb"), n, seed, src.photons, src)
     if name == "C5":
         src = TrackSource(n, seed, disc_radius=200.0, beta_lo=0.9999)
-        return Workload(name, _scene("lhcb"), n, seed, src.photons)
+        return Workload(name, _scene("lhcb"), n, seed, src.photons, src)
     raise KeyError(name)

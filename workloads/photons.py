@@ -89,6 +89,20 @@ class TrackSource:
         beta = self.beta_lo + (1.0 - self.beta_lo) * u[4]
         return o, w, beta
 
+    def steps(self):
+        """The track-step table behind the same photon ids, as the INPUT of on-device generation (SURVEY.md 8(f) row
+        f4): x (S,3) step start, w (S,3) unit direction, length (S,), beta (S,) float32 and
+        first (S+1,) uint64 = exclusive prefix sum of the per-step photon counts, truncated to n_total photons.
+        What Geant4 would hand over per step; the emission itself is the method's, not this module's."""
+        S = self.n_tracks * self.n_steps
+        t = np.repeat(np.arange(self.n_tracks, dtype=np.uint64), self.n_steps)
+        k = np.tile(np.arange(self.n_steps, dtype=np.float64), self.n_tracks)
+        o_t, w, beta = self.tracks(t)
+        x = o_t + (k * self.step)[:, None] * w
+        first = np.minimum(self.offsets[:S + 1], self.n_total).astype(np.uint64)
+        return dict(x=np.ascontiguousarray(x.astype(np.float32)), w=np.ascontiguousarray(w.astype(np.float32)),
+                    length=np.full(S, self.step, np.float32), beta=np.ascontiguousarray(beta.astype(np.float32)), first=first)
+
     def photons(self, ids):
         ids = np.asarray(ids, dtype=np.uint64)
         assert ids.size == 0 or int(ids.max()) < self.n_total
