@@ -213,6 +213,33 @@ opx_status opx_prefilter(const opx_scene* scene, uint64_t n, uint64_t photon_id_
                          float* d_out_origins, float* d_out_dirs, float* d_out_wavelengths, uint32_t* d_out_index,
                          uint64_t* d_n_kept, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Track steps for opx_emit_cherenkov: DEVICE pointers.  Step s starts at x[s], runs along the unit vector w[s] for
+ * length[s] mm with velocity beta[s]; first (n_steps + 1 entries, non-decreasing, first[0] = 0) is the exclusive
+ * prefix sum of the photons emitted per step: global photon g belongs to the step with first[s] <= g < first[s+1].
+ * The photon COUNT per step is the caller's (Geant4's, or a Frank-Tamm yield). */
+typedef struct {
+    const float* x;        /* n_steps x 3 */
+    const float* w;        /* n_steps x 3, unit */
+    const float* length;   /* n_steps, mm */
+    const float* beta;     /* n_steps */
+    const uint64_t* first; /* n_steps + 1 */
+    uint64_t n_steps;
+} opx_track_steps;
+
+/* Cherenkov photons generated on the device from charged-track steps (PAPER.md:71:
+ * cos(theta_c) = 1/(n beta); the paper writes Geant4's photons to a file and wants the loop
+ * memory-resident).  Photons photon_id_base .. photon_id_base + n - 1 are written to d_origins / d_dirs (n x 3) and
+ * d_wavelengths (n) - the arrays opx_propagate and opx_prefilter read - entry g - photon_id_base for photon g:
+ * position uniform along its step, polar angle theta_c about the track (along the track if n beta <= 1), azimuth
+ * uniform, wavelength with density 1/lambda^2 on [lambda1_nm, lambda2_nm]; operation by operation DESIGN.md 3.12.
+ * A photon depends on (seed, g, its step) only, so any split of the id range over calls or GPUs gives the same bits.
+ * n_total = first[n_steps] as the HOST knows it: photon_id_base + n > n_total, n_steps = 0 with n > 0, NULL pointers,
+ * lambda1 <= 0 or lambda2 <= lambda1, n_index not finite => OPX_ERR_INVALID_ARG.  n = 0 is valid.  Enqueues one
+ * kernel on cuda_stream; needs no scene. */
+opx_status opx_emit_cherenkov(const opx_track_steps* steps, uint64_t n_total, float n_index, float lambda1_nm,
+                              float lambda2_nm, uint64_t n, uint64_t photon_id_base, uint64_t seed, float* d_origins,
+                              float* d_dirs, float* d_wavelengths, void* cuda_stream);
+
 /* Same computation with the closest hit found by testing EVERY triangle on the GPU (no BVH
  * traversal).  A debugging aid that separates the arithmetic of DESIGN.md section 3 from the BVH;
  * O(n x triangles), never timed. */

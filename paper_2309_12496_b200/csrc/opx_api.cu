@@ -243,6 +243,26 @@ opx_status opx_prefilter(const opx_scene* scene, uint64_t n, uint64_t photon_id_
                             d_out_dirs, d_out_wavelengths, d_out_index, d_n_kept, d_workspace, (cudaStream_t)cuda_stream);
 }
 
+opx_status opx_emit_cherenkov(const opx_track_steps* steps, uint64_t n_total, float n_index, float lambda1_nm,
+                              float lambda2_nm, uint64_t n, uint64_t photon_id_base, uint64_t seed, float* d_origins,
+                              float* d_dirs, float* d_wavelengths, void* cuda_stream) {
+    if (!steps) return fail(OPX_ERR_INVALID_ARG, "steps is NULL");
+    if (!(lambda1_nm > 0.f) || !(lambda2_nm > lambda1_nm) || !std::isfinite(lambda2_nm) || !std::isfinite(n_index))
+        return fail(OPX_ERR_INVALID_ARG, "need 0 < lambda1 < lambda2 and a finite refractive index");
+    if (n == 0) return OPX_OK;
+    if (steps->n_steps == 0 || !steps->x || !steps->w || !steps->length || !steps->beta || !steps->first)
+        return fail(OPX_ERR_INVALID_ARG, "empty or NULL step table");
+    if (photon_id_base > n_total || n > n_total - photon_id_base) return fail(OPX_ERR_INVALID_ARG, "photon ids beyond first[n_steps]");
+    if (!d_origins || !d_dirs || !d_wavelengths) return fail(OPX_ERR_INVALID_ARG, "NULL output array");
+    if (misaligned(d_origins, 4) || misaligned(d_dirs, 4) || misaligned(d_wavelengths, 4) || misaligned(steps->first, 8) ||
+        misaligned(steps->x, 4) || misaligned(steps->w, 4) || misaligned(steps->length, 4) || misaligned(steps->beta, 4))
+        return fail(OPX_ERR_INVALID_ARG, "misaligned pointer");
+    if (opx_status st = device_ok()) return st;
+    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_emit_cherenkov")) return st;
+    return launch_emit(*steps, n_index, lambda1_nm, lambda2_nm, n, photon_id_base, seed, d_origins, d_dirs, d_wavelengths,
+                       (cudaStream_t)cuda_stream);
+}
+
 opx_status opx_propagate_brute(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
                                const float* d_dirs, const float* d_wavelengths, uint64_t seed, const opx_hits* out,
                                uint32_t* d_hitmap, uint64_t* d_counters, void* cuda_stream) {

@@ -103,6 +103,9 @@ opx_status launch_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const 
 opx_status launch_packet_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,
                                const float* wl, uint64_t seed, const opx_hits& out, uint64_t* stats, cudaStream_t stream);
 size_t wide_node_capacity(size_t n_triangles);
+// Cherenkov emission (opx_emit.cu)
+opx_status launch_emit(const opx_track_steps& st, float n_index, float lambda1, float lambda2, uint64_t n, uint64_t id_base,
+                       uint64_t seed, float* o, float* d, float* wl, cudaStream_t stream);
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 

@@ -22,7 +22,7 @@ FLAG_NO_EFFICIENCY = 1                   # opx_flags
 TABLE_LINEAR, TABLE_HISTOGRAM = 0, 1     # opx_table_interp
 
 EXPORTS = ("opx_scene_create", "opx_scene_workspace_bytes", "opx_bvh_build", "opx_propagate",
-           "opx_propagate_flags", "opx_prefilter_workspace_bytes", "opx_prefilter", "opx_propagate_brute", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
+           "opx_propagate_flags", "opx_prefilter_workspace_bytes", "opx_prefilter", "opx_emit_cherenkov", "opx_propagate_brute", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
            "opx_profile_begin", "opx_profile_end", "opx_propagate_stats", "opx_propagate_packet_stats",
            "opx_scene_wide_info", "opx_measure_fp32_peak",
            "opx_scene_info", "opx_scene_get_layout", "opx_launch_count", "opx_scene_destroy",
@@ -61,6 +61,11 @@ class Hits(C.Structure):
                 ("state", C.c_void_p), ("bounces", C.c_void_p)]
 
 
+class TrackSteps(C.Structure):
+    _fields_ = [("x", C.c_void_p), ("w", C.c_void_p), ("length", C.c_void_p), ("beta", C.c_void_p), ("first", C.c_void_p),
+                ("n_steps", C.c_uint64)]
+
+
 class SceneLayout(C.Structure):
     _fields_ = [(k, C.c_uint64) for k in ("nodes", "triangles", "normals", "surfaces", "mat_kinds", "tables",
                                           "frames", "sorted_keys", "parents", "wide_nodes", "wide_node_capacity",
@@ -91,6 +96,7 @@ def load_library(path=LIB_PATH):
     lib.opx_propagate_flags.argtypes = [vp, u64, vp, u64, vp, vp, vp, u64, u32, vp, vp, vp, vp]
     lib.opx_prefilter_workspace_bytes.argtypes = [u64, vp]
     lib.opx_prefilter.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, u32, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.opx_emit_cherenkov.argtypes = [vp, u64, C.c_float, C.c_float, C.c_float, u64, u64, u64, vp, vp, vp, vp]
     lib.opx_propagate_host_workspace_bytes.argtypes = [vp, u64, vp]
     lib.opx_propagate_host.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp, vp, vp, C.c_size_t, u64, vp]
     lib.opx_profile_begin.argtypes = [vp, u32]
@@ -119,6 +125,33 @@ def measure_fp32_peak(device="cuda"):
     _check(load_library().opx_measure_fp32_peak(C.byref(out), scratch.data_ptr(),
                                                 C.c_void_p(torch.cuda.current_stream(device).cuda_stream)))
     return out.value
+
+
+def upload_track_steps(steps, device="cuda"):
+    """Host step table (dict x, w, length, beta float32; first uint64 -- e.g. workloads.TrackSource.steps()) -> the
+    same dict as CUDA tensors plus n_total = first[-1] as a Python int (first as an int64 view of the uint64 bits)."""
+    import torch
+    out = {k: torch.from_numpy(np.ascontiguousarray(steps[k], dtype=np.float32)).to(device) for k in ("x", "w", "length", "beta")}
+    first = np.ascontiguousarray(steps["first"], dtype=np.uint64)
+    out["first"] = torch.from_numpy(first.view(np.int64)).to(device)
+    out["n_total"] = int(first[-1]) if len(first) else 0
+    return out
+
+
+def emit_cherenkov(dev_steps, n, photon_id_base=0, seed=0, n_index=1.0014, lambda1=200.0, lambda2=600.0, out=None, stream=None):
+    """opx_emit_cherenkov on an uploaded step table -> (origins (n,3), dirs (n,3), wavelengths (n,)) CUDA tensors."""
+    import torch
+    dev = dev_steps["first"].device
+    if out is None:
+        out = (torch.empty((n, 3), dtype=torch.float32, device=dev), torch.empty((n, 3), dtype=torch.float32, device=dev),
+               torch.empty(n, dtype=torch.float32, device=dev))
+    st = TrackSteps(dev_steps["x"].data_ptr(), dev_steps["w"].data_ptr(), dev_steps["length"].data_ptr(),
+                    dev_steps["beta"].data_ptr(), dev_steps["first"].data_ptr(), int(dev_steps["length"].shape[0]))
+    s = stream if stream is not None else torch.cuda.current_stream(dev)
+    _check(load_library().opx_emit_cherenkov(C.byref(st), int(dev_steps["n_total"]), n_index, lambda1, lambda2, int(n),
+                                             int(photon_id_base), int(seed), out[0].data_ptr(), out[1].data_ptr(),
+                                             out[2].data_ptr(), C.c_void_p(s.cuda_stream)))
+    return out
 
 
 def launch_count():
