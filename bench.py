@@ -370,6 +370,39 @@ def main():
                                         "unit": "GB/s", "frac": pf_bytes / times["prefilter"] / 1e9 / peaks["hbm_gbs"],
                                         "bytes_per_photon": pf_bytes / n}}
 
+    # ---- on-device Cherenkov generation from track steps, alone and chained into opx_propagate
+    emit = None
+    if world == 1:
+        src = w.track_source if w.track_source is not None else workloads.make_config("C3", n=n).track_source
+        dsteps = pkg.upload_track_steps(src.steps(), dev)
+        gen = (torch.empty_like(d_o), torch.empty_like(d_d), torch.empty_like(d_l))
+        hm3, ct3 = scene.alloc_accumulators(dev)
+
+        def emit_step(trace):
+            pkg.emit_cherenkov(dsteps, n, photon_id_base=0, seed=args.seed, out=gen, stream=stream)
+            if trace:
+                hm3.zero_(); ct3.zero_()
+                scene.propagate(*gen, seed=args.seed, records=records, hitmap=hm3, counters=ct3, stream=stream)
+        etimes = {}
+        for name, trace in (("emit", False), ("chain", True)):
+            for _ in range(args.warmup):
+                emit_step(trace)
+            torch.cuda.synchronize()
+            ev0.record(stream)
+            for _ in range(args.steps):
+                emit_step(trace)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            etimes[name] = ev0.elapsed_time(ev1) / args.steps * 1e-3
+        emit = {"what": f"opx_emit_cherenkov: {n} photons from {int(dsteps['length'].shape[0])} track steps"
+                        + ("" if w.track_source is not None else " (step table of C3: C2's photons are a point source, not tracks)"),
+                "value": n / etimes["emit"], "unit": UNIT, "ms_per_step": 1e3 * etimes["emit"],
+                "roofline": {"bound": "hbm", "achieved": BYTES_IN * n / etimes["emit"] / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                             "frac": BYTES_IN * n / etimes["emit"] / 1e9 / peaks["hbm_gbs"], "bytes_per_photon": BYTES_IN,
+                             "note": "issue-bound on the contract's arithmetic (Philox, IEEE divides), not HBM: profiles/r01_v11_emit.md"},
+                "emit_then_propagate": {"value": n / etimes["chain"], "unit": UNIT, "ms_per_step": 1e3 * etimes["chain"],
+                                        "detected": int(ct3[0].item())}}
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         n_sample = min(n, args.cpu_sample)
@@ -391,7 +424,7 @@ def main():
                    "photons_per_gpu": n, "triangles": w.scene.n_triangles, "pixels": scene.n_pixels, "seed": args.seed,
                    "id_partition": "contiguous global photon-id range per rank; scene + BVH replicated"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
-        "paper_pipeline": paper, "bvh_build_ms": min(t_build), "bvh_build_launches": int(build_launches),
+        "paper_pipeline": paper, "emit": emit, "bvh_build_ms": min(t_build), "bvh_build_launches": int(build_launches),
         "states": dict(zip(pkg.STATE_NAMES, (int(x) for x in cnt[:7]))),
         "context_paper": "paper: 1.2e6 photons/s per Tesla T4 and 2e5 per Xeon thread, end to end (PAPER.md:9); other hardware, not the target",
     }

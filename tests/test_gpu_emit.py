@@ -39,9 +39,11 @@ def test_emit_matches_oracle_bit_for_bit():
     """Random steps in both hemispheres and at the poles of the frame, beta above / at / below threshold, steps
     without photons, a 64-bit seed; ~1e5 photons, ragged against the 256-thread blocks."""
     rng = np.random.default_rng(41)
-    S = 300
-    counts = rng.integers(0, 700, S)
-    counts[[3, 4, 17, 299]] = 0
+    S = 1500
+    counts = rng.integers(0, 140, S)
+    counts[[3, 4, 17, S - 1]] = 0
+    counts[200:900] = 0                                # a block of photons that spans 700 steps without photons
+    counts[950:1300:2] = 0
     beta = rng.uniform(0.9980, 1.0, S)
     beta[:8] = [1.0, 0.99860196, 0.9986, 0.5, 0.9, 1.0, 1.0, 1.0]
     st = _random_steps(rng, S, counts, beta)
