@@ -20,10 +20,17 @@
 namespace opx {
 namespace {
 
-constexpr int kPktThreads = 512;
+#ifndef OPX_PKT_THREADS
+#define OPX_PKT_THREADS 512
+#endif
+#ifndef OPX_PKT_CTAS
+#define OPX_PKT_CTAS 2
+#endif
+constexpr int kPktThreads = OPX_PKT_THREADS;
+constexpr int kPktCtas = OPX_PKT_CTAS;               // resident CTAs per SM the kernel is compiled for
 constexpr int kPktWarps = kPktThreads / 32;          // 16
-constexpr int kTile = 2048;                          // photons per CTA tile
-constexpr int kItems = kTile / kPktThreads;          // 4
+constexpr int kItems = 4;                            // photons per thread in the staging / sort phases
+constexpr int kTile = kItems * kPktThreads;          // 2048 photons per CTA tile
 constexpr int kPktStack = 96;                        // depth bound of the Karras tree (see opx_lane.cuh)
 constexpr int kStackSmem = kPktStack - 32;
 
@@ -191,7 +198,7 @@ __device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW
 }
 
 template <bool kStats>
-__global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const SceneDev sc, uint64_t n, uint64_t id_base,
+__global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(const SceneDev sc, uint64_t n, uint64_t id_base,
                                                                      const float* __restrict__ origins,
                                                                      const float* __restrict__ dirs,
                                                                      const float* __restrict__ wl, uint64_t seed, opx_hits out,
@@ -260,7 +267,7 @@ __global__ void __launch_bounds__(kPktThreads, 2) k_propagate_packet(const Scene
         for (int r = 0; r < kItems; ++r) { cur[r] = cu / (float)m; cvr[r] = cv / (float)m; }
         if (__syncthreads_or(any)) {      // rare: the tile holds photons of more than one track
             uint32_t* chunk = &sm.cnt[0][0];                       // kItems x kPktWarps jump counts, in tile order
-            float* rs = reinterpret_cast<float*>(chunk + 64);      // 4 runs x (sum u, sum v, count)
+            float* rs = reinterpret_cast<float*>(chunk + kItems * kPktWarps);      // 4 runs x (sum u, sum v, count)
             unsigned bal[kItems];
 #pragma unroll
             for (int r = 0; r < kItems; ++r) {
