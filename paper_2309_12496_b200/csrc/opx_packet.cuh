@@ -202,6 +202,7 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
                                                                      const float* __restrict__ origins,
                                                                      const float* __restrict__ dirs,
                                                                      const float* __restrict__ wl, uint64_t seed, opx_hits out,
+                                                                     uint32_t* hitmap, unsigned long long* counters,
                                                                      unsigned long long* stats) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PacketSmem& sm = *reinterpret_cast<PacketSmem*>(smem_raw);
@@ -394,6 +395,37 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
             atomicAdd(&stats[0], (unsigned long long)bstats.beam_segments); atomicAdd(&stats[1], (unsigned long long)bstats.fallback_segments);
             atomicAdd(&stats[2], (unsigned long long)bstats.visits); atomicAdd(&stats[3], (unsigned long long)bstats.tris);
             atomicAdd(&stats[4], (unsigned long long)bstats.overflows); atomicAdd(&stats[5], (unsigned long long)bstats.culls);
+        }
+    }
+
+    // 4a. A11 + A12 for this tile, straight from shared memory (what k_bin does for the other kernels): detected photons of
+    //     a warp that share a pixel are merged into one atomic, states are counted with ballots.  Integer adds only.
+    if (hitmap || counters) {
+        uint32_t* s_cnt = sm.scan_tot;                       // 8 of its kPktWarps words; free since the sort
+        static_assert(kPktWarps >= 8, "state counters alias scan_tot");
+        if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0;
+        __syncthreads();
+        unsigned seg = 0, acc = 0;                           // acc: seven 4-bit per-state counts of this thread (<= kItems each)
+        static_assert(kItems <= 7, "4-bit state counts per thread, 8-bit per warp");
+        for (int k = threadIdx.x; k < kTile; k += kPktThreads) {           // uniform trip count: warp collectives inside
+            const bool ok = k < m;
+            const int st = ok ? (int)sm.state[k] : 7;
+            if (ok) { seg += (unsigned)sm.bounces[k] + (st != OPX_BOUNCE_LIMIT ? 1u : 0u); acc += 1u << (4 * st); }
+            const int key = st == OPX_DETECTED ? __float_as_int(sm.wl[k]) : -1 - lane;     // unique key for the other lanes
+            const unsigned peers = __match_any_sync(0xffffffffu, key);
+            if (hitmap && st == OPX_DETECTED && lane == __ffs(peers) - 1) atomicAdd(&hitmap[key], (unsigned)__popc(peers));
+        }
+        if (counters) {
+            // widen the 4-bit fields to 8 bits (a warp sums to <= 32 * kItems = 128 per state) and add across the warp
+            const unsigned lo4 = (acc & 0xfu) | ((acc & 0xf0u) << 4) | ((acc & 0xf00u) << 8) | ((acc & 0xf000u) << 12);       // states 0..3
+            const unsigned hi4 = ((acc >> 16) & 0xfu) | ((acc >> 12) & 0xf00u) | ((acc >> 8) & 0xf0000u);                    // states 4..6
+            const unsigned a = __reduce_add_sync(0xffffffffu, lo4), b = __reduce_add_sync(0xffffffffu, hi4);
+            seg = __reduce_add_sync(0xffffffffu, seg);
+            if (lane < 4) { const unsigned c = (a >> (8 * lane)) & 0xffu; if (c) atomicAdd(&s_cnt[lane], c); }
+            else if (lane < 7) { const unsigned c = (b >> (8 * (lane - 4))) & 0xffu; if (c) atomicAdd(&s_cnt[lane], c); }
+            else if (lane == 7 && seg) atomicAdd(&s_cnt[7], seg);
+            __syncthreads();
+            if (threadIdx.x < 8 && s_cnt[threadIdx.x]) atomicAdd(&counters[threadIdx.x], (unsigned long long)s_cnt[threadIdx.x]);
         }
     }
 

@@ -17,6 +17,7 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
     cudaEvent_t* ev = nullptr;
     if (s.prof_used < s.prof_max) { ev = &s.prof_events[3 * (size_t)s.prof_used]; ++s.prof_used; }
     if (ev) cudaEventRecord(ev[0], stream);
+    bool binned = false;         // A11/A12 done inside the propagation kernel
     if (brute || s.dev.n_tri < 2) {
         // debug mode, or a scene with fewer than two triangles (no hierarchy): test the triangle list directly
         const uint64_t blocks = (n + 127) / 128;
@@ -33,12 +34,13 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
         }
         const uint64_t tiles = (n + kTile - 1) / kTile;
         if (tiles > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
-        if (packet_stats) k_propagate_packet<true><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(dev, n, id_base, o, d, wl, seed, out, (unsigned long long*)packet_stats);
-        else k_propagate_packet<false><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr);
+        if (packet_stats) k_propagate_packet<true><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr, nullptr, (unsigned long long*)packet_stats);
+        else k_propagate_packet<false><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
+        binned = !packet_stats;
     }
     count_launch(1);
     if (ev) cudaEventRecord(ev[1], stream);
-    if (hitmap || counters) {
+    if (!binned && (hitmap || counters)) {
         const uint64_t bb = (n + 255) / 256;
         const unsigned grid = (unsigned)(bb < 148ull * 8 ? bb : 148ull * 8);
         k_bin<<<grid, 256, 0, stream>>>(out.state, out.bounces, out.pixel, n, (const unsigned long long*)d_n, hitmap, (unsigned long long*)counters);
