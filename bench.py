@@ -276,7 +276,7 @@ def main():
     e2e = None
     if rank == 0 or dist is not None:
         host_out = pkg.alloc_host_records(n, scene.n_pixels)
-        chunk = min(n, 1 << 21)
+        chunk = min(n, 1 << 20)
         scene.propagate_host(*pin, seed=args.seed, photon_id_base=id_base, chunk=chunk, out=host_out, stream=stream)
         torch.cuda.synchronize()
         t0 = time.perf_counter()

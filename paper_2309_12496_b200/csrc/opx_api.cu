@@ -271,7 +271,12 @@ opx_status opx_propagate_brute(const opx_scene* scene, uint64_t n, uint64_t phot
 }
 
 // ------------------------------------------------------------------------- host-buffer streaming
-// Device staging per slot (two slots): inputs 28 B/photon, records 34 B/photon.
+// Device staging per slot (kSlots slots, one stream each): inputs 28 B/photon, records 34 B/photon.  Three slots let the
+// upload of chunk k+2 run while chunk k+1 computes and chunk k downloads, so neither copy engine waits for a buffer.
+#ifndef OPX_HOST_SLOTS
+#define OPX_HOST_SLOTS 3
+#endif
+static constexpr int kSlots = OPX_HOST_SLOTS;
 static size_t slot_bytes(uint64_t chunk) {
     size_t b = 0;
     b += align_up(chunk * 12, 256) * 4;   // origins, dirs, pos, dir
@@ -282,7 +287,7 @@ static size_t slot_bytes(uint64_t chunk) {
 
 opx_status opx_propagate_host_workspace_bytes(const opx_scene* scene, uint64_t chunk, size_t* bytes) {
     if (!scene || !bytes || chunk == 0) return fail(OPX_ERR_INVALID_ARG, "NULL argument or chunk = 0");
-    *bytes = 2 * slot_bytes(chunk) + align_up(scene->n_pixels * 4 + 4, 256) + 256;
+    *bytes = kSlots * slot_bytes(chunk) + align_up(scene->n_pixels * 4 + 4, 256) + 256;
     return OPX_OK;
 }
 
@@ -305,10 +310,10 @@ opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photo
 
     cudaStream_t main = (cudaStream_t)cuda_stream;
     struct Slot { float *o, *d, *wl, *pos, *dir; int32_t *pixel, *surface; uint8_t *state, *bounces; cudaStream_t st; cudaEvent_t done; };
-    Slot slot[2];
+    Slot slot[kSlots];
     char* p = (char*)d_workspace;
     auto take = [&](size_t bytes) { char* r = p; p += align_up(bytes, 256); return r; };
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < kSlots; ++k) {
         Slot& s = slot[k];
         s.o = (float*)take(chunk * 12); s.d = (float*)take(chunk * 12); s.pos = (float*)take(chunk * 12); s.dir = (float*)take(chunk * 12);
         s.wl = (float*)take(chunk * 4); s.pixel = (int32_t*)take(chunk * 4); s.surface = (int32_t*)take(chunk * 4);
@@ -320,7 +325,7 @@ opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photo
     opx_status st = OPX_OK;
     cudaEvent_t start;
     if ((st = check_cuda(cudaEventCreateWithFlags(&start, cudaEventDisableTiming), "cudaEventCreate"))) return st;
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < kSlots; ++k) {
         cudaStreamCreateWithFlags(&slot[k].st, cudaStreamNonBlocking);
         cudaEventCreateWithFlags(&slot[k].done, cudaEventDisableTiming);
     }
@@ -328,12 +333,21 @@ opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photo
     cudaMemsetAsync(d_hitmap, 0, scene->n_pixels * 4 + 4, main);
     cudaMemsetAsync(d_counters, 0, 64, main);
     cudaEventRecord(start, main);
-    for (int k = 0; k < 2; ++k) cudaStreamWaitEvent(slot[k].st, start, 0);
+    for (int k = 0; k < kSlots; ++k) cudaStreamWaitEvent(slot[k].st, start, 0);
 
     uint64_t done = 0;
     int k = 0;
+    // Chunk schedule: the first upload and the last download cannot overlap anything, so the stream is ramped up
+    // (chunk/8, chunk/8, chunk/4, chunk/2, then full chunks) and ramped down (halving the remainder, floor chunk/8).
+    const uint64_t small = chunk >= 8 ? chunk / 8 : 1;
+    uint32_t issued = 0;
     while (done < n && st == OPX_OK) {
-        const uint64_t m = (n - done < chunk) ? (n - done) : chunk;
+        uint64_t m = chunk;
+        if (issued < 2) m = small; else if (issued == 2) m = chunk / 4 ? chunk / 4 : 1; else if (issued == 3) m = chunk / 2 ? chunk / 2 : 1;
+        const uint64_t left = n - done;
+        if (left < 2 * m) { const uint64_t half = (left + 1) / 2; m = half > small ? half : (left < small ? left : small); }
+        if (m > left) m = left;
+        ++issued;
         Slot& s = slot[k];
         cudaMemcpyAsync(s.o, h_origins + 3 * done, m * 12, cudaMemcpyHostToDevice, s.st);
         cudaMemcpyAsync(s.d, h_dirs + 3 * done, m * 12, cudaMemcpyHostToDevice, s.st);
@@ -348,16 +362,16 @@ opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photo
         cudaMemcpyAsync(h_out->state + done, s.state, m, cudaMemcpyDeviceToHost, s.st);
         cudaMemcpyAsync(h_out->bounces + done, s.bounces, m, cudaMemcpyDeviceToHost, s.st);
         done += m;
-        k ^= 1;
+        k = (k + 1) % kSlots;
     }
     // join
-    for (int j = 0; j < 2; ++j) { cudaEventRecord(slot[j].done, slot[j].st); cudaStreamWaitEvent(main, slot[j].done, 0); }
+    for (int j = 0; j < kSlots; ++j) { cudaEventRecord(slot[j].done, slot[j].st); cudaStreamWaitEvent(main, slot[j].done, 0); }
     std::vector<uint32_t> hm(scene->n_pixels);
     uint64_t cnt[8] = {0};
     if (scene->n_pixels) cudaMemcpyAsync(hm.data(), d_hitmap, scene->n_pixels * 4, cudaMemcpyDeviceToHost, main);
     cudaMemcpyAsync(cnt, d_counters, 64, cudaMemcpyDeviceToHost, main);
     cudaError_t e = cudaStreamSynchronize(main);
-    for (int j = 0; j < 2; ++j) { cudaStreamDestroy(slot[j].st); cudaEventDestroy(slot[j].done); }
+    for (int j = 0; j < kSlots; ++j) { cudaStreamDestroy(slot[j].st); cudaEventDestroy(slot[j].done); }
     cudaEventDestroy(start);
     if (st != OPX_OK) return st;
     if (e != cudaSuccess) return check_cuda(e, "opx_propagate_host");

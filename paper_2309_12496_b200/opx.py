@@ -363,7 +363,7 @@ class Scene:
         _check(load_library().opx_scene_wide_info(self._h, C.byref(a), C.byref(b)))
         return a.value, b.value
 
-    def propagate_host(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, chunk=1 << 21, out=None,
+    def propagate_host(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, chunk=1 << 20, out=None,
                        stream=None, device="cuda"):
         """opx_propagate_host: host (pinned torch or numpy) buffers in, host buffers out."""
         import torch
