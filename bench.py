@@ -125,29 +125,45 @@ def run_sweep(args, scene, photons, records, hitmap, counters, n, stream, w, pkg
     import torch
     d_o, d_d, d_l = photons
     rows = []
+    side = [torch.cuda.Stream(device=d_o.device) for _ in range(max(0, args.streams - 1))]
+    fork, joins = torch.cuda.Event(), [torch.cuda.Event() for _ in side]
     for chunk in [int(c) for c in args.chunks.split(",") if int(c) <= n]:
-        def one_pass(base):
-            for a in range(0, n - chunk + 1, chunk):
-                rec = {k: v[a:a + chunk] for k, v in records.items()}
-                scene.propagate(d_o[a:a + chunk], d_d[a:a + chunk], d_l[a:a + chunk], seed=args.seed, photon_id_base=base + a,
-                                records=rec, hitmap=hitmap, counters=counters, stream=stream)
-        per_pass = (n // chunk) * chunk
-        passes = max(1, min(args.total // per_pass, 50))
-        hitmap.zero_(); counters.zero_()
-        one_pass(0)                                                    # warm-up
-        torch.cuda.synchronize()
-        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        l0 = pkg.launch_count()
-        ev0.record(stream)
-        for p in range(passes):
-            one_pass((p + 1) * per_pass)
-        ev1.record(stream)
-        torch.cuda.synchronize()
-        ms = ev0.elapsed_time(ev1)
-        done = passes * per_pass
-        rows.append({"chunk": chunk, "photons": done, "calls": passes * (n // chunk), "ms": ms,
-                     "photons_per_s": done / (ms * 1e-3), "hbm_gbs_algorithmic": done * (BYTES_IN + BYTES_OUT + BYTES_BIN) / (ms * 1e-3) / 1e9,
-                     "gpu_launches": pkg.launch_count() - l0})
+        for n_streams in sorted({1, args.streams}):
+            lanes = [stream] + side[:n_streams - 1]
+
+            def one_pass(base):
+                for k, a in enumerate(range(0, n - chunk + 1, chunk)):
+                    rec = {key: v[a:a + chunk] for key, v in records.items()}
+                    scene.propagate(d_o[a:a + chunk], d_d[a:a + chunk], d_l[a:a + chunk], seed=args.seed, photon_id_base=base + a,
+                                    records=rec, hitmap=hitmap, counters=counters, stream=lanes[k % n_streams])
+
+            def timed(passes_, per_pass_):
+                # calls are independent (hit-map and counters are integer atomics), so they may be spread over streams:
+                # the side streams fork from and join back into the timed stream
+                fork.record(stream)
+                for st in lanes[1:]:
+                    st.wait_event(fork)
+                for p in range(passes_):
+                    one_pass((p + 1) * per_pass_)
+                for st, ev in zip(lanes[1:], joins):
+                    ev.record(st)
+                    stream.wait_event(ev)
+            per_pass = (n // chunk) * chunk
+            passes = max(1, min(args.total // per_pass, 50))
+            hitmap.zero_(); counters.zero_()
+            timed(1, 0)                                                    # warm-up
+            torch.cuda.synchronize()
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            l0 = pkg.launch_count()
+            ev0.record(stream)
+            timed(passes, per_pass)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            ms = ev0.elapsed_time(ev1)
+            done = passes * per_pass
+            rows.append({"chunk": chunk, "streams": n_streams, "photons": done, "calls": passes * (n // chunk), "ms": ms,
+                         "photons_per_s": done / (ms * 1e-3), "hbm_gbs_algorithmic": done * (BYTES_IN + BYTES_OUT) / (ms * 1e-3) / 1e9,
+                         "gpu_launches": pkg.launch_count() - l0})
     best = max(rows, key=lambda r: r["photons_per_s"])
     print(json.dumps({"metric": METRIC, "value": best["photons_per_s"], "unit": UNIT, "n_gpus": 1, "higher_is_better": True,
                       "dtype": "f32", "data": "synthetic", "scaling": "weak", "vs_baseline": None,
@@ -177,6 +193,7 @@ def main():
                          "and report photons/s and HBM GB/s per chunk size instead of the default line")
     ap.add_argument("--total", type=int, default=1_000_000_000, help="photons streamed per chunk size in --sweep")
     ap.add_argument("--chunks", type=str, default="100000,1000000,10000000,100000000")
+    ap.add_argument("--streams", type=int, default=4, help="--sweep: also time every chunk size with the calls spread over this many streams")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "opx" else args.warmup
     if args.impl == "reference":

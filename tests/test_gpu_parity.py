@@ -236,6 +236,28 @@ def test_c4_scene_bvh_and_sampled_parity(lhcb):
     assert a["counters"][:7].sum() == len(ids2) and a["hitmap"].sum() == a["counters"][0]
 
 
+def test_c5_sampled_parity(lhcb):
+    """Config 4 (the stress config): every 500 000th photon id of the 1e9-photon workload of mixed tracks
+    (beta in [0.9999, 1], origins in a 200 mm disc) on the C4 scene against the oracle, through a chunked call
+    sequence with advancing id bases as the config streams it."""
+    sc, gs = lhcb
+    w = wl.make_config("C5")
+    ids = np.arange(3, w.n, 500_000, dtype=np.uint64)
+    o, d, lam = w.photons(ids)
+    ref = oracle.trace_mesh(sc, o, d, lam, seed=9)
+    do, dd, dl = _dev(o, d, lam)
+    hm, ct = gs.alloc_accumulators()
+    parts = []
+    for a, b in ((0, 700), (700, 701), (701, len(ids))):
+        parts.append(_host(gs.propagate(do[a:b].contiguous(), dd[a:b].contiguous(), dl[a:b].contiguous(), seed=9,
+                                        photon_id_base=a, hitmap=hm, counters=ct)))
+    got = {k: np.concatenate([p[k] for p in parts]) for k in ("state", "surface", "pixel", "bounces", "pos", "dir")}
+    got["hitmap"], got["counters"] = parts[-1]["hitmap"], parts[-1]["counters"]
+    nbad, dmax = assert_parity(got, ref, len(ids))
+    assert nbad == 0 and dmax == 0.0
+    assert len(np.unique(ref["state"])) >= 5 and ref["bounces"].max() == 2
+
+
 def test_rebuild_is_deterministic(toy):
     sc, _ = toy
     a = pkg.Scene(sc).build()
