@@ -37,7 +37,9 @@ __global__ void __launch_bounds__(kFThreads) k_prefilter_mark(const SceneDev sc,
         if (i < n) {
             const float lambda = __ldcs(wl + i);
             float p = 1.f;
-            for (uint32_t k = 0; k < fa.n; ++k) {
+#pragma unroll
+            for (uint32_t k = 0; k < (uint32_t)kMaxFactors; ++k) {       // unrolled: the factor list is read with constant indices
+                if (k >= fa.n) break;
                 const float e = table_value(sc, fa.m[k], fa.mk[k], lambda);
                 p = k == 0 ? e : __fmul_rn(p, e);
             }
