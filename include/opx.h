@@ -240,6 +240,23 @@ opx_status opx_emit_cherenkov(const opx_track_steps* steps, uint64_t n_total, fl
                               float lambda2_nm, uint64_t n, uint64_t photon_id_base, uint64_t seed, float* d_origins,
                               float* d_dirs, float* d_wavelengths, void* cuda_stream);
 
+/* opx_emit_cherenkov followed by opx_prefilter in one call, without ever writing the photons the filter discards
+ * (6 of 7 with the paper's efficiencies): the paper's whole front end - photons from track steps, the three
+ * efficiencies applied before propagation - memory-resident.  By definition the
+ * result is that of the two calls (DESIGN.md 3.12 then 3.9, nothing new is computed): the survivors among photons
+ * photon_id_base .. photon_id_base + n - 1, in id order, in d_out_origins / d_out_dirs / d_out_wavelengths, their
+ * offsets g - photon_id_base in d_out_index (may be NULL), their number in *d_n_kept (DEVICE uint64, overwritten).
+ * The out arrays must hold n entries in the worst case (factors with efficiency 1); size them by an upper bound on
+ * the kept fraction at your own risk: nothing is written beyond *d_n_kept entries, but that number is not checked
+ * against a capacity.  n <= 2^32 - 1.  Arguments and errors as in opx_emit_cherenkov and opx_prefilter;
+ * d_workspace: opx_prefilter_workspace_bytes(n) device bytes, 256-byte aligned.  Three launches, no host round trip;
+ * trace the survivors with opx_propagate_flags(..., n, d_n_kept, ..., OPX_FLAG_NO_EFFICIENCY, ...). */
+opx_status opx_emit_cherenkov_filtered(const opx_scene* scene, const opx_track_steps* steps, uint64_t n_total, float n_index,
+                                       float lambda1_nm, float lambda2_nm, uint64_t n, uint64_t photon_id_base, uint64_t seed,
+                                       const uint32_t* factors, uint32_t n_factors, float* d_out_origins, float* d_out_dirs,
+                                       float* d_out_wavelengths, uint32_t* d_out_index, uint64_t* d_n_kept, void* d_workspace,
+                                       size_t workspace_bytes, void* cuda_stream);
+
 /* Same computation with the closest hit found by testing EVERY triangle on the GPU (no BVH
  * traversal).  A debugging aid that separates the arithmetic of DESIGN.md section 3 from the BVH;
  * O(n x triangles), never timed. */

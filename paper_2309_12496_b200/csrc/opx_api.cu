@@ -263,6 +263,37 @@ opx_status opx_emit_cherenkov(const opx_track_steps* steps, uint64_t n_total, fl
                        (cudaStream_t)cuda_stream);
 }
 
+opx_status opx_emit_cherenkov_filtered(const opx_scene* scene, const opx_track_steps* steps, uint64_t n_total, float n_index,
+                                       float lambda1_nm, float lambda2_nm, uint64_t n, uint64_t photon_id_base, uint64_t seed,
+                                       const uint32_t* factors, uint32_t n_factors, float* d_out_origins, float* d_out_dirs,
+                                       float* d_out_wavelengths, uint32_t* d_out_index, uint64_t* d_n_kept, void* d_workspace,
+                                       size_t workspace_bytes, void* cuda_stream) {
+    if (!scene || !steps) return fail(OPX_ERR_INVALID_ARG, "scene/steps is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_emit_cherenkov_filtered before opx_bvh_build");
+    if (!d_n_kept || misaligned(d_n_kept, 8)) return fail(OPX_ERR_INVALID_ARG, "d_n_kept is NULL or misaligned");
+    if (!(lambda1_nm > 0.f) || !(lambda2_nm > lambda1_nm) || !std::isfinite(lambda2_nm) || !std::isfinite(n_index))
+        return fail(OPX_ERR_INVALID_ARG, "need 0 < lambda1 < lambda2 and a finite refractive index");
+    if (n > 0xffffffffull) return fail(OPX_ERR_INVALID_ARG, "n must be <= 2^32 - 1");
+    if (n_factors > 8 || (n_factors && !factors)) return fail(OPX_ERR_INVALID_ARG, "n_factors must be <= 8 and factors non-NULL");
+    for (uint32_t k = 0; k < n_factors; ++k) {
+        if (factors[k] >= scene->mat_kinds.size()) return fail(OPX_ERR_INVALID_ARG, "factor material index out of range");
+        if ((scene->mat_kinds[factors[k]] & 0xffu) == OPX_MAT_ABSORBER) return fail(OPX_ERR_INVALID_ARG, "an absorber has no efficiency table");
+    }
+    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_emit_cherenkov_filtered")) return st;
+    if (n == 0) return check_cuda(cudaMemsetAsync(d_n_kept, 0, 8, (cudaStream_t)cuda_stream), "cudaMemsetAsync");
+    if (steps->n_steps == 0 || !steps->x || !steps->w || !steps->length || !steps->beta || !steps->first)
+        return fail(OPX_ERR_INVALID_ARG, "empty or NULL step table");
+    if (photon_id_base > n_total || n > n_total - photon_id_base) return fail(OPX_ERR_INVALID_ARG, "photon ids beyond first[n_steps]");
+    if (!d_out_origins || !d_out_dirs || !d_out_wavelengths || !d_workspace) return fail(OPX_ERR_INVALID_ARG, "NULL output/workspace pointer");
+    if (misaligned(d_out_origins, 4) || misaligned(d_out_dirs, 4) || misaligned(d_out_wavelengths, 4) || misaligned(d_out_index, 4) ||
+        misaligned(d_workspace, 256) || misaligned(steps->first, 8) || misaligned(steps->x, 4) || misaligned(steps->w, 4) ||
+        misaligned(steps->length, 4) || misaligned(steps->beta, 4))
+        return fail(OPX_ERR_INVALID_ARG, "misaligned pointer");
+    if (workspace_bytes < prefilter_workspace_bytes(n)) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_prefilter_workspace_bytes)");
+    return launch_emit_filtered(*scene, *steps, n_index, lambda1_nm, lambda2_nm, n, photon_id_base, seed, factors, n_factors,
+                                d_out_origins, d_out_dirs, d_out_wavelengths, d_out_index, d_n_kept, d_workspace, (cudaStream_t)cuda_stream);
+}
+
 opx_status opx_propagate_brute(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
                                const float* d_dirs, const float* d_wavelengths, uint64_t seed, const opx_hits* out,
                                uint32_t* d_hitmap, uint64_t* d_counters, void* cuda_stream) {

@@ -60,6 +60,22 @@ __device__ __forceinline__ float table_value(const SceneDev& sc, uint32_t m, uin
     return table_lerp(y, sc.n_lambda, sc.lambda_min, sc.inv_dlambda, lambda);
 }
 
+// --------------------------------------------------------------------- pre-propagation filter (3.9)
+constexpr int kMaxFactors = 8;
+struct FilterFactors { uint32_t m[kMaxFactors]; uint32_t mk[kMaxFactors]; uint32_t n; };   // material indices, their mat_kinds words
+
+// p = e_0(lambda) * e_1(lambda) * ... left to right in fp32 (1 for an empty list)
+__device__ __forceinline__ float filter_probability(const SceneDev& sc, const FilterFactors& fa, float lambda) {
+    float p = 1.f;
+#pragma unroll
+    for (uint32_t k = 0; k < (uint32_t)kMaxFactors; ++k) {       // unrolled: the factor list is read with constant indices
+        if (k >= fa.n) break;
+        const float e = table_value(sc, fa.m[k], fa.mk[k], lambda);
+        p = k == 0 ? e : __fmul_rn(p, e);
+    }
+    return p;
+}
+
 // ------------------------------------------------------------------------------- ray set-up (3.3)
 struct RayW {                 // watertight-test constants of one segment
     float okx, oky, okz;      // origin permuted to (kx, ky, kz)

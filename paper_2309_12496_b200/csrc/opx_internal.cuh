@@ -103,7 +103,11 @@ opx_status launch_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const 
 opx_status launch_packet_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,
                                const float* wl, uint64_t seed, const opx_hits& out, uint64_t* stats, cudaStream_t stream);
 size_t wide_node_capacity(size_t n_triangles);
+void launch_prefilter_scan(uint32_t* counts, uint32_t nb, uint64_t* d_total, cudaStream_t stream);   // exclusive scan in place + total
 // Cherenkov emission (opx_emit.cu)
+opx_status launch_emit_filtered(const SceneHost& s, const opx_track_steps& st, float n_index, float lambda1, float lambda2, uint64_t n,
+                                uint64_t id_base, uint64_t seed, const uint32_t* factors, uint32_t n_factors, float* o, float* d,
+                                float* wl, uint32_t* oidx, uint64_t* d_n_kept, void* ws, cudaStream_t stream);
 opx_status launch_emit(const opx_track_steps& st, float n_index, float lambda1, float lambda2, uint64_t n, uint64_t id_base,
                        uint64_t seed, float* o, float* d, float* wl, cudaStream_t stream);
 

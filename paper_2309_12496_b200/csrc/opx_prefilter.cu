@@ -18,9 +18,7 @@ constexpr int kFWarps = kFThreads / 32;
 constexpr int kBlk = 2048;                      // photons per CTA
 constexpr int kRounds = kBlk / kFThreads;       // 8 mask words per warp
 constexpr int kWords = kBlk / 32;               // 64 mask words per CTA
-constexpr int kMaxFactors = 8;
-
-struct Factors { uint32_t m[kMaxFactors]; uint32_t mk[kMaxFactors]; uint32_t n; };
+using Factors = FilterFactors;
 
 __global__ void __launch_bounds__(kFThreads) k_prefilter_mark(const SceneDev sc, const Factors fa, uint64_t n, uint64_t id_base,
                                                               const float* __restrict__ wl, uint64_t seed,
@@ -36,13 +34,7 @@ __global__ void __launch_bounds__(kFThreads) k_prefilter_mark(const SceneDev sc,
         bool keep = false;
         if (i < n) {
             const float lambda = __ldcs(wl + i);
-            float p = 1.f;
-#pragma unroll
-            for (uint32_t k = 0; k < (uint32_t)kMaxFactors; ++k) {       // unrolled: the factor list is read with constant indices
-                if (k >= fa.n) break;
-                const float e = table_value(sc, fa.m[k], fa.mk[k], lambda);
-                p = k == 0 ? e : __fmul_rn(p, e);
-            }
+            const float p = filter_probability(sc, fa, lambda);
             keep = philox_uniform(seed, id_base + i, 0u, 1u) < p;
         }
         const uint32_t mask = __ballot_sync(0xffffffffu, keep);
@@ -126,6 +118,10 @@ __global__ void __launch_bounds__(kFThreads) k_prefilter_compact(uint64_t n, con
 }
 
 }  // namespace
+
+void launch_prefilter_scan(uint32_t* counts, uint32_t nb, uint64_t* d_total, cudaStream_t stream) {
+    k_prefilter_scan<<<1, 1024, 0, stream>>>(counts, nb, (unsigned long long*)d_total);
+}
 
 size_t prefilter_workspace_bytes(uint64_t n) {
     const uint64_t nb = (n + kBlk - 1) / kBlk;

@@ -22,7 +22,7 @@ FLAG_NO_EFFICIENCY = 1                   # opx_flags
 TABLE_LINEAR, TABLE_HISTOGRAM = 0, 1     # opx_table_interp
 
 EXPORTS = ("opx_scene_create", "opx_scene_workspace_bytes", "opx_bvh_build", "opx_propagate",
-           "opx_propagate_flags", "opx_prefilter_workspace_bytes", "opx_prefilter", "opx_emit_cherenkov", "opx_propagate_brute", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
+           "opx_propagate_flags", "opx_prefilter_workspace_bytes", "opx_prefilter", "opx_emit_cherenkov", "opx_emit_cherenkov_filtered", "opx_propagate_brute", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
            "opx_profile_begin", "opx_profile_end", "opx_propagate_stats", "opx_propagate_packet_stats",
            "opx_scene_wide_info", "opx_measure_fp32_peak",
            "opx_scene_info", "opx_scene_get_layout", "opx_launch_count", "opx_scene_destroy",
@@ -97,6 +97,8 @@ def load_library(path=LIB_PATH):
     lib.opx_prefilter_workspace_bytes.argtypes = [u64, vp]
     lib.opx_prefilter.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, u32, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
     lib.opx_emit_cherenkov.argtypes = [vp, u64, C.c_float, C.c_float, C.c_float, u64, u64, u64, vp, vp, vp, vp]
+    lib.opx_emit_cherenkov_filtered.argtypes = [vp, vp, u64, C.c_float, C.c_float, C.c_float, u64, u64, u64, vp, u32,
+                                                vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
     lib.opx_propagate_host_workspace_bytes.argtypes = [vp, u64, vp]
     lib.opx_propagate_host.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp, vp, vp, C.c_size_t, u64, vp]
     lib.opx_profile_begin.argtypes = [vp, u32]
@@ -312,6 +314,35 @@ class Scene:
             fac, len(factors), out["origins"].data_ptr(), out["dirs"].data_ptr(), out["wavelengths"].data_ptr(),
             None if idx is None else idx.data_ptr(), out["n_kept"].data_ptr(), _aligned(ws), need.value,
             C.c_void_p(st.cuda_stream)))
+        return out
+
+    def emit_cherenkov_filtered(self, dev_steps, n, factors, photon_id_base=0, seed=0, n_index=1.0014, lambda1=200.0,
+                                lambda2=600.0, out=None, stream=None, capacity=None):
+        """opx_emit_cherenkov_filtered on an uploaded step table -> the dict prefilter() returns (origins, dirs,
+        wavelengths, index, n_kept, workspace).  capacity (default n) sizes the output arrays."""
+        import torch
+        dev = dev_steps["first"].device
+        cap = int(n if capacity is None else capacity)
+        if out is None:
+            out = dict(origins=torch.empty((cap, 3), dtype=torch.float32, device=dev),
+                       dirs=torch.empty((cap, 3), dtype=torch.float32, device=dev),
+                       wavelengths=torch.empty(cap, dtype=torch.float32, device=dev),
+                       index=torch.empty(cap, dtype=torch.int32, device=dev),
+                       n_kept=torch.zeros(1, dtype=torch.int64, device=dev))
+        need = C.c_size_t()
+        _check(load_library().opx_prefilter_workspace_bytes(int(n), C.byref(need)))
+        ws = out.get("workspace")
+        if ws is None or ws.numel() < need.value + 256:
+            ws = out["workspace"] = torch.empty(need.value + 256, dtype=torch.uint8, device=dev)
+        st = TrackSteps(dev_steps["x"].data_ptr(), dev_steps["w"].data_ptr(), dev_steps["length"].data_ptr(),
+                        dev_steps["beta"].data_ptr(), dev_steps["first"].data_ptr(), int(dev_steps["length"].shape[0]))
+        fac = (C.c_uint32 * max(1, len(factors)))(*[int(f) for f in factors])
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        idx = out.get("index")
+        _check(load_library().opx_emit_cherenkov_filtered(
+            self._h, C.byref(st), int(dev_steps["n_total"]), n_index, lambda1, lambda2, int(n), int(photon_id_base), int(seed),
+            fac, len(factors), out["origins"].data_ptr(), out["dirs"].data_ptr(), out["wavelengths"].data_ptr(),
+            None if idx is None else idx.data_ptr(), out["n_kept"].data_ptr(), _aligned(ws), need.value, C.c_void_p(s.cuda_stream)))
         return out
 
     def profile_begin(self, max_calls):

@@ -131,3 +131,46 @@ def test_emit_error_paths():
                                   C.c_void_p(x.data_ptr()), None) == opx.OPX_ERR_INVALID_ARG
     o, d, lam = pkg.emit_cherenkov(ds, 50, seed=1)                       # still works afterwards
     assert torch.isfinite(d).all()
+
+
+def test_fused_emit_filter_equals_the_two_calls_and_the_oracle_chain():
+    """opx_emit_cherenkov_filtered == opx_emit_cherenkov then opx_prefilter == oracle.emit_cherenkov then
+    oracle.prefilter: survivor count, ids (stable order) and every bit of the survivors' photons; block boundaries
+    (2048 ids), a ragged tail, a 64-bit id base into the table, K = 0 (everything kept) and n = 0."""
+    w = wl.make_config("C3", n=3_000_000)
+    st = w.track_source.steps()
+    ds = pkg.upload_track_steps(st)
+    gs = pkg.Scene(w.scene).build()
+    fac = [w.scene.info["m_det"], w.scene.info["m_mir"], w.scene.info["m_mir"]]
+    for a, m in ((0, 1), (5, 2048), (2_000_001, 2049), (1_111_111, 300_037)):
+        fused = gs.emit_cherenkov_filtered(ds, m, fac, photon_id_base=a, seed=6)
+        o, d, lam = pkg.emit_cherenkov(ds, m, photon_id_base=a, seed=6)
+        two = gs.prefilter(o, d, lam, fac, seed=6, photon_id_base=a)
+        k = int(fused["n_kept"].item())
+        assert k == int(two["n_kept"].item())
+        for key in ("origins", "dirs", "wavelengths", "index"):
+            assert torch.equal(fused[key][:k], two[key][:k]), key
+        ro, rd, rl = oracle.emit_cherenkov(st, m, id_base=a, seed=6)
+        f = oracle.prefilter(w.scene, rl, fac, seed=6, id_base=a)
+        assert k == len(f.index) and np.array_equal(fused["index"][:k].cpu().numpy().view(np.uint32), f.index)
+        _assert_same_bits((fused["origins"][:k], fused["dirs"][:k], fused["wavelengths"][:k]), (ro[f.index], rd[f.index], rl[f.index]))
+    allk = gs.emit_cherenkov_filtered(ds, 5000, [], photon_id_base=77, seed=6)
+    assert int(allk["n_kept"].item()) == 5000
+    _assert_same_bits((allk["origins"], allk["dirs"], allk["wavelengths"]), oracle.emit_cherenkov(st, 5000, id_base=77, seed=6))
+    none = gs.emit_cherenkov_filtered(ds, 0, fac, out=dict(allk, n_kept=torch.full((1,), 9, dtype=torch.int64, device="cuda")))
+    assert int(none["n_kept"].item()) == 0
+    # the chain to hits: survivors traced with efficiencies off == the oracle's chain
+    a, m = 1_500_000, 40_000
+    fused = gs.emit_cherenkov_filtered(ds, m, fac[:2], photon_id_base=a, seed=2, capacity=m // 2)
+    geo = gs.propagate(fused["origins"], fused["dirs"], fused["wavelengths"], flags=opx.FLAG_NO_EFFICIENCY, n_dev=fused["n_kept"])
+    ro, rd, rl = oracle.emit_cherenkov(st, m, id_base=a, seed=2)
+    f = oracle.prefilter(w.scene, rl, fac[:2], seed=2, id_base=a)
+    ref = oracle.trace_mesh(w.scene, ro[f.index], rd[f.index], rl[f.index], flags=oracle.NO_EFFICIENCY)
+    k = len(f.index)
+    for key in ("state", "surface", "pixel", "bounces"):
+        assert np.array_equal(geo[key][:k].cpu().numpy(), ref[key]), key
+    assert np.array_equal(geo["hitmap"].cpu().numpy(), ref["hitmap"])
+    with pytest.raises(pkg.OpxError):
+        gs.emit_cherenkov_filtered(ds, 10, [len(w.scene.materials)])
+    with pytest.raises(pkg.OpxError):
+        gs.emit_cherenkov_filtered(ds, 10, fac, photon_id_base=ds["n_total"] - 5)
