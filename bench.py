@@ -411,14 +411,45 @@ def main():
             ev1.record(stream)
             torch.cuda.synchronize()
             etimes[name] = ev0.elapsed_time(ev1) / args.steps * 1e-3
+        # the paper's whole pipeline from track steps: emission fused with the filter, survivors traced with efficiencies off
+        kinds_e = [m["kind"] for m in w.scene.materials]
+        fac_e = [kinds_e.index(2)] + [kinds_e.index(1)] * (2 if args.config in ("C4", "C5") else 1)
+        cap = n // 2 + 4096
+        fpre = scene.emit_cherenkov_filtered(dsteps, n, fac_e, seed=args.seed, stream=stream, capacity=cap)
+        if int(fpre["n_kept"].item()) > cap:
+            raise SystemExit("bench: survivor capacity exceeded")
+
+        def fused_step(trace):
+            scene.emit_cherenkov_filtered(dsteps, n, fac_e, seed=args.seed, out=fpre, stream=stream)
+            if trace:
+                hm3.zero_(); ct3.zero_()
+                scene.propagate(fpre["origins"], fpre["dirs"], fpre["wavelengths"], seed=args.seed,
+                                records={k: v[:cap] for k, v in records.items()}, hitmap=hm3, counters=ct3, stream=stream,
+                                flags=pkg.FLAG_NO_EFFICIENCY, n_dev=fpre["n_kept"])
+        for name, trace in (("fused", False), ("fused_chain", True)):
+            for _ in range(args.warmup):
+                fused_step(trace)
+            torch.cuda.synchronize()
+            ev0.record(stream)
+            for _ in range(args.steps):
+                fused_step(trace)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            etimes[name] = ev0.elapsed_time(ev1) / args.steps * 1e-3
         emit = {"what": f"opx_emit_cherenkov: {n} photons from {int(dsteps['length'].shape[0])} track steps"
                         + ("" if w.track_source is not None else " (step table of C3: C2's photons are a point source, not tracks)"),
                 "value": n / etimes["emit"], "unit": UNIT, "ms_per_step": 1e3 * etimes["emit"],
                 "roofline": {"bound": "hbm", "achieved": BYTES_IN * n / etimes["emit"] / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                              "frac": BYTES_IN * n / etimes["emit"] / 1e9 / peaks["hbm_gbs"], "bytes_per_photon": BYTES_IN,
                              "note": "issue-bound on the contract's arithmetic (Philox, IEEE divides), not HBM: profiles/r01_v11_emit.md"},
-                "emit_then_propagate": {"value": n / etimes["chain"], "unit": UNIT, "ms_per_step": 1e3 * etimes["chain"],
-                                        "detected": int(ct3[0].item())}}
+                "emit_then_propagate": {"value": n / etimes["chain"], "unit": UNIT, "ms_per_step": 1e3 * etimes["chain"]},
+                "emit_filtered": {"what": "opx_emit_cherenkov_filtered (emission fused with the pre-propagation filter)",
+                                  "value": n / etimes["fused"], "unit": UNIT, "ms_per_step": 1e3 * etimes["fused"],
+                                  "kept_fraction": int(fpre["n_kept"].item()) / n},
+                "emit_filtered_then_propagate": {"what": "the paper's pipeline from track steps to hits, memory-resident: fused "
+                                                         "emission + filter, survivors traced with NO_EFFICIENCY",
+                                                 "value": n / etimes["fused_chain"], "unit": UNIT,
+                                                 "ms_per_step": 1e3 * etimes["fused_chain"], "detected": int(ct3[0].item())}}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
