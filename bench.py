@@ -3,7 +3,7 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config C2] [--photons n]
 
-One "step" = one opx_propagate call (propagation kernel + hit binning + counters) over one batch of
+One "step" = one opx_propagate call (one kernel: propagation with hit binning and counters inside) over one batch of
 synthetic photons of the named BASELINE.json config (default C2 = configs[1]: toy RICH, 20 014
 triangles, 1e7 photons), inputs resident in HBM.  The BVH build is timed separately (`bvh_build_ms`)
 as SURVEY.md 8(d) prescribes.  N > 1 (torchrun): every rank propagates its own contiguous id range
