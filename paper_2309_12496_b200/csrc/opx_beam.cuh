@@ -160,7 +160,8 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayW&
         const unsigned mt = __ballot_sync(full, hit && cref < 0);
         if (mt) {
             unsigned mine = mt;                      // the triangle children this lane still has to test
-            if (!kMixed && __popc(mt) >= kCullMin) {
+            const bool culled = !kMixed && __popc(mt) >= kCullMin;       // warp-uniform
+            if (culled) {
                 // per-lane cull: own ray against the candidate boxes (all member rays share the beam's sign octant, so
                 // near/far are the same planes for every lane).  Approximate reciprocals: see slab_setup.
                 if (kStats) ++stats.culls;
@@ -180,13 +181,25 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayW&
                     if (en <= exi) mine |= 1u << L;
                 } while (m);
             }
-            while (__any_sync(full, mine != 0u)) {
-                const bool has = mine != 0u;
-                const int L = has ? __ffs(mine) - 1 : 0;
-                mine &= mine - 1u;
-                const int j = ~__shfl_sync(full, cref, L);
-                if (kStats) ++stats.tris;
-                if (alive && has) consider(sc, rw, j, tmin, last, h);
+            if (!culled) {
+                // no per-lane cull (warp-uniform): one uniform pass over the candidates, no votes, no per-lane bit scans
+                unsigned m = mt;
+                do {
+                    const int L = __ffs(m) - 1;
+                    m &= m - 1u;
+                    const int j = ~__shfl_sync(full, cref, L);
+                    if (kStats) ++stats.tris;
+                    if (alive) consider(sc, rw, j, tmin, last, h);
+                } while (m);
+            } else {
+                while (__any_sync(full, mine != 0u)) {
+                    const bool has = mine != 0u;
+                    const int L = has ? __ffs(mine) - 1 : 0;
+                    mine &= mine - 1u;
+                    const int j = ~__shfl_sync(full, cref, L);
+                    if (kStats) ++stats.tris;
+                    if (alive && has) consider(sc, rw, j, tmin, last, h);
+                }
             }
             thi = warp_max(alive ? h.t - s : -kInf);
         }

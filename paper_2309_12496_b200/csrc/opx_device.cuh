@@ -103,6 +103,27 @@ __device__ __forceinline__ RayW ray_setup(float ox, float oy, float oz, float dx
     return r;
 }
 
+// The same set-up for a segment stored as o[3], d[3] in (shared) memory: the permuted components are fetched with
+// indexed loads instead of register selects.  Same values, same operations.
+__device__ __forceinline__ RayW ray_setup_mem(const float* o, const float* d) {
+    RayW r;
+    const float dx = d[0], dy = d[1], dz = d[2];
+    int kz = 0;
+    float best = fabsf(dx);
+    if (fabsf(dy) > best) { kz = 1; best = fabsf(dy); }
+    if (fabsf(dz) > best) { kz = 2; }
+    int kx = kz == 2 ? 0 : kz + 1;
+    int ky = kx == 2 ? 0 : kx + 1;
+    const float dkz = d[kz];
+    if (dkz < 0.f) { const int t = kx; kx = ky; ky = t; }
+    r.kx = kx; r.ky = ky; r.kz = kz;
+    r.Sx = __fdiv_rn(d[kx], dkz);
+    r.Sy = __fdiv_rn(d[ky], dkz);
+    r.Sz = __fdiv_rn(1.f, dkz);
+    r.okx = o[kx]; r.oky = o[ky]; r.okz = o[kz];
+    return r;
+}
+
 // Contract triangle test on vertex components already permuted to (kx, ky, kz) and shifted to the ray
 // origin (A = a - o, ...).  Returns true with t when the triangle is hit at finite t > tmin.
 __device__ __forceinline__ bool tri_test(const RayW& r, float Akx, float Aky, float Akz, float Bkx, float Bky, float Bkz,
@@ -125,7 +146,8 @@ __device__ __forceinline__ bool tri_test(const RayW& r, float Akx, float Aky, fl
         const double T = __fma_rn(Wd, Cz, __fma_rn(Vd, Bz, __dmul_rn(Ud, Az)));
         t = __double2float_rn(__ddiv_rn(T, det));
     } else {
-        if ((U < 0.f || V < 0.f || W < 0.f) && (U > 0.f || V > 0.f || W > 0.f)) return false;
+        // (U<0 || V<0 || W<0) && (U>0 || V>0 || W>0): fminf/fmaxf skip a NaN operand exactly as the comparisons do
+        if (fminf(fminf(U, V), W) < 0.f && fmaxf(fmaxf(U, V), W) > 0.f) return false;
         const float det = __fadd_rn(__fadd_rn(U, V), W);
         if (det == 0.f) return false;
         const float Az = __fmul_rn(r.Sz, Akz), Bz = __fmul_rn(r.Sz, Bkz), Cz = __fmul_rn(r.Sz, Ckz);

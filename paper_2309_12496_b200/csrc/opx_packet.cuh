@@ -340,7 +340,7 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
             bool done = false;
             {
                 const float ox = so[0], oy = so[1], oz = so[2], dx = sd[0], dy = sd[1], dz = sd[2];
-                rw = ray_setup(ox, oy, oz, dx, dy, dz);
+                rw = ray_setup_mem(so, sd);
                 Beam bm;
                 float s;
                 const unsigned tris_before = bstats.tris, visits_before = bstats.visits;
