@@ -20,23 +20,18 @@
 namespace opx {
 namespace {
 
-#ifndef OPX_PKT_THREADS
-#define OPX_PKT_THREADS 512
-#endif
-#ifndef OPX_PKT_CTAS
-#define OPX_PKT_CTAS 2
-#endif
-constexpr int kPktThreads = OPX_PKT_THREADS;
-constexpr int kPktCtas = OPX_PKT_CTAS;               // resident CTAs per SM the kernel is compiled for
-constexpr int kPktWarps = kPktThreads / 32;          // 16
-constexpr int kItems = 4;                            // photons per thread in the staging / sort phases
-constexpr int kTile = kItems * kPktThreads;          // 2048 photons per CTA tile
 constexpr int kPktStack = 96;                        // depth bound of the Karras tree (see opx_lane.cuh)
 constexpr int kStackSmem = kPktStack - 32;
-
 constexpr int kRadixBits = 6, kRadix = 1 << kRadixBits;      // 2 passes over the 12-bit key
 
-struct PacketSmem {
+// The kernel is compiled for two tile sizes on 512 threads: kItems = 4 photons per thread, 2048-photon tiles (the
+// product shape: the more photons of a ring a tile holds, the narrower its packets; each warp walks 4 packets), and
+// kItems = 1, 512-photon tiles where each warp walks ONE packet, for calls too small to fill the machine with large
+// tiles: four times the CTAs and a quarter of the latency (the paper's own runs are 600 ... 6e5 photons).
+template <int kPktThreads, int kItems>
+struct PacketSmemT {
+    static constexpr int kPktWarps = kPktThreads / 32;
+    static constexpr int kTile = kItems * kPktThreads;
     float o[kTile * 3];          // in: origins            out: hit positions
     float d[kTile * 3];          // in: directions         out: arrival directions
     float wl[kTile];             // in: wavelengths        out: pixel ids (int bits)
@@ -51,7 +46,7 @@ struct PacketSmem {
     float beam_tn[kPktWarps][kBeamStack];        // beam traversal: entry bounds of the stacked wide nodes (refs alias `stack`)
     float red[kPktWarps][3];
     float bcast[3];
-    uint32_t scan_tot[kPktWarps];
+    uint32_t scan_tot[kPktWarps < 8 ? 8 : kPktWarps];    // sort: per-warp totals; store phase: the 8 state counters
     int next_group;              // dynamic hand-out of packet groups to warps
 };
 static_assert(sizeof(int) * kStackSmem >= sizeof(uint32_t) * kRadix, "radix counters alias the stack overflow area");
@@ -70,7 +65,9 @@ __device__ __forceinline__ void octa(float dx, float dy, float dz, float& u, flo
     if (!(fabsf(v) <= 1.f)) v = 0.f;
 }
 
-__device__ __forceinline__ void block_sum3(PacketSmem& sm, float x, float y, float z, float& sx, float& sy, float& sz) {
+template <int kPktThreads, int kItems>
+__device__ __forceinline__ void block_sum3(PacketSmemT<kPktThreads, kItems>& sm, float x, float y, float z, float& sx, float& sy, float& sz) {
+    constexpr int kPktWarps = kPktThreads / 32;
     for (int off = 16; off > 0; off >>= 1) {
         x += __shfl_xor_sync(0xffffffffu, x, off); y += __shfl_xor_sync(0xffffffffu, y, off); z += __shfl_xor_sync(0xffffffffu, z, off);
     }
@@ -88,7 +85,9 @@ __device__ __forceinline__ void block_sum3(PacketSmem& sm, float x, float y, flo
 // One stable radix pass (kRadixBits bits) src -> dst over kTile packed keys.  Warp w owns the
 // 32*kItems consecutive entries [w*32*kItems, ...) and ranks them in kItems rounds with
 // __match_any_sync; the kRadix x kPktWarps counters are scanned in (digit, warp) order.
-__device__ __forceinline__ void smem_radix_pass(PacketSmem& sm, const uint32_t* src, uint32_t* dst, int shift) {
+template <int kPktThreads, int kItems>
+__device__ __forceinline__ void smem_radix_pass(PacketSmemT<kPktThreads, kItems>& sm, const uint32_t* src, uint32_t* dst, int shift) {
+    constexpr int kPktWarps = kPktThreads / 32;
     constexpr int kCnt = kRadix * kPktWarps, kPer = kCnt / kPktThreads;   // 1024 counters, 2 per thread
     static_assert(kCnt % kPktThreads == 0, "counter scan layout");
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -197,7 +196,7 @@ __device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW
     return h;
 }
 
-template <bool kStats>
+template <int kPktThreads, int kItems, int kPktCtas, bool kStats>
 __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(const SceneDev sc, uint64_t n, uint64_t id_base,
                                                                      const float* __restrict__ origins,
                                                                      const float* __restrict__ dirs,
@@ -205,6 +204,8 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
                                                                      uint32_t* hitmap, unsigned long long* counters,
                                                                      unsigned long long* stats) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    using PacketSmem = PacketSmemT<kPktThreads, kItems>;
+    constexpr int kPktWarps = PacketSmem::kPktWarps, kTile = PacketSmem::kTile;
     PacketSmem& sm = *reinterpret_cast<PacketSmem*>(smem_raw);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const uint64_t tile_base = (uint64_t)blockIdx.x * kTile;
@@ -221,11 +222,11 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
         const float4* gd = reinterpret_cast<const float4*>(dirs + 3 * tile_base);
         const float4* gw = reinterpret_cast<const float4*>(wl + tile_base);
 #pragma unroll
-        for (int k = 0; k < 3 * kTile / 4 / kPktThreads; ++k) {
-            reinterpret_cast<float4*>(sm.o)[k * kPktThreads + threadIdx.x] = __ldcs(go + k * kPktThreads + threadIdx.x);
-            reinterpret_cast<float4*>(sm.d)[k * kPktThreads + threadIdx.x] = __ldcs(gd + k * kPktThreads + threadIdx.x);
+        for (int k = threadIdx.x; k < 3 * kTile / 4; k += kPktThreads) {
+            reinterpret_cast<float4*>(sm.o)[k] = __ldcs(go + k);
+            reinterpret_cast<float4*>(sm.d)[k] = __ldcs(gd + k);
         }
-        reinterpret_cast<float4*>(sm.wl)[threadIdx.x] = __ldcs(gw + threadIdx.x);
+        if (threadIdx.x < kTile / 4) reinterpret_cast<float4*>(sm.wl)[threadIdx.x] = __ldcs(gw + threadIdx.x);
     } else {
         for (int k = threadIdx.x; k < 3 * m; k += kPktThreads) {
             sm.o[k] = __ldcs(origins + 3 * tile_base + k);
@@ -402,7 +403,6 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
     //     a warp that share a pixel are merged into one atomic, states are counted with ballots.  Integer adds only.
     if (hitmap || counters) {
         uint32_t* s_cnt = sm.scan_tot;                       // 8 of its kPktWarps words; free since the sort
-        static_assert(kPktWarps >= 8, "state counters alias scan_tot");
         if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0;
         __syncthreads();
         unsigned seg = 0, acc = 0;                           // acc: seven 4-bit per-state counts of this thread (<= kItems each)

@@ -24,18 +24,26 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
         if (blocks > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
         k_propagate_lane<true, false><<<(unsigned)blocks, 128, 0, stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr);
     } else {
+        // tile size: 2048 photons (4 packets per warp) unless the call is too small to give every SM one such tile; then
+        // 512 photons (1 packet per warp: four times the CTAs, a quarter of the latency)
+        using Big = PacketSmemT<512, 4>;
+        using Small = PacketSmemT<512, 1>;
         static bool configured = false;
         if (!configured) {
-            if (opx_status st = check_cuda(cudaFuncSetAttribute(k_propagate_packet<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                                (int)sizeof(PacketSmem)), "cudaFuncSetAttribute")) return st;
-            if (opx_status st = check_cuda(cudaFuncSetAttribute(k_propagate_packet<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                                (int)sizeof(PacketSmem)), "cudaFuncSetAttribute")) return st;
+            cudaError_t e = cudaSuccess;
+            if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
+            if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
+            if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 1, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Small));
+            if (opx_status st = check_cuda(e, "cudaFuncSetAttribute")) return st;
             configured = true;
         }
-        const uint64_t tiles = (n + kTile - 1) / kTile;
+        const bool small = !packet_stats && n < (uint64_t)Big::kTile * 148;
+        const uint64_t tile = small ? Small::kTile : Big::kTile;
+        const uint64_t tiles = (n + tile - 1) / tile;
         if (tiles > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
-        if (packet_stats) k_propagate_packet<true><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr, nullptr, (unsigned long long*)packet_stats);
-        else k_propagate_packet<false><<<(unsigned)tiles, kPktThreads, sizeof(PacketSmem), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
+        if (packet_stats) k_propagate_packet<512, 4, 2, true><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr, nullptr, (unsigned long long*)packet_stats);
+        else if (small) k_propagate_packet<512, 1, 2, false><<<(unsigned)tiles, 512, sizeof(Small), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
+        else k_propagate_packet<512, 4, 2, false><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
         binned = !packet_stats;
     }
     count_launch(1);

@@ -101,6 +101,25 @@ def test_c2_c3_sampled_parity(toy, name, stride, seed):
         assert len(np.unique(ref["state"])) >= 5        # the workload exercises the terminal states
 
 
+def test_both_cta_shapes_against_the_oracle(toy):
+    """opx_propagate picks 512-photon tiles (one packet per warp) for calls below 148 large tiles and 2048-photon tiles
+    (four packets per warp) above: 620 000 contiguous C3 photons take the large tiles, their first 50 000 alone the small one;
+    both must reproduce the oracle, hence each other, bit for bit."""
+    sc, gs = toy
+    w = wl.make_config("C3", n=2_000_000)
+    n = 620_000
+    o, d, lam = w.photon_range(700_000, 700_000 + n)
+    do, dd, dl = _dev(o, d, lam)
+    big = _host(gs.propagate(do, dd, dl, seed=21, photon_id_base=700_000))
+    ref = oracle.trace_mesh(sc, o, d, lam, seed=21, id_base=700_000)
+    nbad, dmax = assert_parity(big, ref, n)
+    assert nbad == 0 and dmax == 0.0
+    m = 50_000
+    small = _host(gs.propagate(do[:m].contiguous(), dd[:m].contiguous(), dl[:m].contiguous(), seed=21, photon_id_base=700_000))
+    for k in ("state", "pixel", "surface", "bounces", "pos", "dir"):
+        assert np.array_equal(small[k], big[k][:m]), k
+
+
 def test_id_base_and_chunking(toy):
     """Global photon id = base + i keys the RNG: chunked calls reproduce the one-shot call, and match
     the oracle run with the same ids."""
