@@ -399,8 +399,7 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
         }
     }
 
-    // 4a. A11 + A12 for this tile, straight from shared memory (what k_bin does for the other kernels): detected photons of
-    //     a warp that share a pixel are merged into one atomic, states are counted with ballots.  Integer adds only.
+    // 4a. A11 + A12 for this tile, straight from shared memory (what k_bin does for the other kernels).  Integer adds only.
     if (hitmap || counters) {
         uint32_t* s_cnt = sm.scan_tot;                       // 8 of its kPktWarps words; free since the sort
         if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0;
@@ -411,9 +410,21 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
             const bool ok = k < m;
             const int st = ok ? (int)sm.state[k] : 7;
             if (ok) { seg += (unsigned)sm.bounces[k] + (st != OPX_BOUNCE_LIMIT ? 1u : 0u); acc += 1u << (4 * st); }
-            const int key = st == OPX_DETECTED ? __float_as_int(sm.wl[k]) : -1 - lane;     // unique key for the other lanes
-            const unsigned peers = __match_any_sync(0xffffffffu, key);
-            if (hitmap && st == OPX_DETECTED && lane == __ffs(peers) - 1) atomicAdd(&hitmap[key], (unsigned)__popc(peers));
+            if (hitmap) {
+                // one atomic per detected photon, except when all detected photons of the warp share a pixel (a focused spot:
+                // the case that would serialise on one address), which costs one atomic per warp.  A full __match_any_sync
+                // merge of equal pixels was measured at 3 % of the kernel on C2, where a ring spreads over ~700 pixels.
+                const bool det = st == OPX_DETECTED;
+                const unsigned dm = __ballot_sync(0xffffffffu, det);
+                if (dm) {
+                    const int pix = det ? __float_as_int(sm.wl[k]) : 0;
+                    const int lead = __ffs(dm) - 1;
+                    const int first = __shfl_sync(0xffffffffu, pix, lead);
+                    const unsigned same = __ballot_sync(0xffffffffu, det && pix == first);
+                    if (same == dm) { if (lane == lead) atomicAdd(&hitmap[first], (unsigned)__popc(dm)); }
+                    else if (det) atomicAdd(&hitmap[pix], 1u);
+                }
+            }
         }
         if (counters) {
             // widen the 4-bit fields to 8 bits (a warp sums to <= 32 * kItems = 128 per state) and add across the warp
