@@ -166,11 +166,11 @@ struct Hit { float t; int j; int gid; };   // j: leaf-order index; gid: global t
 // lanes of a warp read the same sectors), so no register selects are needed.
 __device__ __forceinline__ void consider(const SceneDev& sc, const RayW& rw, int j, float tmin, int last, Hit& h) {
     const float* t = reinterpret_cast<const float*>(sc.tris + 3 * (size_t)j);
-    const int gid = __float_as_int(__ldg(t + 3));
-    if (gid == last) return;
+    const int gid = __float_as_int(__ldg(t + 3));      // all ten loads are issued before the first use: one latency, not two
     const float Akx = __fsub_rn(__ldg(t + rw.kx), rw.okx), Aky = __fsub_rn(__ldg(t + rw.ky), rw.oky), Akz = __fsub_rn(__ldg(t + rw.kz), rw.okz);
     const float Bkx = __fsub_rn(__ldg(t + 4 + rw.kx), rw.okx), Bky = __fsub_rn(__ldg(t + 4 + rw.ky), rw.oky), Bkz = __fsub_rn(__ldg(t + 4 + rw.kz), rw.okz);
     const float Ckx = __fsub_rn(__ldg(t + 8 + rw.kx), rw.okx), Cky = __fsub_rn(__ldg(t + 8 + rw.ky), rw.oky), Ckz = __fsub_rn(__ldg(t + 8 + rw.kz), rw.okz);
+    if (gid == last) return;
     float tt;
     if (!tri_test(rw, Akx, Aky, Akz, Bkx, Bky, Bkz, Ckx, Cky, Ckz, tmin, tt)) return;
     if (tt < h.t || (tt == h.t && gid < h.gid)) { h.t = tt; h.j = j; h.gid = gid; }
