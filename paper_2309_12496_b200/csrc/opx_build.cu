@@ -16,7 +16,10 @@ namespace opx {
 
 namespace {
 
-constexpr float kBeamWidthInTriangles = 8.f;    // beam_max_width = this x the typical triangle size
+#ifndef OPX_BEAM_WIDTH
+#define OPX_BEAM_WIDTH 4.f
+#endif
+constexpr float kBeamWidthInTriangles = OPX_BEAM_WIDTH;    // beam_max_width = this x the typical triangle size
 constexpr int kSortBlock = 256;
 constexpr int kSortItems = 8;
 constexpr int kSortTile = kSortBlock * kSortItems;  // 2048 keys per block per pass
