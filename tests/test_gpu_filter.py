@@ -262,3 +262,29 @@ def test_filter_error_paths(toy):
     assert e.value.status == opx.OPX_ERR_INVALID_ARG
     out = _host(gs.propagate(x3, x3, x1, flags=opx.FLAG_NO_EFFICIENCY))  # the library still works
     assert np.all(out["state"] == 6)
+
+
+def test_large_scene_filtered_stream_kernel_shape_equals_small_calls(lhcb):
+    """On a large scene a NO_EFFICIENCY call of >= 148 large tiles runs the 384-thread kernel shape, smaller calls the
+    512-photon-tile shape (which test_filter_then_trace_matches_oracle_c4 pins to the oracle on this scene): the same
+    400 000 photons through one call and through two calls must give identical records, hit-maps and counters."""
+    sc, gs = lhcb
+    w = wl.make_config("C4")
+    n = 400_000
+    o, d, lam = w.photon_range(5_000_000, 5_000_000 + n)
+    do, dd, dl = _dev(o, d, lam)
+    one = _host(gs.propagate(do, dd, dl, flags=opx.FLAG_NO_EFFICIENCY))
+    hm, ct = gs.alloc_accumulators()
+    h = n // 2
+    parts = [_host(gs.propagate(do[a:b].contiguous(), dd[a:b].contiguous(), dl[a:b].contiguous(), flags=opx.FLAG_NO_EFFICIENCY,
+                                hitmap=hm, counters=ct)) for a, b in ((0, h), (h, n))]
+    for k in ("state", "pixel", "surface", "bounces", "pos", "dir"):
+        assert np.array_equal(np.concatenate([p[k] for p in parts]), one[k]), k
+    assert np.array_equal(parts[-1]["hitmap"], one["hitmap"]) and np.array_equal(parts[-1]["counters"], one["counters"])
+    assert int(one["counters"][:7].sum()) == n and not np.isin(one["state"], [1, 3]).any()
+    # and against the oracle on a sample of the one-call result
+    idx = np.arange(0, n, 400)
+    ref = oracle.trace_mesh(sc, o[idx], d[idx], lam[idx], flags=oracle.NO_EFFICIENCY)
+    for k in REC:
+        assert np.array_equal(one[k][idx], ref[k]), k
+    assert np.array_equal(one["pos"][idx].astype(np.float64), ref["pos"])
