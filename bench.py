@@ -181,7 +181,7 @@ def main():
     ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--photons", type=int, default=None, help="photons per GPU per step (default: the config's N)")
     ap.add_argument("--seed", type=int, default=0)
-    ap.add_argument("--cpu-sample", type=int, default=60000, help="photons of the cpu_baseline sample")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0, help="CPU time budget of each cpu_baseline leg (all cores, one thread)")
     ap.add_argument("--reference-sample", type=int, default=20000)
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -453,9 +453,12 @@ def main():
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        n_sample = min(n, args.cpu_sample)
+        # bounded sample: a quick probe sets the size so that each leg is about --cpu-seconds of CPU work
+        probe_n = min(n, 2000)
+        rate, threads, _, _ = time_oracle(w, probe_n, args.seed)
+        n_sample = int(min(n, max(probe_n, rate * args.cpu_seconds)))
         v, threads, secs, segs = time_oracle(w, n_sample, args.seed)
-        n1 = max(1000, n_sample // max(2, threads))
+        n1 = int(min(n_sample, max(500, v / max(1, threads) * args.cpu_seconds)))
         v1, _, secs1, _ = time_oracle(w, n1, args.seed, n_threads=1)
         cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
                "sample": f"first {n_sample} photon ids of {args.config}, brute force over {w.scene.n_triangles} triangles, {secs:.1f} s "
