@@ -95,11 +95,17 @@ def run_reference(args):
         return
     import workloads
     w = workloads.make_config(args.config, n=args.photons)
-    n_sample = min(w.n, args.reference_sample)
     import oracle
+    # bounded sample per step: at most --reference-sample photons, and no more than about 3 s of work (probed), so that
+    # `--steps K --warmup W` ends within minutes on any config
+    po, pd, pl = w.photon_range(0, 1000)
+    t0 = time.perf_counter()
+    oracle.trace_mesh(w.scene, po, pd, pl, seed=args.seed)
+    rate = 1000 / (time.perf_counter() - t0)
+    n_sample = int(min(w.n, args.reference_sample, max(1000, rate * 3.0)))
     o, d, lam = w.photon_range(0, n_sample)
     for _ in range(args.warmup):
-        oracle.trace_mesh(w.scene, o[:2000], d[:2000], lam[:2000], seed=args.seed)
+        oracle.trace_mesh(w.scene, o[:1000], d[:1000], lam[:1000], seed=args.seed)
     t0 = time.perf_counter()
     threads = 0
     for _ in range(args.steps):
