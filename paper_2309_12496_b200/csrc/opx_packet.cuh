@@ -48,9 +48,40 @@ struct PacketSmemT {
     float bcast[3];
     uint32_t scan_tot[kPktWarps < 8 ? 8 : kPktWarps];    // sort: per-warp totals; store phase: the 8 state counters
     int next_group;              // dynamic hand-out of packet groups to warps
+    alignas(8) unsigned long long mbar;          // completion barrier of the bulk loads of the staging phase
 };
 static_assert(sizeof(int) * kStackSmem >= sizeof(uint32_t) * kRadix, "radix counters alias the stack overflow area");
 static_assert(kBeamStack <= kStackSmem, "the beam stack refs alias the binary walk's overflow area");
+
+// ---- TMA bulk copies (cp.async.bulk, 1-D): a full tile's inputs and records are contiguous 16-byte-aligned blocks, so one
+// elected thread moves them between global and shared memory instead of 512 threads looping over float4s.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(void* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity) {
+    asm volatile("{\n"
+                 ".reg .pred p;\n"
+                 "OPX_WAIT_%=:\n"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+                 "@p bra OPX_DONE_%=;\n"
+                 "bra OPX_WAIT_%=;\n"
+                 "OPX_DONE_%=:\n"
+                 "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, void* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(__cvta_generic_to_global(src)), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                 ::"l"(__cvta_generic_to_global(dst)), "r"(smem_u32(src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
 // Octahedral map of a direction to [-1,1]^2 (NaN-safe: garbage maps to 0,0).
 __device__ __forceinline__ void octa(float dx, float dy, float dz, float& u, float& v) {
@@ -222,27 +253,27 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
     const int m = (int)min((uint64_t)kTile, n - tile_base);
     if (threadIdx.x == 0) sm.next_group = 0;
 
-    // 1. stage the tile (coalesced, streaming: read once); 16-byte loads for full, aligned tiles
-    const bool vec = m == kTile && ((reinterpret_cast<uintptr_t>(origins) | reinterpret_cast<uintptr_t>(dirs) |
-                                     reinterpret_cast<uintptr_t>(wl)) & 15) == 0;
-    if (vec) {
-        const float4* go = reinterpret_cast<const float4*>(origins + 3 * tile_base);
-        const float4* gd = reinterpret_cast<const float4*>(dirs + 3 * tile_base);
-        const float4* gw = reinterpret_cast<const float4*>(wl + tile_base);
-#pragma unroll
-        for (int k = threadIdx.x; k < 3 * kTile / 4; k += kPktThreads) {
-            reinterpret_cast<float4*>(sm.o)[k] = __ldcs(go + k);
-            reinterpret_cast<float4*>(sm.d)[k] = __ldcs(gd + k);
+    // 1. stage the tile (read once).  A full tile whose three input blocks are 16-byte aligned is fetched by three TMA bulk
+    //    copies issued by one thread; anything else (the ragged last tile, odd slices) by coalesced streaming loads.
+    const bool bulk_in = m == kTile && aligned16(origins + 3 * tile_base) && aligned16(dirs + 3 * tile_base) && aligned16(wl + tile_base);
+    if (bulk_in) {
+        if (threadIdx.x == 0) mbar_init(&sm.mbar, 1);
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            mbar_expect_tx(&sm.mbar, (uint32_t)(kTile * 28));
+            bulk_g2s(sm.o, origins + 3 * tile_base, kTile * 12, &sm.mbar);
+            bulk_g2s(sm.d, dirs + 3 * tile_base, kTile * 12, &sm.mbar);
+            bulk_g2s(sm.wl, wl + tile_base, kTile * 4, &sm.mbar);
         }
-        if (threadIdx.x < kTile / 4) reinterpret_cast<float4*>(sm.wl)[threadIdx.x] = __ldcs(gw + threadIdx.x);
+        mbar_wait(&sm.mbar, 0);
     } else {
         for (int k = threadIdx.x; k < 3 * m; k += kPktThreads) {
             sm.o[k] = __ldcs(origins + 3 * tile_base + k);
             sm.d[k] = __ldcs(dirs + 3 * tile_base + k);
         }
         for (int k = threadIdx.x; k < m; k += kPktThreads) sm.wl[k] = __ldcs(wl + tile_base + k);
+        __syncthreads();
     }
-    __syncthreads();
 
     // 2. sort key: (run of the tile the photon belongs to, 10-bit pseudo-angle of its direction about
     //    the run's mean direction in the octahedral plane).  A run is a stretch of consecutive photons
@@ -448,7 +479,25 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
         }
     }
 
-    // 4. write the tile's records (coalesced, streaming)
+    // 4. write the tile's records: six TMA bulk stores by one thread for a full, aligned tile, else coalesced streaming stores
+    const bool bulk_out = m == kTile && aligned16(out.pos + 3 * tile_base) && aligned16(out.dir + 3 * tile_base) &&
+                          aligned16(out.pixel + tile_base) && aligned16(out.surface + tile_base) && aligned16(out.state + tile_base) &&
+                          aligned16(out.bounces + tile_base);
+    if (bulk_out) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // this thread's record writes -> visible to the TMA engine
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            bulk_s2g(out.pos + 3 * tile_base, sm.o, kTile * 12);
+            bulk_s2g(out.dir + 3 * tile_base, sm.d, kTile * 12);
+            bulk_s2g(out.pixel + tile_base, sm.wl, kTile * 4);
+            bulk_s2g(out.surface + tile_base, sm.surface, kTile * 4);
+            bulk_s2g(out.state + tile_base, sm.state, kTile);
+            bulk_s2g(out.bounces + tile_base, sm.bounces, kTile);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");      // shared memory must outlive the reads: the CTA ends after this
+        }
+        return;
+    }
     for (int k = threadIdx.x; k < 3 * m; k += kPktThreads) {
         __stcs(out.pos + 3 * tile_base + k, sm.o[k]);
         __stcs(out.dir + 3 * tile_base + k, sm.d[k]);
@@ -457,14 +506,7 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
         __stcs(out.pixel + tile_base + k, __float_as_int(sm.wl[k]));
         __stcs(out.surface + tile_base + k, sm.surface[k]);
     }
-    if ((reinterpret_cast<uintptr_t>(out.state) & 3) == 0 && (reinterpret_cast<uintptr_t>(out.bounces) & 3) == 0 && (m & 3) == 0) {
-        for (int k = threadIdx.x; k < m / 4; k += kPktThreads) {      // tile_base is a multiple of 4
-            __stcs(reinterpret_cast<uint32_t*>(out.state + tile_base) + k, reinterpret_cast<const uint32_t*>(sm.state)[k]);
-            __stcs(reinterpret_cast<uint32_t*>(out.bounces + tile_base) + k, reinterpret_cast<const uint32_t*>(sm.bounces)[k]);
-        }
-    } else {
-        for (int k = threadIdx.x; k < m; k += kPktThreads) { out.state[tile_base + k] = sm.state[k]; out.bounces[tile_base + k] = sm.bounces[k]; }
-    }
+    for (int k = threadIdx.x; k < m; k += kPktThreads) { out.state[tile_base + k] = sm.state[k]; out.bounces[tile_base + k] = sm.bounces[k]; }
 }
 
 }  // namespace
