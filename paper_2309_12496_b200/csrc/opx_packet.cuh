@@ -73,13 +73,19 @@ __device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity) {
                  "OPX_DONE_%=:\n"
                  "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, void* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(__cvta_generic_to_global(src)), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+// Photon inputs and records are touched once: an evict-first L2 policy keeps them from pushing the BVH out of L2.
+__device__ __forceinline__ uint64_t l2_evict_first() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
 }
-__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-                 ::"l"(__cvta_generic_to_global(dst)), "r"(smem_u32(src)), "r"(bytes) : "memory");
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, void* bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 ::"r"(smem_u32(dst)), "l"(__cvta_generic_to_global(src)), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes, uint64_t pol) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+                 ::"l"(__cvta_generic_to_global(dst)), "r"(smem_u32(src)), "r"(bytes), "l"(pol) : "memory");
 }
 __device__ __forceinline__ bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
@@ -260,10 +266,11 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
         if (threadIdx.x == 0) mbar_init(&sm.mbar, 1);
         __syncthreads();
         if (threadIdx.x == 0) {
+            const uint64_t pol = l2_evict_first();
             mbar_expect_tx(&sm.mbar, (uint32_t)(kTile * 28));
-            bulk_g2s(sm.o, origins + 3 * tile_base, kTile * 12, &sm.mbar);
-            bulk_g2s(sm.d, dirs + 3 * tile_base, kTile * 12, &sm.mbar);
-            bulk_g2s(sm.wl, wl + tile_base, kTile * 4, &sm.mbar);
+            bulk_g2s(sm.o, origins + 3 * tile_base, kTile * 12, &sm.mbar, pol);
+            bulk_g2s(sm.d, dirs + 3 * tile_base, kTile * 12, &sm.mbar, pol);
+            bulk_g2s(sm.wl, wl + tile_base, kTile * 4, &sm.mbar, pol);
         }
         mbar_wait(&sm.mbar, 0);
     } else {
@@ -487,12 +494,13 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // this thread's record writes -> visible to the TMA engine
         __syncthreads();
         if (threadIdx.x == 0) {
-            bulk_s2g(out.pos + 3 * tile_base, sm.o, kTile * 12);
-            bulk_s2g(out.dir + 3 * tile_base, sm.d, kTile * 12);
-            bulk_s2g(out.pixel + tile_base, sm.wl, kTile * 4);
-            bulk_s2g(out.surface + tile_base, sm.surface, kTile * 4);
-            bulk_s2g(out.state + tile_base, sm.state, kTile);
-            bulk_s2g(out.bounces + tile_base, sm.bounces, kTile);
+            const uint64_t pol = l2_evict_first();
+            bulk_s2g(out.pos + 3 * tile_base, sm.o, kTile * 12, pol);
+            bulk_s2g(out.dir + 3 * tile_base, sm.d, kTile * 12, pol);
+            bulk_s2g(out.pixel + tile_base, sm.wl, kTile * 4, pol);
+            bulk_s2g(out.surface + tile_base, sm.surface, kTile * 4, pol);
+            bulk_s2g(out.state + tile_base, sm.state, kTile, pol);
+            bulk_s2g(out.bounces + tile_base, sm.bounces, kTile, pol);
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
             asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");      // shared memory must outlive the reads: the CTA ends after this
         }
