@@ -502,7 +502,7 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
             bulk_s2g(out.state + tile_base, sm.state, kTile, pol);
             bulk_s2g(out.bounces + tile_base, sm.bounces, kTile, pol);
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-            asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");      // shared memory must outlive the reads: the CTA ends after this
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); // shared memory must outlive the reads: the CTA ends after this
         }
         return;
     }
