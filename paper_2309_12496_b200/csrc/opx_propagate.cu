@@ -29,16 +29,18 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
         using Big = PacketSmemT<512, 4>;
         using Small = PacketSmemT<512, 1>;
         // a filtered stream (NO_EFFICIENCY: 1 photon in 7-9 survives, so packets are wide and walk more nodes) on a large
-        // scene runs 14 % faster with 3 CTAs of 384 threads per SM (36 warps at 56 registers) than with 2 x 512 (32 warps
-        // at 64); everything else is faster with 2 x 512 (C4 in flight -3 %, toy-scene pipeline -23 % with 384 x 3)
-        using Mid = PacketSmemT<384, 4>;
+        // scene runs 22 % faster with 4 CTAs of 256 threads per SM (1024-photon tiles) than with 2 x 512: its packets differ
+        // widely in cost, and a tile's warps wait at its barrier for the slowest packet, so finer tiles waste fewer warp
+        // slots (384 x 3: +14 %, 128 x 8: -15 %); everything else is faster with 2 x 512 (more photons per ring in a tile:
+        // C4 in flight -10 %, toy-scene pipeline -23 % with the finer shapes)
+        using Mid = PacketSmemT<256, 4>;
         static bool configured = false;
         if (!configured) {
             cudaError_t e = cudaSuccess;
             if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
             if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
             if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 1, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Small));
-            if (!e) e = cudaFuncSetAttribute(k_propagate_packet<384, 4, 3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Mid));
+            if (!e) e = cudaFuncSetAttribute(k_propagate_packet<256, 4, 4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Mid));
             if (opx_status st = check_cuda(e, "cudaFuncSetAttribute")) return st;
             configured = true;
         }
@@ -48,7 +50,7 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
         const uint64_t tiles = (n + tile - 1) / tile;
         if (tiles > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
         if (packet_stats) k_propagate_packet<512, 4, 2, true><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr, nullptr, (unsigned long long*)packet_stats);
-        else if (mid) k_propagate_packet<384, 4, 3, false><<<(unsigned)tiles, 384, sizeof(Mid), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
+        else if (mid) k_propagate_packet<256, 4, 4, false><<<(unsigned)tiles, 256, sizeof(Mid), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
         else if (small) k_propagate_packet<512, 1, 2, false><<<(unsigned)tiles, 512, sizeof(Small), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
         else k_propagate_packet<512, 4, 2, false><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
         binned = !packet_stats;
