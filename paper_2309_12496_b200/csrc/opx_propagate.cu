@@ -34,22 +34,29 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
         // slots (384 x 3: +14 %, 128 x 8: -15 %); everything else is faster with 2 x 512 (more photons per ring in a tile:
         // C4 in flight -10 %, toy-scene pipeline -23 % with the finer shapes)
         using Mid = PacketSmemT<256, 4>;
+        // a small scene (its BVH lives in L1/L2: the walk is issue-bound, not latency-bound) traced in flight runs 3 % faster
+        // with 448 threads x 2 CTAs, which leaves 72 registers per thread and removes the spills of the 64-register build
+        // (C4 scene: -3.5 %, filtered toy-scene stream: -5 %, so those keep 512 x 2)
+        using Lean = PacketSmemT<448, 4>;
         static bool configured = false;
         if (!configured) {
             cudaError_t e = cudaSuccess;
             if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
             if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
             if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 1, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Small));
+            if (!e) e = cudaFuncSetAttribute(k_propagate_packet<448, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Lean));
             if (!e) e = cudaFuncSetAttribute(k_propagate_packet<256, 4, 4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Mid));
             if (opx_status st = check_cuda(e, "cudaFuncSetAttribute")) return st;
             configured = true;
         }
         const bool small = !packet_stats && n < (uint64_t)Big::kTile * 148;
         const bool mid = !packet_stats && !small && s.dev.n_tri >= (1u << 18) && (flags & OPX_FLAG_NO_EFFICIENCY);
-        const uint64_t tile = small ? Small::kTile : (mid ? Mid::kTile : Big::kTile);
+        const bool lean = !packet_stats && !small && s.dev.n_tri < (1u << 18) && !(flags & OPX_FLAG_NO_EFFICIENCY);
+        const uint64_t tile = small ? Small::kTile : (mid ? Mid::kTile : (lean ? Lean::kTile : Big::kTile));
         const uint64_t tiles = (n + tile - 1) / tile;
         if (tiles > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
         if (packet_stats) k_propagate_packet<512, 4, 2, true><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr, nullptr, (unsigned long long*)packet_stats);
+        else if (lean) k_propagate_packet<448, 4, 2, false><<<(unsigned)tiles, 448, sizeof(Lean), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
         else if (mid) k_propagate_packet<256, 4, 4, false><<<(unsigned)tiles, 256, sizeof(Mid), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
         else if (small) k_propagate_packet<512, 1, 2, false><<<(unsigned)tiles, 512, sizeof(Small), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
         else k_propagate_packet<512, 4, 2, false><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);

@@ -282,8 +282,19 @@ def test_large_scene_filtered_stream_kernel_shape_equals_small_calls(lhcb):
         assert np.array_equal(np.concatenate([p[k] for p in parts]), one[k]), k
     assert np.array_equal(parts[-1]["hitmap"], one["hitmap"]) and np.array_equal(parts[-1]["counters"], one["counters"])
     assert int(one["counters"][:7].sum()) == n and not np.isin(one["state"], [1, 3]).any()
-    # and against the oracle on a sample of the one-call result
+    # the same in flight: one call takes the 512-thread shape with 2048-photon tiles, the halves the small-call shape
+    one_f = _host(gs.propagate(do, dd, dl, seed=3, photon_id_base=5_000_000))
+    hm, ct = gs.alloc_accumulators()
+    parts = [_host(gs.propagate(do[a:b].contiguous(), dd[a:b].contiguous(), dl[a:b].contiguous(), seed=3,
+                                photon_id_base=5_000_000 + a, hitmap=hm, counters=ct)) for a, b in ((0, h), (h, n))]
+    for k in ("state", "pixel", "surface", "bounces", "pos", "dir"):
+        assert np.array_equal(np.concatenate([p[k] for p in parts]), one_f[k]), k
+    assert np.array_equal(parts[-1]["hitmap"], one_f["hitmap"]) and np.array_equal(parts[-1]["counters"], one_f["counters"])
+    # and against the oracle on a sample of the one-call results
     idx = np.arange(0, n, 400)
+    ref_f = oracle.trace_mesh(sc, o[idx], d[idx], lam[idx], seed=3, ids=(5_000_000 + idx).astype(np.uint64))
+    for k in REC:
+        assert np.array_equal(one_f[k][idx], ref_f[k]), k
     ref = oracle.trace_mesh(sc, o[idx], d[idx], lam[idx], flags=oracle.NO_EFFICIENCY)
     for k in REC:
         assert np.array_equal(one[k][idx], ref[k]), k
