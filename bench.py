@@ -32,7 +32,7 @@ FLOP_NODE, FLOP_TRI, FLOP_SEGMENT, FLOP_INTERACTION = 48, 50, 15, 35
 BYTES_IN, BYTES_OUT, BYTES_BIN = 28, 34, 6          # per photon: inputs, hit record, re-read by k_bin
 # dram__bytes_read.sum + dram__bytes_write.sum of k_propagate per launch from the ncu --set full
 # capture summarised in profiles/ (None until one exists for the current kernel)
-NCU_TRAFFIC_BYTES = {"C2": 570140416}   # profiles/r01_v23_k_propagate_packet.md
+NCU_TRAFFIC_BYTES = {"C2": 567209728}   # profiles/r01_v27_k_propagate_packet.md
 
 
 def measured_peaks():
