@@ -271,8 +271,10 @@ opx_status opx_propagate_host_workspace_bytes(const opx_scene* scene, uint64_t c
 /* End-to-end form with HOST buffers (pinned memory recommended): origins, dirs, wavelengths and the
  * six record arrays of `out` are host pointers of length n; h_hitmap (n_pixels, +=) and h_counters
  * (8, +=, may be NULL) are host arrays.  Photons are streamed through the caller's device workspace
- * in chunks of `chunk` photons, copies of one chunk overlapping the kernels of the other on two
- * internal-order streams forked from `cuda_stream`.  Synchronises `cuda_stream` before returning. */
+ * in chunks of at most `chunk` photons (the first and last few are smaller, to shorten the part of the
+ * pipeline that cannot overlap), the upload of one chunk, the kernel of the next and the download of a
+ * third overlapping on three internal streams forked from and joined into `cuda_stream`.  Synchronises
+ * `cuda_stream` before returning.  DESIGN.md 8.5. */
 opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,
                               const float* h_origins, const float* h_dirs, const float* h_wavelengths,
                               uint64_t seed, const opx_hits* h_out, uint32_t* h_hitmap,
