@@ -140,6 +140,7 @@ opx_status opx_scene_create(const opx_scene_params* params, const opx_mesh* mesh
     }
     s->normals.resize(total * 3);
     for (uint64_t t = 0; t < total; ++t) face_normal(&s->tri[9 * t], &s->normals[3 * t]);
+    compute_scene_stats(*s);
     compute_layout(*s, &s->layout, nullptr);
     *out = s;
     return OPX_OK;

@@ -393,6 +393,32 @@ void compute_layout(const SceneHost& s, opx_scene_layout* lay, size_t* tmp_bytes
     }
 }
 
+// Scene constants the build needs, computed once when the scene is created (host only).
+void compute_scene_stats(SceneHost& s) {
+    const size_t T = s.tri_surface.size();
+    // padding of the leaf boxes: 2^-16 of the largest |coordinate| (>= 128 ulp there), at least 1e-6
+    float maxabs = 0.f;
+    for (float v : s.tri) { const float a = std::fabs(v); if (a > maxabs) maxabs = a; }
+    s.leaf_pad = fmaxf(maxabs * (1.0f / 65536.0f), 1e-6f);
+    // typical triangle size (log-mean of the largest AABB extent) and scene extent: a beam much wider
+    // than the triangles it meets gains nothing over per-ray box tests
+    double logsum = 0.0;
+    float slo[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, shi[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
+    for (size_t t = 0; t < T; ++t) {
+        const float* v = &s.tri[9 * t];
+        float ext = 0.f;
+        for (int c = 0; c < 3; ++c) {
+            const float lo = std::fmin(v[c], std::fmin(v[3 + c], v[6 + c])), hi = std::fmax(v[c], std::fmax(v[3 + c], v[6 + c]));
+            ext = std::fmax(ext, hi - lo);
+            slo[c] = std::fmin(slo[c], lo); shi[c] = std::fmax(shi[c], hi);
+        }
+        logsum += std::log2((double)std::fmax(ext, 1e-20f));
+    }
+    s.tri_size = T ? (float)std::exp2(logsum / (double)T) : 0.f;
+    s.scene_ext = T ? std::fmax(shi[0] - slo[0], std::fmax(shi[1] - slo[1], shi[2] - slo[2])) : 0.f;
+
+}
+
 opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_t stream) {
     const size_t T = s.tri_surface.size();
     const opx_scene_layout& lay = s.layout;
@@ -430,26 +456,7 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
         (e = up(ws + lay.vertex_normals, s.tri_vnormals.data(), s.tri_vnormals.size() * 4)))
         return check_cuda(e, "scene upload");
 
-    // padding of the leaf boxes: 2^-16 of the largest |coordinate| (>= 128 ulp there), at least 1e-6
-    float maxabs = 0.f;
-    for (float v : s.tri) { const float a = std::fabs(v); if (a > maxabs) maxabs = a; }
-    const float pad = fmaxf(maxabs * (1.0f / 65536.0f), 1e-6f);
-    // typical triangle size (log-mean of the largest AABB extent) and scene extent: a beam much wider
-    // than the triangles it meets gains nothing over per-ray box tests
-    double logsum = 0.0;
-    float slo[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, shi[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
-    for (size_t t = 0; t < T; ++t) {
-        const float* v = &s.tri[9 * t];
-        float ext = 0.f;
-        for (int c = 0; c < 3; ++c) {
-            const float lo = std::fmin(v[c], std::fmin(v[3 + c], v[6 + c])), hi = std::fmax(v[c], std::fmax(v[3 + c], v[6 + c]));
-            ext = std::fmax(ext, hi - lo);
-            slo[c] = std::fmin(slo[c], lo); shi[c] = std::fmax(shi[c], hi);
-        }
-        logsum += std::log2((double)std::fmax(ext, 1e-20f));
-    }
-    const float tri_size = T ? (float)std::exp2(logsum / (double)T) : 0.f;
-    const float scene_ext = T ? std::fmax(shi[0] - slo[0], std::fmax(shi[1] - slo[1], shi[2] - slo[2])) : 0.f;
+    const float pad = s.leaf_pad, tri_size = s.tri_size, scene_ext = s.scene_ext;      // scene constants (compute_scene_stats)
 
     const int Ti = (int)T;
     uint32_t n_wide = 0;

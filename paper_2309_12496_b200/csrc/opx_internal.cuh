@@ -68,6 +68,7 @@ struct SceneHost {
     std::vector<FrameDev> frames;
     uint64_t n_pixels = 0;
     float inv_dlambda = 0.f, inv_bin = 0.f;
+    float leaf_pad = 1e-6f, tri_size = 0.f, scene_ext = 0.f;   // compute_scene_stats: box padding, typical triangle size, extent
     // set by opx_bvh_build
     bool built = false;
     void* d_scene_ws = nullptr;
@@ -87,6 +88,7 @@ void count_launch(uint64_t n = 1);
 
 // build (opx_build.cu)
 void compute_layout(const SceneHost& s, opx_scene_layout* lay, size_t* tmp_bytes);
+void compute_scene_stats(SceneHost& s);
 opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_t stream);
 
 // propagate (opx_propagate.cu)
