@@ -24,8 +24,7 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
         if (blocks > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
         k_propagate_lane<true, false><<<(unsigned)blocks, 128, 0, stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr);
     } else {
-        // tile size: 2048 photons (4 packets per warp) unless the call is too small to give every SM one such tile; then
-        // 512 photons (1 packet per warp: four times the CTAs, a quarter of the latency)
+        // tile size: 2048 photons (4 packets per warp) unless the call is small; then 512 photons (1 packet per warp)
         using Big = PacketSmemT<512, 4>;
         using Small = PacketSmemT<512, 1>;
         // a filtered stream (NO_EFFICIENCY: 1 photon in 7-9 survives, so packets are wide and walk more nodes) on a large
@@ -49,7 +48,10 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
             if (opx_status st = check_cuda(e, "cudaFuncSetAttribute")) return st;
             configured = true;
         }
-        const bool small = !packet_stats && n < (uint64_t)Big::kTile * 148;
+        // measured crossover (kernel time vs n, both tile sizes): on a small scene the 512-photon tiles win while they
+        // number at most one per SM (n < 148 x 512), on a large scene (longer, latency-bound packets) up to about 2e5 photons
+        const uint64_t small_below = s.dev.n_tri < (1u << 18) ? 148ull * Small::kTile : 100ull * Big::kTile;
+        const bool small = !packet_stats && n < small_below;
         const bool mid = !packet_stats && !small && s.dev.n_tri >= (1u << 18) && (flags & OPX_FLAG_NO_EFFICIENCY);
         const bool lean = !packet_stats && !small && s.dev.n_tri < (1u << 18) && !(flags & OPX_FLAG_NO_EFFICIENCY);
         const uint64_t tile = small ? Small::kTile : (mid ? Mid::kTile : (lean ? Lean::kTile : Big::kTile));

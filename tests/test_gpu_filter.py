@@ -265,7 +265,7 @@ def test_filter_error_paths(toy):
 
 
 def test_large_scene_filtered_stream_kernel_shape_equals_small_calls(lhcb):
-    """On a large scene a NO_EFFICIENCY call of >= 148 large tiles runs the 256-thread kernel shape (1024-photon tiles), smaller calls the
+    """On a large scene a NO_EFFICIENCY call of >= 204 800 photons runs the 256-thread kernel shape (1024-photon tiles), smaller calls the
     512-photon-tile shape (which test_filter_then_trace_matches_oracle_c4 pins to the oracle on this scene): the same
     400 000 photons through one call and through two calls must give identical records, hit-maps and counters."""
     sc, gs = lhcb

@@ -102,7 +102,7 @@ def test_c2_c3_sampled_parity(toy, name, stride, seed):
 
 
 def test_both_cta_shapes_against_the_oracle(toy):
-    """opx_propagate picks 512-photon tiles (one packet per warp) for calls below 148 large tiles and large tiles (on this
+    """opx_propagate picks 512-photon tiles (one packet per warp) for small calls (on this scene: below 75 776 photons) and large tiles (on this
     small scene, in flight: 448 threads x 4 photons) above: 620 000 contiguous C3 photons take the large tiles, their
     first 50 000 alone the small ones; both must reproduce the oracle, hence each other, bit for bit.  (The 512-thread
     shape is pinned by test_no_efficiency_trace_at_scale on this scene and by tests/test_gpu_filter.py on the large one.)"""
