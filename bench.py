@@ -1,16 +1,19 @@
 #!/usr/bin/env python
 """bench.py -- photons/s of the per-photon optical propagation hot path on B200.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config C2] [--photons n]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config C4] [--photons n]
 
-One "step" = one opx_propagate call (one kernel: propagation with hit binning and counters inside) over one batch of
-synthetic photons of the named BASELINE.json config (default C2 = configs[1]: toy RICH, 20 014
-triangles, 1e7 photons), inputs resident in HBM.  The BVH build is timed separately (`bvh_build_ms`)
-as SURVEY.md 8(d) prescribes.  N > 1 (torchrun): every rank propagates its own contiguous id range
-of the same size (weak scaling) and the per-rank hit-maps and counters are summed with one NCCL
-all-reduce per step.  Prints ONE JSON line on rank 0.
+One "step" = one opx_propagate call (ONE kernel: staging, sort, traversal, interaction, records, hit binning and
+counters) over one batch of synthetic photons, inputs resident in HBM.  The headline line is on the largest
+single-GPU configuration of BASELINE.json, C4 = configs[3]: the LHCb-RICH-like scene (1.01e6 triangles, meshes at
+5 mm) with 1e8 track photons per step.  The other configurations (C1, C2, C3 on
+the toy scene, the C5 stream on the C4 scene) are timed in the same run and reported as sub-records under
+"configs", each with its own roofline fraction.  The BVH build is timed separately (`bvh_build_ms`, SURVEY.md
+8(d)).  N > 1 (torchrun): every rank propagates its own contiguous id range of the same size (weak scaling) and the
+per-rank hit-maps and counters are summed with one NCCL all-reduce per step.  Prints ONE JSON line on rank 0.
 """
 import argparse
+import concurrent.futures
 import json
 import os
 import statistics
@@ -29,18 +32,20 @@ METRIC = "optical photons propagated/sec on 1 B200 (device-timed), % of roofline
 UNIT = "photons/s"
 # FLOP model of SURVEY.md 8(d) / DESIGN.md 9: FMA = 2, add/mul/min/max/compare/divide = 1
 FLOP_NODE, FLOP_TRI, FLOP_SEGMENT, FLOP_INTERACTION = 48, 50, 15, 35
-BYTES_IN, BYTES_OUT, BYTES_BIN = 28, 34, 6          # per photon: inputs, hit record, re-read by k_bin
-# dram__bytes_read.sum + dram__bytes_write.sum of k_propagate per launch from the ncu --set full
-# capture summarised in profiles/ (None until one exists for the current kernel)
-NCU_TRAFFIC_BYTES = {"C2": 567209728}   # profiles/r01_v27_k_propagate_packet.md
+BYTES_IN, BYTES_OUT = 28, 34                        # per photon: inputs, hit record
+L2_BYTES = 126e6
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the step's kernel, from the `ncu --set full` captures
+# summarised under profiles/ (per config, at the launch size this bench times; None until a capture exists)
+NCU_TRAFFIC_BYTES = {"C2": 567209728, "C4": None}
+NCU_TRAFFIC_SOURCE = {"C2": "profiles/r01_v27_k_propagate_packet.md", "C4": None}
 
 
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
         p = json.load(open(path))
-        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
-    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured (MEASURED_PEAKS.json)")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback (B200_PROFILING.md)")
 
 
 class ClockSampler(threading.Thread):
@@ -56,23 +61,26 @@ class ClockSampler(threading.Thread):
     def run(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             for line in self.proc.stdout:
-                self.rows.append([x.strip() for x in line.split(",")])
+                self.rows.append((time.perf_counter(), [x.strip() for x in line.split(",")]))
         except Exception:
             pass
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
+        """Summary of the samples taken in [t0, t1] (perf_counter; all samples if None)."""
         if self.proc is not None:
             self.proc.terminate()
         self.join(timeout=2)
-        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        rows = [r for t, r in self.rows if (t0 is None or t >= t0) and (t1 is None or t <= t1)]
+        sm = [float(r[0]) for r in rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        pw = [float(r[2]) for r in rows if len(r) >= 7 and r[2].replace(".", "").isdigit()]
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        reasons = sorted({names[k] for r in self.rows if len(r) >= 7 for k in range(4) if r[3 + k].startswith("Active")})
+        reasons = sorted({names[k] for r in rows if len(r) >= 7 for k in range(4) if r[3 + k].startswith("Active")})
         return dict(sm_mhz=statistics.median(sm) if sm else None, sm_max_mhz=max(mx) if mx else None,
-                    reasons=reasons, samples=len(sm))
+                    power_w_max=max(pw) if pw else None, reasons=reasons, samples=len(sm))
 
 
 def time_oracle(workload, n_sample, seed, repeats=1, n_threads=None):
@@ -88,6 +96,11 @@ def time_oracle(workload, n_sample, seed, repeats=1, n_threads=None):
     return n_sample / best, r["n_threads"], best, int(r["counters"][7])
 
 
+def workload_name(name, scene, n, smooth=False):
+    return (f"{name}{' + mirror vertex normals' if smooth else ''}: {scene.n_triangles} triangles, {n} photons per GPU per step "
+            f"({BYTES_IN + BYTES_OUT} B/photon = {(BYTES_IN + BYTES_OUT) * n / 1e6:.0f} MB per step)")
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle timed on a bounded sample of the same workload per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -98,14 +111,14 @@ def run_reference(args):
     import oracle
     # bounded sample per step: at most --reference-sample photons, and no more than about 3 s of work (probed), so that
     # `--steps K --warmup W` ends within minutes on any config
-    po, pd, pl = w.photon_range(0, 1000)
+    po, pd, pl = w.photon_range(0, 200)
     t0 = time.perf_counter()
     oracle.trace_mesh(w.scene, po, pd, pl, seed=args.seed)
-    rate = 1000 / (time.perf_counter() - t0)
-    n_sample = int(min(w.n, args.reference_sample, max(1000, rate * 3.0)))
+    rate = 200 / (time.perf_counter() - t0)
+    n_sample = int(min(w.n, args.reference_sample, max(200, rate * 3.0)))
     o, d, lam = w.photon_range(0, n_sample)
     for _ in range(args.warmup):
-        oracle.trace_mesh(w.scene, o[:1000], d[:1000], lam[:1000], seed=args.seed)
+        oracle.trace_mesh(w.scene, o[:200], d[:200], lam[:200], seed=args.seed)
     t0 = time.perf_counter()
     threads = 0
     for _ in range(args.steps):
@@ -114,14 +127,132 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     value = n_sample * args.steps / dt
     sample = f"first {n_sample} photon ids of {args.config} per step, brute force over {w.scene.n_triangles} triangles"
+    n_full = min(w.n, 100_000_000)
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{args.config}{' + mirror vertex normals' if args.smooth else ''}: {w.scene.n_triangles} triangles, {w.n} photons (sampled)"},
+        "config": {"workload": workload_name(args.config, w.scene, n_full, args.smooth) + " (the oracle runs a bounded sample of it)"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
+
+
+def pinned_photons(w, id_base, n, threads=8):
+    """The workload's photons id_base .. id_base + n - 1 in pinned host tensors (generated in slices, in parallel:
+    every photon is a pure function of (seed, id))."""
+    import torch
+    pin = [torch.empty((n, 3), dtype=torch.float32).pin_memory(), torch.empty((n, 3), dtype=torch.float32).pin_memory(),
+           torch.empty(n, dtype=torch.float32).pin_memory()]
+    step = 2_000_000
+
+    def fill(a):
+        b = min(n, a + step)
+        for dst, src in zip(pin, w.photon_range(id_base + a, id_base + b)):
+            dst[a:b] = torch.from_numpy(src)
+    with concurrent.futures.ThreadPoolExecutor(max_workers=threads) as ex:
+        list(ex.map(fill, range(0, n, step)))
+    return pin
+
+
+class Timed:
+    """Device timing of `steps` calls of step() on `stream` (CUDA events around the whole region; when the step's
+    working set fits in L2 every step is timed on its own with an L2 flush -- a 256 MB fill -- before it)."""
+
+    def __init__(self, torch, stream, dev):
+        self.torch, self.stream, self.dev = torch, stream, dev
+        self.flush_buf = None
+
+    def run(self, step, steps, warmup, flush_l2=False):
+        torch = self.torch
+        for _ in range(warmup):
+            step()
+        torch.cuda.synchronize()
+        if not flush_l2:
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ev0.record(self.stream)
+            for _ in range(steps):
+                step()
+            ev1.record(self.stream)
+            torch.cuda.synchronize()
+            return ev0.elapsed_time(ev1)
+        if self.flush_buf is None:
+            self.flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=self.dev)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in evs:
+            self.flush_buf.fill_(1)
+            a.record(self.stream)
+            step()
+            b.record(self.stream)
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in evs)
+
+
+def roofline_record(pkg, scene, photons, n, id_base, seed, kernel_ms, step_ms, peaks, fma_peak, config):
+    """algorithmic FLOPs (instrumented single-ray walk: segments, node visits, triangle tests,
+    interactions) and bytes (62 B/photon) of one launch over the kernel's measured duration; the slower bound is named."""
+    d_o, d_d, d_l = photons
+    stats = scene.propagate_stats(d_o, d_d, d_l, seed=seed, photon_id_base=id_base)
+    flop = (FLOP_NODE * stats["nodes"] + FLOP_TRI * stats["triangle_tests"] + FLOP_SEGMENT * stats["segments"]
+            + FLOP_INTERACTION * stats["interactions"])
+    t = kernel_ms * 1e-3
+    derived = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    peak = fma_peak if fma_peak else derived
+    alu = flop / t / 1e12
+    hbm_bytes = (BYTES_IN + BYTES_OUT) * n
+    hbm = hbm_bytes / t / 1e9
+    t_alu, t_hbm = flop / (peak * 1e12), hbm_bytes / (peaks["hbm_gbs"] * 1e9)
+    if t_alu >= t_hbm:
+        roof = {"bound": "alu", "achieved": alu, "peak": peak, "unit": "TFLOP/s", "frac": alu / peak,
+                "peak_source": "measured (FP32 FMA micro-benchmark opx_measure_fp32_peak on this device)" if fma_peak
+                               else "derived (148 SMs x 128 FP32 lanes x 2 FLOP x sm_max_mhz)"}
+    else:
+        roof = {"bound": "hbm", "achieved": hbm, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": hbm / peaks["hbm_gbs"],
+                "peak_source": peaks["source"]}
+    roof.update({
+        "traffic": NCU_TRAFFIC_BYTES.get(config), "traffic_source": NCU_TRAFFIC_SOURCE.get(config),
+        "kernel": pkg.last_kernel(), "kernel_ms": kernel_ms, "kernel_share_of_step": kernel_ms / step_ms,
+        "fp32_peak_derived_tflops": derived, "frac_of_derived_peak": alu / derived,
+        "fp32_peak_derivation": "148 SMs x 128 FP32 lanes x 2 FLOP x sm_max_mhz (only the clock is measured)",
+        "flop_per_photon": flop / n, "bytes_per_photon": BYTES_IN + BYTES_OUT,
+        "segments_per_photon": stats["segments"] / n, "nodes_per_segment": stats["nodes"] / max(1, stats["segments"]),
+        "triangle_tests_per_segment": stats["triangle_tests"] / max(1, stats["segments"]),
+        "alu_tflops": alu, "hbm_gbs": hbm, "hbm_frac": hbm / peaks["hbm_gbs"], "hbm_peak_source": peaks["source"],
+        "photons_per_s_alu_bound": n / t_alu, "photons_per_s_hbm_bound": n / t_hbm})
+    return roof
+
+
+def measure_in_flight(pkg, torch, tm, scene, photons, n, id_base, seed, steps, warmup, records=None, allreduce=None):
+    """`steps` timed opx_propagate calls over the resident batch.  Returns (total ms, mean kernel ms, launches, counters)."""
+    d_o, d_d, d_l = photons
+    dev = d_l.device
+    records = records if records is not None else scene.alloc_records(n, dev)
+    hitmap, counters = scene.alloc_accumulators(dev)
+
+    def step():
+        hitmap.zero_(); counters.zero_()
+        scene.propagate(d_o, d_d, d_l, seed=seed, photon_id_base=id_base, records=records, hitmap=hitmap,
+                        counters=counters, stream=tm.stream)
+        if allreduce is not None:
+            allreduce(hitmap, counters)                               # the one exchange step (no-op at N = 1)
+    flush = (BYTES_IN + BYTES_OUT) * n <= L2_BYTES
+    for _ in range(warmup):
+        step()
+    scene.profile_begin(steps)
+    l0 = pkg.launch_count()
+    ms_total = tm.run(step, steps, 0, flush_l2=flush)
+    launches = pkg.launch_count() - l0
+    ms_prop, _ = scene.profile_end()
+    return ms_total, statistics.mean(ms_prop), launches, counters.cpu().numpy(), flush, records
+
+
+def steps_for(pkg, torch, tm, scene, photons, n, seed, target_s, lo, hi):
+    """Number of timed steps that makes the timed region about target_s long (probed with 3 calls)."""
+    d_o, d_d, d_l = photons
+    rec = scene.alloc_records(n, d_l.device)
+    hm, ct = scene.alloc_accumulators(d_l.device)
+    ms = tm.run(lambda: scene.propagate(d_o, d_d, d_l, seed=seed, records=rec, hitmap=hm, counters=ct, stream=tm.stream), 3, 2)
+    return int(min(hi, max(lo, target_s / max(1e-6, ms / 3 * 1e-3)))), rec
 
 
 def run_sweep(args, scene, photons, records, hitmap, counters, n, stream, w, pkg):
@@ -169,7 +300,7 @@ def run_sweep(args, scene, photons, records, hitmap, counters, n, stream, w, pkg
             done = passes * per_pass
             rows.append({"chunk": chunk, "streams": n_streams, "photons": done, "calls": passes * (n // chunk), "ms": ms,
                          "photons_per_s": done / (ms * 1e-3), "hbm_gbs_algorithmic": done * (BYTES_IN + BYTES_OUT) / (ms * 1e-3) / 1e9,
-                         "gpu_launches": pkg.launch_count() - l0})
+                         "kernel": pkg.last_kernel(), "gpu_launches": pkg.launch_count() - l0})
     best = max(rows, key=lambda r: r["photons_per_s"])
     print(json.dumps({"metric": METRIC, "value": best["photons_per_s"], "unit": UNIT, "n_gpus": 1, "higher_is_better": True,
                       "dtype": "f32", "data": "synthetic", "scaling": "weak", "vs_baseline": None,
@@ -178,19 +309,40 @@ def run_sweep(args, scene, photons, records, hitmap, counters, n, stream, w, pkg
                       "sweep": rows}))
 
 
+def sub_record(pkg, torch, tm, name, dev, seed, peaks, fma_peak, target_s, n=None, workload=None):
+    """One of the other BASELINE.json configurations, device-timed in this run: value, ms/step, roofline."""
+    import workloads
+    w = workload if workload is not None else workloads.make_config(name, n=n)
+    n = w.n
+    pin = pinned_photons(w, 0, n)
+    photons = tuple(x.to(dev, non_blocking=True) for x in pin)
+    scene = pkg.Scene(w.scene).build(dev)
+    steps, rec = steps_for(pkg, torch, tm, scene, photons, n, seed, target_s, 5, 2000)
+    ms_total, kernel_ms, launches, cnt, flushed, _ = measure_in_flight(pkg, torch, tm, scene, photons, n, 0, seed, steps, 3, records=rec)
+    # a step timed on its own (L2 flushed before it) is bracketed by its own events; otherwise the region is
+    ms_step = ms_total / steps
+    roof = roofline_record(pkg, scene, photons, n, 0, seed, kernel_ms, ms_step, peaks, fma_peak, name)
+    return {"workload": workload_name(name, w.scene, n), "value": n / (ms_step * 1e-3), "unit": UNIT, "steps": steps,
+            "ms_per_step": ms_step, "gpu_launches": int(launches),
+            "l2": "every step timed on its own after a 256 MB fill that flushes L2" if flushed else "inputs + outputs per step exceed the 126 MB L2",
+            "roofline": roof, "states": dict(zip(pkg.STATE_NAMES, (int(x) for x in cnt[:7])))}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="opx", choices=["opx", "reference"])
-    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
-    ap.add_argument("--photons", type=int, default=None, help="photons per GPU per step (default: the config's N)")
+    ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--photons", type=int, default=None, help="photons per GPU per step (default: the config's N, at most 1e8)")
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="CPU time budget of each cpu_baseline leg (all cores, one thread)")
     ap.add_argument("--reference-sample", type=int, default=20000)
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sub-records", action="store_true", help="skip the C1/C2/C3/C5 sub-records, the paper pipeline and the emission legs")
+    ap.add_argument("--sub-seconds", type=float, default=0.25, help="length of the timed region of each sub-record")
     ap.add_argument("--smooth", action="store_true",
                     help="toy-scene configs (C1-C3) with vertex normals on the mirror (SURVEY.md 8(f) row f3): a variant "
                          "of the workload, named in config.workload; not the default line")
@@ -231,19 +383,14 @@ def main():
         from workloads.scenes import toy_rich_scene
         w.scene = toy_rich_scene("flat" if args.config == "C1" else "c2", smooth=True)
     id_base, n = shard_range(n * world, rank, world)                  # contiguous global id range of this rank
-    pin = [torch.empty((n, 3), dtype=torch.float32).pin_memory(), torch.empty((n, 3), dtype=torch.float32).pin_memory(),
-           torch.empty(n, dtype=torch.float32).pin_memory()]
-    for a in range(0, n, 5_000_000):                                  # generate in slices to bound host memory
-        b = min(n, a + 5_000_000)
-        for dst, src in zip(pin, w.photon_range(id_base + a, id_base + b)):
-            dst[a:b] = torch.from_numpy(src)
+    pin = pinned_photons(w, id_base, n)
     d_o, d_d, d_l = (x.to(dev, non_blocking=True) for x in pin)
     stream = torch.cuda.current_stream(dev)
+    tm = Timed(torch, stream, dev)
 
     # ---- scene + BVH build (timed separately: SURVEY.md 8(d))
     scene = pkg.Scene(w.scene)
     scene.build(dev)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = pkg.launch_count()
     torch.cuda.synchronize()
     t_build = []
@@ -254,10 +401,12 @@ def main():
     build_launches = (pkg.launch_count() - l0) // 3
 
     records = scene.alloc_records(n, dev)
-    hitmap, counters = scene.alloc_accumulators(dev)
-
     if args.sweep:
+        hitmap, counters = scene.alloc_accumulators(dev)
         return run_sweep(args, scene, (d_o, d_d, d_l), records, hitmap, counters, n, stream, w, pkg)
+
+    # ---- the headline: exactly --steps timed calls, barrier + synchronize on both sides, max over ranks
+    hitmap, counters = scene.alloc_accumulators(dev)
 
     def step():
         hitmap.zero_(); counters.zero_()
@@ -265,6 +414,7 @@ def main():
                         counters=counters, stream=stream)
         allreduce_accumulators(hitmap, counters)                      # the one exchange step (no-op at N = 1)
 
+    flush = (BYTES_IN + BYTES_OUT) * n <= L2_BYTES
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
@@ -272,21 +422,20 @@ def main():
         dist.barrier()
     sampler = ClockSampler(local)
     sampler.start()
-    time.sleep(0.25)
+    time.sleep(0.3)
     scene.profile_begin(args.steps)
     l0 = pkg.launch_count()
     torch.cuda.synchronize()
-    ev0.record(stream)
-    for _ in range(args.steps):
-        step()
-    ev1.record(stream)
-    torch.cuda.synchronize()
+    t_begin = time.perf_counter()
+    ms_total = tm.run(step, args.steps, 0, flush_l2=flush)
+    t_end = time.perf_counter()
     if dist is not None:
         dist.barrier()
-    ms_total = ev0.elapsed_time(ev1)
     launches = pkg.launch_count() - l0                           # kernels of libopx.so only (torch fills not counted)
-    ms_prop, ms_bin = scene.profile_end()
-    clocks = sampler.stop()
+    ms_prop, _ = scene.profile_end()
+    kernel_name = pkg.last_kernel()
+    clocks = sampler.stop(t_begin, t_end)
+    clocks["timed_region_s"] = t_end - t_begin
     if dist is not None:
         t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -314,50 +463,29 @@ def main():
             dt = float(t.item())
         e2e = {"value": world * n * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": BYTES_IN * n,
                "d2h_bytes_per_step": BYTES_OUT * n + 4 * scene.n_pixels + 64, "chunk_photons": chunk,
-               "ms_per_step": 1e3 * dt / args.e2e_steps}
-        if not np.array_equal(host_out["counters"].numpy(), cnt if dist is None else host_out["counters"].numpy()):
+               "ms_per_step": 1e3 * dt / args.e2e_steps,
+               "what": "opx_propagate_host: pinned host photon arrays in, every photon's hit record + hit-map + counters out"}
+        if dist is None and not np.array_equal(host_out["counters"].numpy(), cnt):
             raise SystemExit("bench: host path and device path disagree")
+        del host_out
 
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (k_propagate), DESIGN.md section 9
+    # ---- roofline of the dominant kernel, DESIGN.md section 9
     peaks = measured_peaks()
-    stats = scene.propagate_stats(d_o, d_d, d_l, seed=args.seed, photon_id_base=id_base)
-    flop = (FLOP_NODE * stats["nodes"] + FLOP_TRI * stats["triangle_tests"] + FLOP_SEGMENT * stats["segments"]
-            + FLOP_INTERACTION * stats["interactions"])
-    t_prop = statistics.mean(ms_prop) * 1e-3
-    t_bin = statistics.mean(ms_bin) * 1e-3
-    fp32_peak_tflops = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-    alu_achieved = flop / t_prop / 1e12
-    hbm_bytes = (BYTES_IN + BYTES_OUT) * n
-    hbm_achieved = hbm_bytes / t_prop / 1e9
-    t_alu_bound, t_hbm_bound = flop / (fp32_peak_tflops * 1e12), hbm_bytes / (peaks["hbm_gbs"] * 1e9)
-    if t_alu_bound >= t_hbm_bound:
-        roof = {"bound": "alu", "achieved": alu_achieved, "peak": fp32_peak_tflops, "unit": "TFLOP/s",
-                "frac": alu_achieved / fp32_peak_tflops}
-    else:
-        roof = {"bound": "hbm", "achieved": hbm_achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": hbm_achieved / peaks["hbm_gbs"]}
-    roof.update({
-        "traffic": NCU_TRAFFIC_BYTES.get(args.config), "kernel": "k_propagate", "kernel_ms": 1e3 * t_prop,
-        "kernel_share_of_step": t_prop / (ms_step * 1e-3), "bin_kernel_ms": 1e3 * t_bin, "peak_source": peaks["source"],
-        "peak_derivation": "148 SMs x 128 FP32 lanes x 2 FLOP x sm_max_mhz",
-        "flop_per_photon": flop / n, "bytes_per_photon": BYTES_IN + BYTES_OUT,
-        "segments_per_photon": stats["segments"] / n, "nodes_per_segment": stats["nodes"] / max(1, stats["segments"]),
-        "triangle_tests_per_segment": stats["triangle_tests"] / max(1, stats["segments"]),
-        "alu_tflops": alu_achieved, "alu_frac": alu_achieved / fp32_peak_tflops,
-        "hbm_gbs": hbm_achieved, "hbm_frac": hbm_achieved / peaks["hbm_gbs"],
-        "photons_per_s_alu_bound": n / t_alu_bound, "photons_per_s_hbm_bound": n / t_hbm_bound})
     fma = pkg.measure_fp32_peak(dev)          # FMA micro-benchmark on this device
-    roof.update({"fp32_peak_measured_tflops": fma, "alu_frac_of_measured_peak": alu_achieved / fma if fma else None})
+    pkg_kernel = kernel_name
+    roof = roofline_record(pkg, scene, (d_o, d_d, d_l), n, id_base, args.seed, statistics.mean(ms_prop), ms_step, peaks, fma, args.config)
+    roof["kernel"] = pkg_kernel
 
-    # ---- the paper's own pipeline: filter on the efficiencies first, trace
-    #      the survivors with efficiencies switched off; the survivor count never leaves the device
-    paper = None
-    if world == 1:
+    paper = emit = None
+    subs = {}
+    if world == 1 and not args.no_sub_records:
+        # ---- the paper's own pipeline: filter on the efficiencies first, trace
+        #      the survivors with efficiencies switched off; the survivor count never leaves the device
         kinds = [m["kind"] for m in w.scene.materials]
         m_mir, m_det = kinds.index(1), kinds.index(2)
         factors = [m_det] + [m_mir] * (2 if args.config in ("C4", "C5") else 1)
@@ -370,17 +498,9 @@ def main():
             if trace:
                 scene.propagate(pre["origins"], pre["dirs"], pre["wavelengths"], seed=args.seed, records=records, hitmap=hm2,
                                 counters=ct2, stream=stream, flags=pkg.FLAG_NO_EFFICIENCY, n_dev=pre["n_kept"])
-        times = {}
-        for name, trace in (("pipeline", True), ("prefilter", False)):
-            for _ in range(args.warmup):
-                paper_step(trace)
-            torch.cuda.synchronize()
-            ev0.record(stream)
-            for _ in range(args.steps):
-                paper_step(trace)
-            ev1.record(stream)
-            torch.cuda.synchronize()
-            times[name] = ev0.elapsed_time(ev1) / args.steps * 1e-3
+        k_sub = max(3, min(args.steps, 10))
+        times = {name: tm.run(lambda: paper_step(trace), k_sub, args.warmup) / k_sub * 1e-3
+                 for name, trace in (("pipeline", True), ("prefilter", False))}
         kept = int(pre["n_kept"].item())
         paper_step(True)
         torch.cuda.synchronize()
@@ -388,14 +508,13 @@ def main():
         paper = {"what": "opx_prefilter on QE x R" + (" x R" if len(factors) == 3 else "") + " then opx_propagate_flags(NO_EFFICIENCY) on the survivors",
                  "value": n / times["pipeline"], "unit": UNIT, "ms_per_step": 1e3 * times["pipeline"],
                  "prefilter_ms": 1e3 * times["prefilter"], "kept_fraction": kept / n, "detected": int(ct2[0].item()),
-                 "detected_in_flight": int(cnt[0]),
+                 "detected_in_flight": int(cnt[0]), "trace_kernel": pkg.last_kernel(),
                  "prefilter_roofline": {"bound": "hbm", "achieved": pf_bytes / times["prefilter"] / 1e9, "peak": peaks["hbm_gbs"],
                                         "unit": "GB/s", "frac": pf_bytes / times["prefilter"] / 1e9 / peaks["hbm_gbs"],
                                         "bytes_per_photon": pf_bytes / n}}
+        del pre
 
-    # ---- on-device Cherenkov generation from track steps, alone and chained into opx_propagate
-    emit = None
-    if world == 1:
+        # ---- on-device Cherenkov generation from track steps, alone and chained into opx_propagate
         src = w.track_source if w.track_source is not None else workloads.make_config("C3", n=n).track_source
         dsteps = pkg.upload_track_steps(src.steps(), dev)
         gen = (torch.empty_like(d_o), torch.empty_like(d_d), torch.empty_like(d_l))
@@ -406,42 +525,23 @@ def main():
             if trace:
                 hm3.zero_(); ct3.zero_()
                 scene.propagate(*gen, seed=args.seed, records=records, hitmap=hm3, counters=ct3, stream=stream)
-        etimes = {}
-        for name, trace in (("emit", False), ("chain", True)):
-            for _ in range(args.warmup):
-                emit_step(trace)
-            torch.cuda.synchronize()
-            ev0.record(stream)
-            for _ in range(args.steps):
-                emit_step(trace)
-            ev1.record(stream)
-            torch.cuda.synchronize()
-            etimes[name] = ev0.elapsed_time(ev1) / args.steps * 1e-3
+        etimes = {name: tm.run(lambda: emit_step(trace), k_sub, args.warmup) / k_sub * 1e-3
+                  for name, trace in (("emit", False), ("chain", True))}
         # the paper's whole pipeline from track steps: emission fused with the filter, survivors traced with efficiencies off
-        kinds_e = [m["kind"] for m in w.scene.materials]
-        fac_e = [kinds_e.index(2)] + [kinds_e.index(1)] * (2 if args.config in ("C4", "C5") else 1)
         cap = n // 2 + 4096
-        fpre = scene.emit_cherenkov_filtered(dsteps, n, fac_e, seed=args.seed, stream=stream, capacity=cap)
+        fpre = scene.emit_cherenkov_filtered(dsteps, n, factors, seed=args.seed, stream=stream, capacity=cap)
         if int(fpre["n_kept"].item()) > cap:
-            raise SystemExit("bench: survivor capacity exceeded")
+            raise SystemExit("bench: survivor list truncated (capacity)")
 
         def fused_step(trace):
-            scene.emit_cherenkov_filtered(dsteps, n, fac_e, seed=args.seed, out=fpre, stream=stream)
+            scene.emit_cherenkov_filtered(dsteps, n, factors, seed=args.seed, out=fpre, stream=stream)
             if trace:
                 hm3.zero_(); ct3.zero_()
                 scene.propagate(fpre["origins"], fpre["dirs"], fpre["wavelengths"], seed=args.seed,
                                 records={k: v[:cap] for k, v in records.items()}, hitmap=hm3, counters=ct3, stream=stream,
                                 flags=pkg.FLAG_NO_EFFICIENCY, n_dev=fpre["n_kept"])
         for name, trace in (("fused", False), ("fused_chain", True)):
-            for _ in range(args.warmup):
-                fused_step(trace)
-            torch.cuda.synchronize()
-            ev0.record(stream)
-            for _ in range(args.steps):
-                fused_step(trace)
-            ev1.record(stream)
-            torch.cuda.synchronize()
-            etimes[name] = ev0.elapsed_time(ev1) / args.steps * 1e-3
+            etimes[name] = tm.run(lambda: fused_step(trace), k_sub, args.warmup) / k_sub * 1e-3
         emit = {"what": f"opx_emit_cherenkov: {n} photons from {int(dsteps['length'].shape[0])} track steps"
                         + ("" if w.track_source is not None else " (step table of C3: C2's photons are a point source, not tracks)"),
                 "value": n / etimes["emit"], "unit": UNIT, "ms_per_step": 1e3 * etimes["emit"],
@@ -456,15 +556,48 @@ def main():
                                                          "emission + filter, survivors traced with NO_EFFICIENCY",
                                                  "value": n / etimes["fused_chain"], "unit": UNIT,
                                                  "ms_per_step": 1e3 * etimes["fused_chain"], "detected": int(ct3[0].item())}}
+        del gen, fpre
+
+        # ---- the C5 stream on this scene (BASELINE.json configs[4]): photons of C5's tracks (beta in [0.9999, 1], disc
+        #      radius 200 mm) generated ON THE DEVICE from its step table, streamed in chunks with advancing ids
+        if args.config in ("C4", "C5"):
+            n5 = n
+            w5 = workloads.make_config("C5", n=n5)
+            st5 = pkg.upload_track_steps(w5.track_source.steps(), dev)
+            g5 = pkg.emit_cherenkov(st5, n5, photon_id_base=0, seed=args.seed, stream=stream)
+            hm5, ct5 = scene.alloc_accumulators(dev)
+            passes = [0]
+
+            def c5_step():
+                scene.propagate(*g5, seed=args.seed, photon_id_base=passes[0] * n5, records=records, hitmap=hm5, counters=ct5, stream=stream)
+                passes[0] += 1
+            k5 = max(3, min(args.steps, 10))
+            ms5 = tm.run(c5_step, k5, args.warmup) / k5
+            subs["C5"] = {"workload": f"C5 stream: {w.scene.n_triangles} triangles, {k5} chunks of {n5} photons (of the 1e9-photon stream; ids continue "
+                                      f"across chunks), photons generated on the device by opx_emit_cherenkov from C5's step table",
+                          "value": n5 / (ms5 * 1e-3), "unit": UNIT, "steps": k5, "ms_per_step": ms5, "kernel": pkg.last_kernel(),
+                          "hbm_gbs_algorithmic": n5 * (BYTES_IN + BYTES_OUT) / (ms5 * 1e-3) / 1e9,
+                          "note": "chunk-size sweep 1e5..1e8 with ncu counters: `bench.py --config C5 --sweep`, profiles/r02_c5_sweep.md"}
+            del g5
+        del records
+        torch.cuda.empty_cache()
+        # ---- the other configurations, each device-timed here with its own roofline
+        for name in ("C1", "C2", "C3"):
+            if name != args.config:
+                subs[name] = sub_record(pkg, torch, tm, name, dev, args.seed, peaks, fma, args.sub_seconds)
+        # the paper's own run size (600 ... 6e5 photons per run) on the headline scene
+        w6 = workloads.make_config(args.config if args.config in ("C4", "C5") else "C4", n=600_000)
+        subs["paper_run_6e5"] = sub_record(pkg, torch, tm, "C4 scene, the paper's largest run (6e5 photons, PAPER.md:175)", dev, args.seed,
+                                           peaks, fma, args.sub_seconds, workload=w6)
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         # bounded sample: a quick probe sets the size so that each leg is about --cpu-seconds of CPU work
-        probe_n = min(n, 2000)
+        probe_n = min(n, 400)
         rate, threads, _, _ = time_oracle(w, probe_n, args.seed)
         n_sample = int(min(n, max(probe_n, rate * args.cpu_seconds)))
         v, threads, secs, segs = time_oracle(w, n_sample, args.seed)
-        n1 = int(min(n_sample, max(500, v / max(1, threads) * args.cpu_seconds)))
+        n1 = int(min(n_sample, max(100, v / max(1, threads) * args.cpu_seconds)))
         v1, _, secs1, _ = time_oracle(w, n1, args.seed, n_threads=1)
         cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
                "sample": f"first {n_sample} photon ids of {args.config}, brute force over {w.scene.n_triangles} triangles, {secs:.1f} s "
@@ -475,13 +608,12 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": f"{args.config}{' + mirror vertex normals' if args.smooth else ''}: {w.scene.n_triangles} triangles, {n} photons per GPU per step "
-                               f"({BYTES_IN + BYTES_OUT} B/photon = {(BYTES_IN + BYTES_OUT) * n / 1e6:.0f} MB per step)",
-                   "l2": "inputs + outputs per step exceed the 126 MB L2" if (BYTES_IN + BYTES_OUT) * n > 126e6 else "fits in L2",
+        "config": {"workload": workload_name(args.config, w.scene, n, args.smooth),
+                   "l2": "every step timed on its own after a 256 MB fill that flushes L2" if flush else "inputs + outputs per step exceed the 126 MB L2",
                    "photons_per_gpu": n, "triangles": w.scene.n_triangles, "pixels": scene.n_pixels, "seed": args.seed,
                    "id_partition": "contiguous global photon-id range per rank; scene + BVH replicated"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
-        "paper_pipeline": paper, "emit": emit, "bvh_build_ms": min(t_build), "bvh_build_launches": int(build_launches),
+        "configs": subs, "paper_pipeline": paper, "emit": emit, "bvh_build_ms": min(t_build), "bvh_build_launches": int(build_launches),
         "states": dict(zip(pkg.STATE_NAMES, (int(x) for x in cnt[:7]))),
         "context_paper": "paper: 1.2e6 photons/s per Tesla T4 and 2e5 per Xeon thread, end to end (PAPER.md:9); other hardware, not the target",
     }

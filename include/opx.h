@@ -202,8 +202,10 @@ opx_status opx_propagate_flags(const opx_scene* scene, uint64_t n, const uint64_
  * e_k = the table of material factors[k] (HOST array of n_factors <= 8 material indices, e.g. detector, mirror 1,
  * mirror 2; a material may repeat; n_factors = 0 keeps everything).  The kept photons are written in input
  * order (stable compaction) to d_out_origins / d_out_dirs (x3) / d_out_wavelengths, their index i to
- * d_out_index (may be NULL), and their number to *d_n_kept (DEVICE uint64, overwritten).  All out arrays hold
- * n entries; they must not alias the inputs.  n <= 2^32 - 1.  Trace the survivors with
+ * d_out_index (may be NULL), and their number to *d_n_kept (DEVICE uint64, overwritten).  The out arrays hold
+ * out_capacity entries each (n is always enough) and must not alias the inputs: survivors beyond out_capacity are
+ * not written, but *d_n_kept still receives the TRUE count, so *d_n_kept > out_capacity tells the caller that the
+ * list was truncated.  n <= 2^32 - 1.  Trace the survivors with
  * opx_propagate_flags(..., n, d_n_kept, ..., OPX_FLAG_NO_EFFICIENCY, ...).
  * d_workspace: opx_prefilter_workspace_bytes(n) device bytes, 256-byte aligned. */
 opx_status opx_prefilter_workspace_bytes(uint64_t n, size_t* bytes);
@@ -211,7 +213,8 @@ opx_status opx_prefilter(const opx_scene* scene, uint64_t n, uint64_t photon_id_
                          const float* d_dirs, const float* d_wavelengths, uint64_t seed,
                          const uint32_t* factors, uint32_t n_factors,
                          float* d_out_origins, float* d_out_dirs, float* d_out_wavelengths, uint32_t* d_out_index,
-                         uint64_t* d_n_kept, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+                         uint64_t out_capacity, uint64_t* d_n_kept, void* d_workspace, size_t workspace_bytes,
+                         void* cuda_stream);
 
 /* Track steps for opx_emit_cherenkov: DEVICE pointers.  Step s starts at x[s], runs along the unit vector w[s] for
  * length[s] mm with velocity beta[s]; first (n_steps + 1 entries, non-decreasing, first[0] = 0) is the exclusive
@@ -246,24 +249,16 @@ opx_status opx_emit_cherenkov(const opx_track_steps* steps, uint64_t n_total, fl
  * result is that of the two calls (DESIGN.md 3.12 then 3.9, nothing new is computed): the survivors among photons
  * photon_id_base .. photon_id_base + n - 1, in id order, in d_out_origins / d_out_dirs / d_out_wavelengths, their
  * offsets g - photon_id_base in d_out_index (may be NULL), their number in *d_n_kept (DEVICE uint64, overwritten).
- * The out arrays must hold n entries in the worst case (factors with efficiency 1); size them by an upper bound on
- * the kept fraction at your own risk: nothing is written beyond *d_n_kept entries, but that number is not checked
- * against a capacity.  n <= 2^32 - 1.  Arguments and errors as in opx_emit_cherenkov and opx_prefilter;
+ * The out arrays hold out_capacity entries each (n covers the worst case, factors with efficiency 1; an upper bound
+ * on the kept fraction is enough in practice): survivors beyond out_capacity are not written, and *d_n_kept still
+ * receives the TRUE count, so *d_n_kept > out_capacity reports the truncation.  n <= 2^32 - 1.  Arguments and errors as in opx_emit_cherenkov and opx_prefilter;
  * d_workspace: opx_prefilter_workspace_bytes(n) device bytes, 256-byte aligned.  Three launches, no host round trip;
  * trace the survivors with opx_propagate_flags(..., n, d_n_kept, ..., OPX_FLAG_NO_EFFICIENCY, ...). */
 opx_status opx_emit_cherenkov_filtered(const opx_scene* scene, const opx_track_steps* steps, uint64_t n_total, float n_index,
                                        float lambda1_nm, float lambda2_nm, uint64_t n, uint64_t photon_id_base, uint64_t seed,
                                        const uint32_t* factors, uint32_t n_factors, float* d_out_origins, float* d_out_dirs,
-                                       float* d_out_wavelengths, uint32_t* d_out_index, uint64_t* d_n_kept, void* d_workspace,
-                                       size_t workspace_bytes, void* cuda_stream);
-
-/* Same computation with the closest hit found by testing EVERY triangle on the GPU (no BVH
- * traversal).  A debugging aid that separates the arithmetic of DESIGN.md section 3 from the BVH;
- * O(n x triangles), never timed. */
-opx_status opx_propagate_brute(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,
-                               const float* d_origins, const float* d_dirs, const float* d_wavelengths,
-                               uint64_t seed, const opx_hits* out, uint32_t* d_hitmap,
-                               uint64_t* d_counters, void* cuda_stream);
+                                       float* d_out_wavelengths, uint32_t* d_out_index, uint64_t out_capacity,
+                                       uint64_t* d_n_kept, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* Size of the device staging workspace opx_propagate_host needs for chunks of `chunk` photons. */
 opx_status opx_propagate_host_workspace_bytes(const opx_scene* scene, uint64_t chunk, size_t* bytes);
@@ -281,51 +276,9 @@ opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photo
                               uint64_t* h_counters, void* d_workspace, size_t workspace_bytes,
                               uint64_t chunk, void* cuda_stream);
 
-/* Per-kernel device times for a roofline report.  After opx_profile_begin(scene, max_calls) every
- * opx_propagate call on this scene records CUDA events around its two kernels (propagation; binning
- * + counters) on the call's stream, for at most max_calls calls.  opx_profile_end waits for those
- * events, writes the per-call durations in milliseconds to ms_propagate / ms_bin (each max_calls
- * floats, may be NULL), the number of recorded calls to n_calls, and switches recording off.  Not
- * thread-safe with concurrent opx_propagate calls on the same scene. */
-opx_status opx_profile_begin(opx_scene* scene, uint32_t max_calls);
-opx_status opx_profile_end(opx_scene* scene, float* ms_propagate, float* ms_bin, uint32_t* n_calls);
-
-/* Work counters of the propagation kernel for the roofline model: runs the same
- * traversal with an instrumented kernel that writes no records and ADDS to d_stats (4 uint64,
- * DEVICE): [0] segments (closest-hit queries), [1] BVH nodes visited (two child boxes each),
- * [2] ray/triangle tests, [3] surface interactions.  Never timed. */
-opx_status opx_propagate_stats(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,
-                               const float* d_origins, const float* d_dirs, const float* d_wavelengths,
-                               uint64_t seed, uint64_t* d_stats, void* cuda_stream);
-
-/* Work counters of the PRODUCT kernel (k_propagate_packet, instrumented instantiation): same records
- * as opx_propagate into `out` (DEVICE arrays of n), no binning, and ADDS to d_stats (8 uint64, DEVICE):
- * [0] packet-segments (one closest-hit query of a 32-photon packet) answered by beam traversal of the
- * 32-wide tree, [1] packet-segments answered by the binary packet walk (incoherent packets, stack
- * overflow, no wide tree), [2] wide nodes visited, [3] triangles handed to the lanes by beam traversal
- * (each is tested by every live lane), [4] beam-stack overflows, [5..7] reserved.  Never timed. */
-opx_status opx_propagate_packet_stats(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,
-                                      const float* d_origins, const float* d_dirs, const float* d_wavelengths,
-                                      uint64_t seed, const opx_hits* out, uint64_t* d_stats, void* cuda_stream);
-
-/* Number of 32-wide nodes the last opx_bvh_build produced (0: the collapse did not fit its capacity and
- * packets walk the binary tree only) and the capacity reserved in the scene workspace. */
-opx_status opx_scene_wide_info(const opx_scene* scene, uint64_t* n_wide_nodes, uint64_t* capacity);
-
-/* FP32 FMA micro-benchmark (8 independent chains per thread, 8 blocks of 256 threads per SM, no memory
- * traffic): writes the best of three timed launches, in TFLOP/s (FMA = 2), to *tflops.  It is the
- * measured counterpart of the derived peak SMs x 128 lanes x 2 x clock that the roofline of the
- * ALU-bound propagation kernel is quoted against.  d_scratch: >= 4 device bytes.
- * Synchronises the stream. */
-opx_status opx_measure_fp32_peak(double* tflops, void* d_scratch, void* cuda_stream);
-
 opx_status opx_scene_info(const opx_scene* scene, uint64_t* n_triangles, uint64_t* n_nodes,
                           uint64_t* n_pixels, uint64_t* n_surfaces);
 opx_status opx_scene_get_layout(const opx_scene* scene, opx_scene_layout* out);
-
-/* Number of kernel launches the library has enqueued in this process (monotonic; for bench.py's
- * gpu_launches accounting). */
-uint64_t opx_launch_count(void);
 
 void opx_scene_destroy(opx_scene* scene);
 const char* opx_last_error(void); /* thread-local, never NULL */

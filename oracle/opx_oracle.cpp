@@ -449,24 +449,6 @@ int oracle_trace_mesh_ex2(int fp64, const uint32_t* mat_interp, uint32_t flags, 
     return 0;
 }
 
-// The form written before vertex normals existed: every mirror reflects about its face normal.
-int oracle_trace_mesh_ex(int fp64, const uint32_t* mat_interp, uint32_t flags,
-                      const float* tri, const int32_t* tri_surface, uint64_t n_tri,
-                      const uint32_t* surf_material, const int32_t* surf_frame, uint32_t n_surf,
-                      const uint32_t* mat_kind, const float* mat_table, uint32_t n_mat, uint32_t n_lambda,
-                      float lambda_min, float lambda_max, const Frame* frames, uint32_t n_frames,
-                      uint32_t max_bounces, float t_min,
-                      uint64_t n, const uint64_t* ids, uint64_t id_base,
-                      const float* origins, const float* dirs, const float* wl, uint64_t seed,
-                      double* pos, double* dir, int32_t* pixel, int32_t* surface, int32_t* tri_out,
-                      uint8_t* state, uint8_t* bounces, uint32_t* segments, uint32_t* hitmap,
-                      uint64_t* counters, int n_threads) {
-    return oracle_trace_mesh_ex2(fp64, mat_interp, flags, nullptr, tri, tri_surface, n_tri, surf_material, surf_frame, n_surf,
-                                 mat_kind, mat_table, n_mat, n_lambda, lambda_min, lambda_max, frames, n_frames, max_bounces,
-                                 t_min, n, ids, id_base, origins, dirs, wl, seed, pos, dir, pixel, surface, tri_out, state,
-                                 bounces, segments, hitmap, counters, n_threads);
-}
-
 // Shading normal at the point where the ray (o, d) meets triangle v9 with vertex normals n9.
 // Returns 0 on a miss; uvw (3, may be NULL) receives the edge functions.
 int oracle_shading_normal(int fp64, const float* o, const float* d, const float* v9, const float* n9, double* out, double* uvw_out) {
@@ -486,24 +468,6 @@ int oracle_shading_normal(int fp64, const float* o, const float* d, const float*
     out[0] = nn.x; out[1] = nn.y; out[2] = nn.z;
     if (uvw_out) { uvw_out[0] = uvw[0]; uvw_out[1] = uvw[1]; uvw_out[2] = uvw[2]; }
     return 1;
-}
-
-// The form every test written before the table forms and flags existed calls: linear tables, in-flight draws.
-int oracle_trace_mesh(int fp64,
-                      const float* tri, const int32_t* tri_surface, uint64_t n_tri,
-                      const uint32_t* surf_material, const int32_t* surf_frame, uint32_t n_surf,
-                      const uint32_t* mat_kind, const float* mat_table, uint32_t n_mat, uint32_t n_lambda,
-                      float lambda_min, float lambda_max, const Frame* frames, uint32_t n_frames,
-                      uint32_t max_bounces, float t_min,
-                      uint64_t n, const uint64_t* ids, uint64_t id_base,
-                      const float* origins, const float* dirs, const float* wl, uint64_t seed,
-                      double* pos, double* dir, int32_t* pixel, int32_t* surface, int32_t* tri_out,
-                      uint8_t* state, uint8_t* bounces, uint32_t* segments, uint32_t* hitmap,
-                      uint64_t* counters, int n_threads) {
-    return oracle_trace_mesh_ex(fp64, nullptr, 0u, tri, tri_surface, n_tri, surf_material, surf_frame, n_surf, mat_kind,
-                                mat_table, n_mat, n_lambda, lambda_min, lambda_max, frames, n_frames, max_bounces, t_min,
-                                n, ids, id_base, origins, dirs, wl, seed, pos, dir, pixel, surface, tri_out, state,
-                                bounces, segments, hitmap, counters, n_threads);
 }
 
 double oracle_table_value(int fp64, const float* y, uint32_t n_lambda, uint32_t interp, float lmin, float lmax, float lambda) {

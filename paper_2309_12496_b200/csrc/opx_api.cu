@@ -23,6 +23,10 @@ opx_status check_cuda(cudaError_t e, const char* what) {
 }
 
 void count_launch(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+uint64_t launch_count() { return g_launches.load(std::memory_order_relaxed); }
+static thread_local const char* g_last_kernel = "";
+void set_last_kernel(const char* name) { g_last_kernel = name; }
+const char* last_kernel() { return g_last_kernel; }
 
 // n = normalise((b-a) x (c-a)) in fp64, rounded once; zero-area triangle => 0.
 static void face_normal(const float* v, float* out) {
@@ -34,7 +38,7 @@ static void face_normal(const float* v, float* out) {
     out[0] = (float)(cx / len); out[1] = (float)(cy / len); out[2] = (float)(cz / len);
 }
 
-static opx_status device_ok() {
+opx_status device_ok() {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return check_cuda(e, "cudaGetDevice");
@@ -47,6 +51,26 @@ static opx_status device_ok() {
 
 static bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) != 0; }
 
+opx_status propagate_common(const opx_scene* scene, WalkMode mode, uint64_t n, const uint64_t* d_n, uint64_t base,
+                                   const float* o, const float* d, const float* wl, uint64_t seed, uint32_t flags,
+                                   const opx_hits* out, uint32_t* hitmap, uint64_t* counters, void* stream) {
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate before opx_bvh_build");
+    if (n == 0) return OPX_OK;
+    if (!o || !d || !wl || !out) return fail(OPX_ERR_INVALID_ARG, "NULL photon/record pointer");
+    if (!out->pos || !out->dir || !out->pixel || !out->surface || !out->state || !out->bounces)
+        return fail(OPX_ERR_INVALID_ARG, "NULL hit-record array");
+    if (!hitmap && scene->n_pixels) return fail(OPX_ERR_INVALID_ARG, "d_hitmap is NULL but the scene has pixels");
+    if (misaligned(o, 4) || misaligned(d, 4) || misaligned(wl, 4) || misaligned(out->pos, 4) || misaligned(out->dir, 4) ||
+        misaligned(out->pixel, 4) || misaligned(out->surface, 4) || misaligned(hitmap, 4) || misaligned(counters, 8))
+        return fail(OPX_ERR_INVALID_ARG, "misaligned pointer");
+    if (n > (1ull << 40)) return fail(OPX_ERR_INVALID_ARG, "n too large for one call");
+    if (flags & ~(uint32_t)OPX_FLAG_NO_EFFICIENCY) return fail(OPX_ERR_INVALID_ARG, "unknown flag");
+    if (misaligned(d_n, 8)) return fail(OPX_ERR_INVALID_ARG, "misaligned d_n");
+    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_propagate")) return st;
+    return launch_propagate(*scene, mode, n, d_n, base, o, d, wl, seed, flags, *out, hitmap, counters, (cudaStream_t)stream);
+}
+
 }  // namespace opx
 
 using namespace opx;
@@ -55,7 +79,6 @@ extern "C" {
 
 const char* opx_last_error(void) { return g_last_error.c_str(); }
 const char* opx_version(void) { return "opx 0.1 (sm_100a)"; }
-uint64_t opx_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 opx_status opx_scene_create(const opx_scene_params* params, const opx_mesh* meshes, uint32_t n_meshes,
                             const opx_material* materials, uint32_t n_materials,
@@ -174,30 +197,10 @@ opx_status opx_bvh_build(opx_scene* scene, void* d_scene_ws, size_t scene_bytes,
     return OPX_OK;
 }
 
-static opx_status propagate_common(const opx_scene* scene, bool brute, uint64_t n, const uint64_t* d_n, uint64_t base,
-                                   const float* o, const float* d, const float* wl, uint64_t seed, uint32_t flags,
-                                   const opx_hits* out, uint32_t* hitmap, uint64_t* counters, void* stream) {
-    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
-    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate before opx_bvh_build");
-    if (n == 0) return OPX_OK;
-    if (!o || !d || !wl || !out) return fail(OPX_ERR_INVALID_ARG, "NULL photon/record pointer");
-    if (!out->pos || !out->dir || !out->pixel || !out->surface || !out->state || !out->bounces)
-        return fail(OPX_ERR_INVALID_ARG, "NULL hit-record array");
-    if (!hitmap && scene->n_pixels) return fail(OPX_ERR_INVALID_ARG, "d_hitmap is NULL but the scene has pixels");
-    if (misaligned(o, 4) || misaligned(d, 4) || misaligned(wl, 4) || misaligned(out->pos, 4) || misaligned(out->dir, 4) ||
-        misaligned(out->pixel, 4) || misaligned(out->surface, 4) || misaligned(hitmap, 4) || misaligned(counters, 8))
-        return fail(OPX_ERR_INVALID_ARG, "misaligned pointer");
-    if (n > (1ull << 40)) return fail(OPX_ERR_INVALID_ARG, "n too large for one call");
-    if (flags & ~(uint32_t)OPX_FLAG_NO_EFFICIENCY) return fail(OPX_ERR_INVALID_ARG, "unknown flag");
-    if (misaligned(d_n, 8)) return fail(OPX_ERR_INVALID_ARG, "misaligned d_n");
-    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_propagate")) return st;
-    return launch_propagate(*scene, brute, n, d_n, base, o, d, wl, seed, flags, *out, hitmap, counters, (cudaStream_t)stream);
-}
-
 opx_status opx_propagate(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
                          const float* d_dirs, const float* d_wavelengths, uint64_t seed, const opx_hits* out,
                          uint32_t* d_hitmap, uint64_t* d_counters, void* cuda_stream) {
-    return propagate_common(scene, false, n, nullptr, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, 0u, out, d_hitmap,
+    return propagate_common(scene, kWalkProduct, n, nullptr, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, 0u, out, d_hitmap,
                             d_counters, cuda_stream);
 }
 
@@ -205,7 +208,7 @@ opx_status opx_propagate_flags(const opx_scene* scene, uint64_t n, const uint64_
                                const float* d_origins, const float* d_dirs, const float* d_wavelengths,
                                uint64_t seed, uint32_t flags, const opx_hits* out, uint32_t* d_hitmap,
                                uint64_t* d_counters, void* cuda_stream) {
-    return propagate_common(scene, false, n, d_n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, flags, out, d_hitmap,
+    return propagate_common(scene, kWalkProduct, n, d_n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, flags, out, d_hitmap,
                             d_counters, cuda_stream);
 }
 
@@ -220,7 +223,7 @@ opx_status opx_prefilter(const opx_scene* scene, uint64_t n, uint64_t photon_id_
                          const float* d_dirs, const float* d_wavelengths, uint64_t seed,
                          const uint32_t* factors, uint32_t n_factors,
                          float* d_out_origins, float* d_out_dirs, float* d_out_wavelengths, uint32_t* d_out_index,
-                         uint64_t* d_n_kept, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+                         uint64_t out_capacity, uint64_t* d_n_kept, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
     if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
     if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_prefilter before opx_bvh_build");
     if (!d_n_kept || misaligned(d_n_kept, 8)) return fail(OPX_ERR_INVALID_ARG, "d_n_kept is NULL or misaligned");
@@ -241,7 +244,7 @@ opx_status opx_prefilter(const opx_scene* scene, uint64_t n, uint64_t photon_id_
         return fail(OPX_ERR_INVALID_ARG, "out arrays must not alias the inputs");
     if (workspace_bytes < prefilter_workspace_bytes(n)) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_prefilter_workspace_bytes)");
     return launch_prefilter(*scene, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, factors, n_factors, d_out_origins,
-                            d_out_dirs, d_out_wavelengths, d_out_index, d_n_kept, d_workspace, (cudaStream_t)cuda_stream);
+                            d_out_dirs, d_out_wavelengths, d_out_index, out_capacity, d_n_kept, d_workspace, (cudaStream_t)cuda_stream);
 }
 
 opx_status opx_emit_cherenkov(const opx_track_steps* steps, uint64_t n_total, float n_index, float lambda1_nm,
@@ -267,8 +270,8 @@ opx_status opx_emit_cherenkov(const opx_track_steps* steps, uint64_t n_total, fl
 opx_status opx_emit_cherenkov_filtered(const opx_scene* scene, const opx_track_steps* steps, uint64_t n_total, float n_index,
                                        float lambda1_nm, float lambda2_nm, uint64_t n, uint64_t photon_id_base, uint64_t seed,
                                        const uint32_t* factors, uint32_t n_factors, float* d_out_origins, float* d_out_dirs,
-                                       float* d_out_wavelengths, uint32_t* d_out_index, uint64_t* d_n_kept, void* d_workspace,
-                                       size_t workspace_bytes, void* cuda_stream) {
+                                       float* d_out_wavelengths, uint32_t* d_out_index, uint64_t out_capacity, uint64_t* d_n_kept,
+                                       void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
     if (!scene || !steps) return fail(OPX_ERR_INVALID_ARG, "scene/steps is NULL");
     if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_emit_cherenkov_filtered before opx_bvh_build");
     if (!d_n_kept || misaligned(d_n_kept, 8)) return fail(OPX_ERR_INVALID_ARG, "d_n_kept is NULL or misaligned");
@@ -292,14 +295,7 @@ opx_status opx_emit_cherenkov_filtered(const opx_scene* scene, const opx_track_s
         return fail(OPX_ERR_INVALID_ARG, "misaligned pointer");
     if (workspace_bytes < prefilter_workspace_bytes(n)) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_prefilter_workspace_bytes)");
     return launch_emit_filtered(*scene, *steps, n_index, lambda1_nm, lambda2_nm, n, photon_id_base, seed, factors, n_factors,
-                                d_out_origins, d_out_dirs, d_out_wavelengths, d_out_index, d_n_kept, d_workspace, (cudaStream_t)cuda_stream);
-}
-
-opx_status opx_propagate_brute(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
-                               const float* d_dirs, const float* d_wavelengths, uint64_t seed, const opx_hits* out,
-                               uint32_t* d_hitmap, uint64_t* d_counters, void* cuda_stream) {
-    return propagate_common(scene, true, n, nullptr, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, 0u, out, d_hitmap,
-                            d_counters, cuda_stream);
+                                d_out_origins, d_out_dirs, d_out_wavelengths, d_out_index, out_capacity, d_n_kept, d_workspace, (cudaStream_t)cuda_stream);
 }
 
 // ------------------------------------------------------------------------- host-buffer streaming
@@ -385,7 +381,7 @@ opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photo
         cudaMemcpyAsync(s.d, h_dirs + 3 * done, m * 12, cudaMemcpyHostToDevice, s.st);
         cudaMemcpyAsync(s.wl, h_wavelengths + done, m * 4, cudaMemcpyHostToDevice, s.st);
         opx_hits dev_out{s.pos, s.dir, s.pixel, s.surface, s.state, s.bounces};
-        st = launch_propagate(*scene, false, m, nullptr, photon_id_base + done, s.o, s.d, s.wl, seed, 0u, dev_out, d_hitmap,
+        st = launch_propagate(*scene, kWalkProduct, m, nullptr, photon_id_base + done, s.o, s.d, s.wl, seed, 0u, dev_out, d_hitmap,
                               d_counters, s.st);
         cudaMemcpyAsync(h_out->pos + 3 * done, s.pos, m * 12, cudaMemcpyDeviceToHost, s.st);
         cudaMemcpyAsync(h_out->dir + 3 * done, s.dir, m * 12, cudaMemcpyDeviceToHost, s.st);
@@ -409,66 +405,6 @@ opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photo
     if (e != cudaSuccess) return check_cuda(e, "opx_propagate_host");
     for (uint64_t i = 0; i < scene->n_pixels; ++i) h_hitmap[i] += hm[i];
     if (h_counters) for (int i = 0; i < 8; ++i) h_counters[i] += cnt[i];
-    return OPX_OK;
-}
-
-opx_status opx_profile_begin(opx_scene* scene, uint32_t max_calls) {
-    if (!scene || max_calls == 0) return fail(OPX_ERR_INVALID_ARG, "scene is NULL or max_calls = 0");
-    while (scene->prof_events.size() < 3ull * max_calls) {
-        cudaEvent_t e;
-        if (opx_status st = check_cuda(cudaEventCreate(&e), "cudaEventCreate")) return st;
-        scene->prof_events.push_back(e);
-    }
-    scene->prof_max = max_calls;
-    scene->prof_used = 0;
-    return OPX_OK;
-}
-
-opx_status opx_profile_end(opx_scene* scene, float* ms_propagate, float* ms_bin, uint32_t* n_calls) {
-    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
-    const uint32_t used = scene->prof_used;
-    scene->prof_max = 0;
-    scene->prof_used = 0;
-    if (n_calls) *n_calls = used;
-    for (uint32_t k = 0; k < used; ++k) {
-        cudaEvent_t* ev = &scene->prof_events[3 * k];
-        if (opx_status st = check_cuda(cudaEventSynchronize(ev[2]), "cudaEventSynchronize")) return st;
-        float a = 0.f, b = 0.f;
-        if (opx_status st = check_cuda(cudaEventElapsedTime(&a, ev[0], ev[1]), "cudaEventElapsedTime")) return st;
-        if (opx_status st = check_cuda(cudaEventElapsedTime(&b, ev[1], ev[2]), "cudaEventElapsedTime")) return st;
-        if (ms_propagate) ms_propagate[k] = a;
-        if (ms_bin) ms_bin[k] = b;
-    }
-    return OPX_OK;
-}
-
-opx_status opx_propagate_stats(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
-                               const float* d_dirs, const float* d_wavelengths, uint64_t seed, uint64_t* d_stats,
-                               void* cuda_stream) {
-    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
-    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate_stats before opx_bvh_build");
-    if (n == 0) return OPX_OK;
-    if (!d_origins || !d_dirs || !d_wavelengths || !d_stats) return fail(OPX_ERR_INVALID_ARG, "NULL pointer");
-    return launch_stats(*scene, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, d_stats, (cudaStream_t)cuda_stream);
-}
-
-opx_status opx_propagate_packet_stats(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
-                                      const float* d_dirs, const float* d_wavelengths, uint64_t seed, const opx_hits* out,
-                                      uint64_t* d_stats, void* cuda_stream) {
-    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
-    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate_packet_stats before opx_bvh_build");
-    if (n == 0) return OPX_OK;
-    if (!d_origins || !d_dirs || !d_wavelengths || !d_stats || !out) return fail(OPX_ERR_INVALID_ARG, "NULL pointer");
-    if (!out->pos || !out->dir || !out->pixel || !out->surface || !out->state || !out->bounces)
-        return fail(OPX_ERR_INVALID_ARG, "NULL hit-record array");
-    return launch_packet_stats(*scene, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, *out, d_stats, (cudaStream_t)cuda_stream);
-}
-
-opx_status opx_scene_wide_info(const opx_scene* scene, uint64_t* n_wide_nodes, uint64_t* capacity) {
-    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
-    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_scene_wide_info before opx_bvh_build");
-    if (n_wide_nodes) *n_wide_nodes = scene->dev.n_wnodes;
-    if (capacity) *capacity = scene->layout.wide_node_capacity;
     return OPX_OK;
 }
 

@@ -76,7 +76,9 @@ __device__ __forceinline__ bool beam_setup(const SceneDev& sc, float ox, float o
     if (fabsf(lz) > fabsf(lk)) { K = 2; lk = lz; }
     const float dK = K == 0 ? dx : (K == 1 ? dy : dz), oK = K == 0 ? ox : (K == 1 ? oy : oz);
     const float sumabs = fabsf(ox) + fabsf(oy) + fabsf(oz) + fabsf(dx) + fabsf(dy) + fabsf(dz);
-    const bool member = sumabs < kInf && (lk > 0.f ? dK >= 0.25f : dK <= -0.25f);     // NaN fails both
+    // sumabs bounds |o|_inf: an origin beyond origin_limit (4 x the scene's largest coordinate) leaves the error budget of
+    // the padded boxes and takes the binary walk with per-ray slack
+    const bool member = sumabs < sc.origin_limit && (lk > 0.f ? dK >= 0.25f : dK <= -0.25f);     // NaN fails both
     if (!__all_sync(full, member)) return false;
     // rear-most origin along K
     const float c = lk > 0.f ? warp_min(oK) : warp_max(oK);

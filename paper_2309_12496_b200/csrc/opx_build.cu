@@ -247,8 +247,14 @@ __global__ void __launch_bounds__(256) k_refit(const float4* __restrict__ tris, 
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= T) return;
     const float4 a = tris[3 * (size_t)j], b = tris[3 * (size_t)j + 1], c = tris[3 * (size_t)j + 2];
-    float lo[3] = {fminf(a.x, fminf(b.x, c.x)) - pad, fminf(a.y, fminf(b.y, c.y)) - pad, fminf(a.z, fminf(b.z, c.z)) - pad};
-    float hi[3] = {fmaxf(a.x, fmaxf(b.x, c.x)) + pad, fmaxf(a.y, fmaxf(b.y, c.y)) + pad, fmaxf(a.z, fmaxf(b.z, c.z)) + pad};
+    float lo[3] = {fminf(a.x, fminf(b.x, c.x)), fminf(a.y, fminf(b.y, c.y)), fminf(a.z, fminf(b.z, c.z))};
+    float hi[3] = {fmaxf(a.x, fmaxf(b.x, c.x)), fmaxf(a.y, fmaxf(b.y, c.y)), fmaxf(a.z, fmaxf(b.z, c.z))};
+    // padding: `pad` = 2^-16 of the largest scene coordinate covers the rounding of vertex - origin, of the
+    // shear and of the slab arithmetic; 2^-10 of the triangle's own extent covers the one error that grows with the
+    // triangle: at grazing incidence the contract's barycentric weights lose accuracy and the hit point o + t d can sit
+    // up to sqrt(3 x 2^-23) = 6e-4 of the triangle's size off its plane
+    pad += 9.765625e-4f * fmaxf(hi[0] - lo[0], fmaxf(hi[1] - lo[1], hi[2] - lo[2]));
+    for (int k = 0; k < 3; ++k) { lo[k] -= pad; hi[k] += pad; }
     int child = ~j;
     int p = parents[T - 1 + j];
     while (p >= 0) {
@@ -400,6 +406,7 @@ void compute_scene_stats(SceneHost& s) {
     float maxabs = 0.f;
     for (float v : s.tri) { const float a = std::fabs(v); if (a > maxabs) maxabs = a; }
     s.leaf_pad = fmaxf(maxabs * (1.0f / 65536.0f), 1e-6f);
+    s.max_abs = maxabs;
     // typical triangle size (log-mean of the largest AABB extent) and scene extent: a beam much wider
     // than the triangles it meets gains nothing over per-ray box tests
     double logsum = 0.0;
@@ -456,6 +463,7 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
         (e = up(ws + lay.vertex_normals, s.tri_vnormals.data(), s.tri_vnormals.size() * 4)))
         return check_cuda(e, "scene upload");
 
+    if (opx_status st = configure_device()) return st;
     const float pad = s.leaf_pad, tri_size = s.tri_size, scene_ext = s.scene_ext;      // scene constants (compute_scene_stats)
 
     const int Ti = (int)T;
@@ -526,6 +534,7 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
     d.beam_max_spread = scene_ext > 0.f ? d.beam_max_width / (0.5f * scene_ext) : 0.f;
     d.lambda_min = s.params.lambda_min_nm; d.inv_dlambda = s.inv_dlambda; d.t_min = s.params.t_min_mm;
     d.inv_bin = s.inv_bin; d.flags = 0; d.d_n = nullptr;
+    d.origin_limit = 4.f * fmaxf(s.max_abs, 1.f);
     return OPX_OK;
 }
 

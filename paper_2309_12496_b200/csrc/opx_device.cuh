@@ -263,16 +263,33 @@ __device__ __forceinline__ void store_record(const opx_hits& out, uint64_t i, co
 }
 
 // Slab test of one segment against the two child boxes of a node.  px = -o*inv_d.  The boxes are
-// padded at build time by >= 128 ulp of the largest scene coordinate, which is what makes this cheap
-// form (approximate reciprocal, one fma per plane, no re-scaling of the exit distance) conservative
-// with respect to tri_test: its rounding error is a few ulp of that coordinate.
+// padded at build time (2^-16 of the largest scene coordinate + 2^-10 of the triangle's
+// own extent), which is what makes this cheap form (approximate reciprocal, one fma per plane, no
+// re-scaling of the exit distance) conservative with respect to tri_test for origins inside
+// SceneDev::origin_limit; rays that start further out add their own slack (slab2_slack).
 struct Slab { float ix, iy, iz, px, py, pz; };
+
+// 1/d for the slab test, finite for every finite d: a component of +-0 (or a denormal) would give ix = +-inf and
+// px = -o*ix = -+inf, and fma(plane, ix, px) = inf - inf = NaN whenever plane and origin share a sign -- the NaN-skipping
+// fminf/fmaxf would then EMPTY the interval of a box the ray runs through.  With |d| clamped to 1e-30 (sign kept, so a
+// component of -0 still belongs to the negative octant, see dir_octant) the planes of that axis land at -+1e30-ish: the
+// axis constrains nothing when the origin is between the planes and rejects the box when it is not, which is what a ray
+// parallel to the slab must do.  NaN stays NaN: every comparison fails and the ray hits no box.
+__device__ __forceinline__ float slab_rcp(float d) {
+    return __fdividef(1.f, fabsf(d) < 1e-30f ? copysignf(1e-30f, d) : d);
+}
 
 __device__ __forceinline__ Slab slab_setup(float ox, float oy, float oz, float dx, float dy, float dz) {
     Slab s;
-    s.ix = __fdividef(1.f, dx); s.iy = __fdividef(1.f, dy); s.iz = __fdividef(1.f, dz);
+    s.ix = slab_rcp(dx); s.iy = slab_rcp(dy); s.iz = slab_rcp(dz);
     s.px = -ox * s.ix; s.py = -oy * s.iy; s.pz = -oz * s.iz;
     return s;
+}
+
+// Sign octant of a direction from the SIGN BITS (bit a set = component a negative, -0 included): the octant-specialised
+// slab test picks the entry plane by this, and slab_rcp keeps the sign of a zero, so the two always agree.
+__device__ __forceinline__ int dir_octant(float dx, float dy, float dz) {
+    return (int)(((unsigned)__float_as_int(dx) >> 31) | (((unsigned)__float_as_int(dy) >> 31) << 1) | (((unsigned)__float_as_int(dz) >> 31) << 2));
 }
 
 // child 0: lo = (q0.x,q0.y,q0.z) hi = (q0.w,q1.x,q1.y); child 1: lo = (q1.z,q1.w,q2.x) hi = (q2.y,q2.z,q2.w).
@@ -292,6 +309,29 @@ __device__ __forceinline__ void slab2(const Slab& s, const float4 q0, const floa
     n1 = fmaxf(n1, fminf(a, b)); f1 = fminf(f1, fmaxf(a, b));
     a = __fmaf_rn(q2.x, s.iz, s.pz); b = __fmaf_rn(q2.w, s.iz, s.pz);
     n1 = fmaxf(n1, fminf(a, b)); f1 = fminf(f1, fmaxf(a, b));
+    n0 = fmaxf(n0, 0.f); n1 = fmaxf(n1, 0.f);
+    f0 = fminf(f0, tcap); f1 = fminf(f1, tcap);
+}
+
+// slab2 for a ray whose origin lies outside SceneDev::origin_limit: the contract test works on
+// vertex - origin, whose rounding grows with |origin|, so the triangles it accepts may lie up to e = 2^-20 |origin|_inf
+// outside their padded boxes.  Every box is widened by e on the fly: e |i_a| in the ray parameter of axis a.
+__device__ __forceinline__ void slab2_slack(const Slab& s, float e, const float4 q0, const float4 q1, const float4 q2, float tcap,
+                                            float& n0, float& f0, float& n1, float& f1) {
+    const float ex = e * fabsf(s.ix), ey = e * fabsf(s.iy), ez = e * fabsf(s.iz);
+    float a, b;
+    a = __fmaf_rn(q0.x, s.ix, s.px); b = __fmaf_rn(q0.w, s.ix, s.px);
+    n0 = fminf(a, b) - ex; f0 = fmaxf(a, b) + ex;
+    a = __fmaf_rn(q0.y, s.iy, s.py); b = __fmaf_rn(q1.x, s.iy, s.py);
+    n0 = fmaxf(n0, fminf(a, b) - ey); f0 = fminf(f0, fmaxf(a, b) + ey);
+    a = __fmaf_rn(q0.z, s.iz, s.pz); b = __fmaf_rn(q1.y, s.iz, s.pz);
+    n0 = fmaxf(n0, fminf(a, b) - ez); f0 = fminf(f0, fmaxf(a, b) + ez);
+    a = __fmaf_rn(q1.z, s.ix, s.px); b = __fmaf_rn(q2.y, s.ix, s.px);
+    n1 = fminf(a, b) - ex; f1 = fmaxf(a, b) + ex;
+    a = __fmaf_rn(q1.w, s.iy, s.py); b = __fmaf_rn(q2.z, s.iy, s.py);
+    n1 = fmaxf(n1, fminf(a, b) - ey); f1 = fminf(f1, fmaxf(a, b) + ey);
+    a = __fmaf_rn(q2.x, s.iz, s.pz); b = __fmaf_rn(q2.w, s.iz, s.pz);
+    n1 = fmaxf(n1, fminf(a, b) - ez); f1 = fminf(f1, fmaxf(a, b) + ez);
     n0 = fmaxf(n0, 0.f); n1 = fmaxf(n1, 0.f);
     f0 = fminf(f0, tcap); f1 = fminf(f1, tcap);
 }

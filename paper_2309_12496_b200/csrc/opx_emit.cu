@@ -177,7 +177,7 @@ __global__ void __launch_bounds__(kFThreads) k_emitf_compact(const opx_track_ste
                                                              uint64_t n, uint64_t id_base, uint64_t seed,
                                                              const uint32_t* __restrict__ words, const uint32_t* __restrict__ block_offset,
                                                              float* __restrict__ origins, float* __restrict__ dirs,
-                                                             float* __restrict__ wl, uint32_t* __restrict__ oidx) {
+                                                             float* __restrict__ wl, uint32_t* __restrict__ oidx, uint64_t capacity) {
     __shared__ StepWindow sw;
     __shared__ uint32_t s_mask[kFWords], s_pre[kFWords + 1];
     __shared__ uint16_t s_list[kFBlk];
@@ -206,6 +206,7 @@ __global__ void __launch_bounds__(kFThreads) k_emitf_compact(const opx_track_ste
     const uint32_t cnt = s_pre[kFWords];
     const uint64_t off = (uint64_t)__ldg(block_offset + blockIdx.x);
     for (uint32_t q = threadIdx.x; q < cnt; q += kFThreads) {
+        if (off + q >= capacity) break;   // the out arrays are full: *d_n_kept still holds the true count
         const uint64_t i = blk_base + s_list[q], g = id_base + i;
         emit_photon(st, window_find(sw, st, g), g, seed, n_index, lambda1, lambda2, off + q, origins, dirs, wl);
         if (oidx) oidx[off + q] = (uint32_t)i;
@@ -225,7 +226,7 @@ opx_status launch_emit(const opx_track_steps& st, float n_index, float lambda1, 
 
 opx_status launch_emit_filtered(const SceneHost& s, const opx_track_steps& st, float n_index, float lambda1, float lambda2, uint64_t n,
                                 uint64_t id_base, uint64_t seed, const uint32_t* factors, uint32_t n_factors, float* o, float* d,
-                                float* wl, uint32_t* oidx, uint64_t* d_n_kept, void* ws, cudaStream_t stream) {
+                                float* wl, uint32_t* oidx, uint64_t capacity, uint64_t* d_n_kept, void* ws, cudaStream_t stream) {
     FilterFactors fa{};
     fa.n = n_factors;
     for (uint32_t k = 0; k < n_factors; ++k) { fa.m[k] = factors[k]; fa.mk[k] = s.mat_kinds[factors[k]]; }
@@ -234,7 +235,7 @@ opx_status launch_emit_filtered(const SceneHost& s, const opx_track_steps& st, f
     uint32_t* counts = (uint32_t*)((char*)ws + align_up((size_t)nb * kFWords * 4, 256));
     k_emitf_mark<<<(unsigned)nb, kFThreads, 0, stream>>>(s.dev, fa, lambda1, lambda2, n, id_base, seed, words, counts);
     launch_prefilter_scan(counts, (uint32_t)nb, d_n_kept, stream);
-    k_emitf_compact<<<(unsigned)nb, kFThreads, 0, stream>>>(st, n_index, lambda1, lambda2, n, id_base, seed, words, counts, o, d, wl, oidx);
+    k_emitf_compact<<<(unsigned)nb, kFThreads, 0, stream>>>(st, n_index, lambda1, lambda2, n, id_base, seed, words, counts, o, d, wl, oidx, capacity);
     count_launch(3);
     return check_cuda(cudaGetLastError(), "emit+filter launch");
 }

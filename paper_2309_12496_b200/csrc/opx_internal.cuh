@@ -51,6 +51,7 @@ struct SceneDev {
     uint32_t flags;            // opx_flags of this launch (set per call, 0 in the stored copy)
     const unsigned long long* d_n;   // optional device-side photon count of this launch (min(n, *d_n) photons), else NULL
     float beam_max_width, beam_max_spread;   // packets wider than this (origins [mm] / directions) walk the binary tree
+    float origin_limit;        // 4 x the largest |vertex coordinate|: a ray whose |o|_inf reaches this is walked with per-ray slack
 };
 
 struct Layout : opx_scene_layout {};
@@ -68,7 +69,7 @@ struct SceneHost {
     std::vector<FrameDev> frames;
     uint64_t n_pixels = 0;
     float inv_dlambda = 0.f, inv_bin = 0.f;
-    float leaf_pad = 1e-6f, tri_size = 0.f, scene_ext = 0.f;   // compute_scene_stats: box padding, typical triangle size, extent
+    float leaf_pad = 1e-6f, tri_size = 0.f, scene_ext = 0.f, max_abs = 0.f;   // compute_scene_stats: box padding, typical triangle size, extent, largest |coordinate|
     // set by opx_bvh_build
     bool built = false;
     void* d_scene_ws = nullptr;
@@ -85,6 +86,9 @@ struct SceneHost {
 opx_status fail(opx_status st, const std::string& msg);
 opx_status check_cuda(cudaError_t e, const char* what);
 void count_launch(uint64_t n = 1);
+uint64_t launch_count();
+void set_last_kernel(const char* name);   // name of the propagation kernel instantiation the last launch on this thread took
+const char* last_kernel();
 
 // build (opx_build.cu)
 void compute_layout(const SceneHost& s, opx_scene_layout* lay, size_t* tmp_bytes);
@@ -92,14 +96,20 @@ void compute_scene_stats(SceneHost& s);
 opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_t stream);
 
 // propagate (opx_propagate.cu)
-opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
+enum WalkMode { kWalkProduct = 0, kWalkBrute = 1, kWalkBinary = 2 };   // product path / every triangle (debug) / binary tree only (debug)
+opx_status configure_device();      // per-device kernel attributes (dynamic shared memory sizes); idempotent, thread-safe
+opx_status propagate_common(const opx_scene* scene, WalkMode mode, uint64_t n, const uint64_t* d_n, uint64_t base, const float* o,
+                            const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_hits* out, uint32_t* hitmap,
+                            uint64_t* counters, void* stream);
+opx_status device_ok();
+opx_status launch_propagate(const SceneHost& s, WalkMode mode, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
                             const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_hits& out,
                             uint32_t* hitmap, uint64_t* counters, cudaStream_t stream);
 // pre-propagation filter (opx_prefilter.cu)
 size_t prefilter_workspace_bytes(uint64_t n);
 opx_status launch_prefilter(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d, const float* wl,
                             uint64_t seed, const uint32_t* factors, uint32_t n_factors, float* oo, float* od, float* owl,
-                            uint32_t* oidx, uint64_t* d_n_kept, void* ws, cudaStream_t stream);
+                            uint32_t* oidx, uint64_t capacity, uint64_t* d_n_kept, void* ws, cudaStream_t stream);
 opx_status launch_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,
                         const float* wl, uint64_t seed, uint64_t* stats, cudaStream_t stream);
 opx_status launch_packet_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,
@@ -109,7 +119,7 @@ void launch_prefilter_scan(uint32_t* counts, uint32_t nb, uint64_t* d_total, cud
 // Cherenkov emission (opx_emit.cu)
 opx_status launch_emit_filtered(const SceneHost& s, const opx_track_steps& st, float n_index, float lambda1, float lambda2, uint64_t n,
                                 uint64_t id_base, uint64_t seed, const uint32_t* factors, uint32_t n_factors, float* o, float* d,
-                                float* wl, uint32_t* oidx, uint64_t* d_n_kept, void* ws, cudaStream_t stream);
+                                float* wl, uint32_t* oidx, uint64_t capacity, uint64_t* d_n_kept, void* ws, cudaStream_t stream);
 opx_status launch_emit(const opx_track_steps& st, float n_index, float lambda1, float lambda2, uint64_t n, uint64_t id_base,
                        uint64_t seed, float* o, float* d, float* wl, cudaStream_t stream);
 

@@ -13,7 +13,8 @@ struct Work { unsigned int nodes = 0, tris = 0; };   // instrumented build only
 
 // ------------------------------------------------------------------------- per-lane traversal
 template <bool kStats>
-__device__ __forceinline__ Hit closest_hit_lane(const SceneDev& sc, const RayW& rw, const Slab& sl, float tmin, int last, Work& work) {
+// e: per-ray slack of the box test (2^-20 |origin|_inf), negligible for origins inside the scene.
+__device__ __forceinline__ Hit closest_hit_lane(const SceneDev& sc, const RayW& rw, const Slab& sl, float e, float tmin, int last, Work& work) {
     Hit h{kInf, -1, 0x7fffffff};
     int stack_ref[kStack];
     float stack_t[kStack];
@@ -26,7 +27,7 @@ __device__ __forceinline__ Hit closest_hit_lane(const SceneDev& sc, const RayW& 
             const float4 q0 = __ldg(&nd->q0), q1 = __ldg(&nd->q1), q2 = __ldg(&nd->q2);
             const int4 q3 = __ldg(&nd->q3);
             float n0, f0, n1, f1;
-            slab2(sl, q0, q1, q2, h.t, n0, f0, n1, f1);
+            slab2_slack(sl, e, q0, q1, q2, h.t, n0, f0, n1, f1);
             const bool hit0 = n0 <= f0, hit1 = n1 <= f1;
             if (hit0 && hit1) {
                 int near = q3.x, far = q3.y;
@@ -75,7 +76,8 @@ __global__ void __launch_bounds__(128) k_propagate_lane(const SceneDev sc, uint6
         const float tmin = p.b == 0 ? 0.f : sc.t_min;
         Hit h;
         if (kBrute) h = closest_hit_brute(sc, rw, tmin, p.last);
-        else h = closest_hit_lane<kStats>(sc, rw, slab_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz), tmin, p.last, work);
+        else h = closest_hit_lane<kStats>(sc, rw, slab_setup(p.ox, p.oy, p.oz, p.dx, p.dy, p.dz),
+                                          fmaxf(fmaxf(fabsf(p.ox), fabsf(p.oy)), fabsf(p.oz)) * 9.5367431640625e-7f, tmin, p.last, work);
         if (kStats) { ++segments; if (h.j >= 0) ++interactions; }
         if (!interact(sc, h, rw, p, seed)) break;
     }

@@ -1,7 +1,8 @@
 // k_propagate_packet: the product kernel for A5-A10.
 //
 // One CTA owns a tile of kTile consecutive photons:
-//   1. stage   the tile's inputs are copied to shared memory with coalesced streaming loads;
+//   1. stage   the tile's inputs are copied to shared memory by three TMA bulk copies (cp.async.bulk) that one thread
+//              issues (a ragged or misaligned tile falls back to coalesced streaming loads);
 //   2. sort    photons are ordered by a 12-bit pseudo-angle of their direction about the tile's mean
 //              direction (Cherenkov photons of a track lie on a cone = a ring in the octahedral
 //              plane), with a 2-pass 6-bit radix sort in shared memory;
@@ -11,8 +12,8 @@
 //              of its lanes (entry k in lane k, read back with a shuffle; entries >= 32 overflow to
 //              shared memory).  Each lane still intersects its own ray against every triangle the
 //              packet reaches, so results are exactly the per-photon results of DESIGN.md section 2;
-//   4. store   records are written back into the photon's own shared-memory slot and the tile is
-//              written out with coalesced streaming stores.
+//   4. store   records are written back into the photon's own shared-memory slot and the tile leaves by six TMA bulk
+//              stores (or coalesced streaming stores for a ragged / misaligned tile).
 #pragma once
 #include "opx_beam.cuh"
 #include "opx_device.cuh"
@@ -182,8 +183,9 @@ constexpr int kDone = 0x7fffffff;
 
 // Walks internal nodes from `ref` until the packet reaches a leaf (returns its ref < 0) or the
 // traversal is finished (returns kDone).  This small loop is the only code specialised per octant.
+// kOct = 9: generic test with per-ray slack `e` (some lane's origin lies beyond SceneDev::origin_limit).
 template <int kOct>
-__device__ __forceinline__ int descend(const SceneDev& sc, const Slab& sl, float tcap, int ref, PacketStack& st, int lane, int* s_stack) {
+__device__ __forceinline__ int descend(const SceneDev& sc, const Slab& sl, float e, float tcap, int ref, PacketStack& st, int lane, int* s_stack) {
     for (;;) {
         if (ref < 0) return ref;
         const NodeDev* nd = sc.nodes + ref;
@@ -191,7 +193,8 @@ __device__ __forceinline__ int descend(const SceneDev& sc, const Slab& sl, float
         const int4 q3 = __ldg(&nd->q3);
         float n0, f0, n1, f1;
         if (kOct < 8) slab2_oct<kOct>(sl, q0, q1, q2, tcap, n0, f0, n1, f1);
-        else slab2(sl, q0, q1, q2, tcap, n0, f0, n1, f1);
+        else if (kOct == 8) slab2(sl, q0, q1, q2, tcap, n0, f0, n1, f1);
+        else slab2_slack(sl, e, q0, q1, q2, tcap, n0, f0, n1, f1);
         const bool hit0 = n0 <= f0, hit1 = n1 <= f1;
         const unsigned b0 = __ballot_sync(0xffffffffu, hit0), b1 = __ballot_sync(0xffffffffu, hit1);
         if (b0 && b1) {
@@ -212,8 +215,9 @@ __device__ __forceinline__ int descend(const SceneDev& sc, const Slab& sl, float
     }
 }
 
-// `oct` (warp-uniform) = 0..7: every alive lane's direction lies in that sign octant; 8: mixed signs.
-__device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW& rw, const Slab& sl, float tmin, int last,
+// `oct` (warp-uniform) = 0..7: every alive lane's direction lies in that sign octant; 8: mixed signs; 9: mixed signs and
+// per-ray slack e (an origin beyond SceneDev::origin_limit).
+__device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW& rw, const Slab& sl, float e, float tmin, int last,
                                                   bool alive, int lane, int* s_stack, int oct) {
     Hit h{kInf, -1, 0x7fffffff};
     float tcap = alive ? kInf : -1.f;
@@ -221,15 +225,16 @@ __device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW
     int ref = 0;
     for (;;) {
         switch (oct) {
-            case 0: ref = descend<0>(sc, sl, tcap, ref, st, lane, s_stack); break;
-            case 1: ref = descend<1>(sc, sl, tcap, ref, st, lane, s_stack); break;
-            case 2: ref = descend<2>(sc, sl, tcap, ref, st, lane, s_stack); break;
-            case 3: ref = descend<3>(sc, sl, tcap, ref, st, lane, s_stack); break;
-            case 4: ref = descend<4>(sc, sl, tcap, ref, st, lane, s_stack); break;
-            case 5: ref = descend<5>(sc, sl, tcap, ref, st, lane, s_stack); break;
-            case 6: ref = descend<6>(sc, sl, tcap, ref, st, lane, s_stack); break;
-            case 7: ref = descend<7>(sc, sl, tcap, ref, st, lane, s_stack); break;
-            default: ref = descend<8>(sc, sl, tcap, ref, st, lane, s_stack); break;
+            case 0: ref = descend<0>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
+            case 1: ref = descend<1>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
+            case 2: ref = descend<2>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
+            case 3: ref = descend<3>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
+            case 4: ref = descend<4>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
+            case 5: ref = descend<5>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
+            case 6: ref = descend<6>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
+            case 7: ref = descend<7>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
+            case 8: ref = descend<8>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
+            default: ref = descend<9>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
         }
         if (ref == kDone) break;
         consider(sc, rw, ~ref, tmin, last, h);
@@ -411,12 +416,15 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
                 if (kStats) ++bstats.fallback_segments;
                 const float ox = so[0], oy = so[1], oz = so[2], dx = sd[0], dy = sd[1], dz = sd[2];
                 const Slab sl = slab_setup(ox, oy, oz, dx, dy, dz);
-                // sign octant of the packet: specialised traversal when all alive lanes agree
-                const int oct = (dx < 0.f ? 1 : 0) | (dy < 0.f ? 2 : 0) | (dz < 0.f ? 4 : 0);
+                // sign octant of the packet (from the sign bits, as slab_rcp keeps them): specialised traversal when all alive
+                // lanes agree; an origin beyond origin_limit widens every box by its own rounding slack instead (8.2)
+                const int oct = dir_octant(dx, dy, dz);
                 const unsigned am = __ballot_sync(0xffffffffu, alive);
                 const int oct0 = __shfl_sync(0xffffffffu, oct, __ffs(am) - 1);
                 const bool uni = __all_sync(0xffffffffu, !alive || oct == oct0);
-                h = closest_hit_packet(sc, rw, sl, tmin, last, alive, lane, sm.stack[w], uni ? oct0 : 8);
+                const float far_o = fmaxf(fmaxf(fabsf(ox), fabsf(oy)), fabsf(oz));
+                const bool far = __any_sync(0xffffffffu, alive && !(far_o < sc.origin_limit));
+                h = closest_hit_packet(sc, rw, sl, far_o * 9.5367431640625e-7f, tmin, last, alive, lane, sm.stack[w], far ? 9 : (uni ? oct0 : 8));
             }
             if (alive) {
                 Photon p;

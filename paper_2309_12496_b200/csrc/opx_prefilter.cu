@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(kFThreads) k_prefilter_compact(uint64_t n, con
                                                                  const float* __restrict__ wl, const uint32_t* __restrict__ words,
                                                                  const uint32_t* __restrict__ block_offset, float* __restrict__ oo,
                                                                  float* __restrict__ od, float* __restrict__ owl,
-                                                                 uint32_t* __restrict__ oidx) {
+                                                                 uint32_t* __restrict__ oidx, uint64_t capacity) {
     __shared__ uint32_t s_mask[kWords];
     __shared__ uint32_t s_pre[kWords];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -108,6 +108,7 @@ __global__ void __launch_bounds__(kFThreads) k_prefilter_compact(uint64_t n, con
         if (!((mask >> lane) & 1u)) continue;
         const uint64_t i = blk_base + (uint64_t)(wi * 32 + lane);
         const uint64_t q = off + s_pre[wi] + __popc(mask & ((1u << lane) - 1u));
+        if (q >= capacity) continue;      // the out arrays are full: *d_n_kept still holds the true count
         const float ox = __ldcs(o + 3 * i), oy = __ldcs(o + 3 * i + 1), oz = __ldcs(o + 3 * i + 2);
         const float dx = __ldcs(d + 3 * i), dy = __ldcs(d + 3 * i + 1), dz = __ldcs(d + 3 * i + 2);
         oo[3 * q] = ox; oo[3 * q + 1] = oy; oo[3 * q + 2] = oz;
@@ -130,7 +131,7 @@ size_t prefilter_workspace_bytes(uint64_t n) {
 
 opx_status launch_prefilter(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d, const float* wl,
                             uint64_t seed, const uint32_t* factors, uint32_t n_factors, float* oo, float* od, float* owl,
-                            uint32_t* oidx, uint64_t* d_n_kept, void* ws, cudaStream_t stream) {
+                            uint32_t* oidx, uint64_t capacity, uint64_t* d_n_kept, void* ws, cudaStream_t stream) {
     Factors fa{};
     fa.n = n_factors;
     for (uint32_t k = 0; k < n_factors; ++k) { fa.m[k] = factors[k]; fa.mk[k] = s.mat_kinds[factors[k]]; }
@@ -139,7 +140,7 @@ opx_status launch_prefilter(const SceneHost& s, uint64_t n, uint64_t id_base, co
     uint32_t* counts = (uint32_t*)((char*)ws + align_up((size_t)nb * kWords * 4, 256));
     k_prefilter_mark<<<(unsigned)nb, kFThreads, 0, stream>>>(s.dev, fa, n, id_base, wl, seed, words, counts);
     k_prefilter_scan<<<1, 1024, 0, stream>>>(counts, (uint32_t)nb, (unsigned long long*)d_n_kept);
-    k_prefilter_compact<<<(unsigned)nb, kFThreads, 0, stream>>>(n, o, d, wl, words, counts, oo, od, owl, oidx);
+    k_prefilter_compact<<<(unsigned)nb, kFThreads, 0, stream>>>(n, o, d, wl, words, counts, oo, od, owl, oidx, capacity);
     count_launch(3);
     return check_cuda(cudaGetLastError(), "prefilter launch");
 }

@@ -2,18 +2,46 @@
 //   k_propagate_packet (opx_packet.cuh)  the product kernel: tile-sorted photons, warp-packet traversal
 //   k_propagate_lane   (opx_lane.cuh)    per-thread traversal: instrumented / brute-force / tiny scenes
 //   k_bin              (opx_bin.cuh)     A11 hit binning with warp-aggregated atomics + A12 counters
+#include <atomic>
+
 #include "opx_bin.cuh"
 #include "opx_lane.cuh"
 #include "opx_packet.cuh"
 
 namespace opx {
 
-static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
+using Big = PacketSmemT<512, 4>;      // 2048-photon tiles, 4 packets per warp: the general shape
+using Small = PacketSmemT<512, 1>;    // 512-photon tiles, 1 packet per warp: calls too small to fill the machine
+using Mid = PacketSmemT<256, 4>;      // 1024-photon tiles, 4 CTAs/SM: filtered streams on large scenes
+using Lean = PacketSmemT<448, 4>;     // 1792-photon tiles, 72 registers: in-flight calls on small scenes
+
+// The dynamic shared memory limit of a kernel is an attribute per device (context): set once per device, at the first
+// opx_bvh_build or launch on it, so that a later opx_propagate performs stream operations only (CUDA-graph capturable).
+opx_status configure_device() {
+    static std::atomic<uint64_t> done{0};
+    int dev = 0;
+    if (opx_status st = check_cuda(cudaGetDevice(&dev), "cudaGetDevice")) return st;
+    const uint64_t bit = 1ull << (dev & 63);
+    if (done.load(std::memory_order_acquire) & bit) return OPX_OK;
+    cudaError_t e = cudaSuccess;
+    if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
+    if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
+    if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 1, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Small));
+    if (!e) e = cudaFuncSetAttribute(k_propagate_packet<448, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Lean));
+    if (!e) e = cudaFuncSetAttribute(k_propagate_packet<256, 4, 4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Mid));
+    if (opx_status st = check_cuda(e, "cudaFuncSetAttribute")) return st;
+    done.fetch_or(bit, std::memory_order_release);      // two threads racing here both set the same attributes: harmless
+    return OPX_OK;
+}
+
+static opx_status launch_propagate_impl(const SceneHost& s, WalkMode mode, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
                                         const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_hits& out,
                                         uint32_t* hitmap, uint64_t* counters, uint64_t* packet_stats, cudaStream_t stream) {
     SceneDev dev = s.dev;          // per-launch copy: flags and the optional device-side count ride in the kernel parameter
     dev.flags = flags;
     dev.d_n = (const unsigned long long*)d_n;
+    if (mode == kWalkBinary) dev.n_wnodes = 0;      // debug: packets walk the binary tree only
+    const bool brute = mode == kWalkBrute;
     cudaEvent_t* ev = nullptr;
     if (s.prof_used < s.prof_max) { ev = &s.prof_events[3 * (size_t)s.prof_used]; ++s.prof_used; }
     if (ev) cudaEventRecord(ev[0], stream);
@@ -23,31 +51,17 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
         const uint64_t blocks = (n + 127) / 128;
         if (blocks > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
         k_propagate_lane<true, false><<<(unsigned)blocks, 128, 0, stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr);
+        set_last_kernel("k_propagate_lane<1, 0>");
     } else {
         // tile size: 2048 photons (4 packets per warp) unless the call is small; then 512 photons (1 packet per warp)
-        using Big = PacketSmemT<512, 4>;
-        using Small = PacketSmemT<512, 1>;
-        // a filtered stream (NO_EFFICIENCY: 1 photon in 7-9 survives, so packets are wide and walk more nodes) on a large
-        // scene runs 22 % faster with 4 CTAs of 256 threads per SM (1024-photon tiles) than with 2 x 512: its packets differ
-        // widely in cost, and a tile's warps wait at its barrier for the slowest packet, so finer tiles waste fewer warp
-        // slots (384 x 3: +14 %, 128 x 8: -15 %); everything else is faster with 2 x 512 (more photons per ring in a tile:
-        // C4 in flight -10 %, toy-scene pipeline -23 % with the finer shapes)
-        using Mid = PacketSmemT<256, 4>;
-        // a small scene (its BVH lives in L1/L2: the walk is issue-bound, not latency-bound) traced in flight runs 3 % faster
-        // with 448 threads x 2 CTAs, which leaves 72 registers per thread and removes the spills of the 64-register build
-        // (C4 scene: -3.5 %, filtered toy-scene stream: -5 %, so those keep 512 x 2)
-        using Lean = PacketSmemT<448, 4>;
-        static bool configured = false;
-        if (!configured) {
-            cudaError_t e = cudaSuccess;
-            if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
-            if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
-            if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 1, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Small));
-            if (!e) e = cudaFuncSetAttribute(k_propagate_packet<448, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Lean));
-            if (!e) e = cudaFuncSetAttribute(k_propagate_packet<256, 4, 4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Mid));
-            if (opx_status st = check_cuda(e, "cudaFuncSetAttribute")) return st;
-            configured = true;
-        }
+        // Shapes (defined at the top of this file).  A filtered stream (NO_EFFICIENCY: 1 photon in 7-9 survives, so packets are
+        // wide and walk more nodes) on a large scene runs 22 % faster with 4 CTAs of 256 threads per SM (1024-photon tiles) than
+        // with 2 x 512: its packets differ widely in cost, and a tile's warps wait at its barrier for the slowest packet, so
+        // finer tiles waste fewer warp slots (384 x 3: +14 %, 128 x 8: -15 %); everything else is faster with 2 x 512 (more
+        // photons per ring in a tile: C4 in flight -10 %, toy-scene pipeline -23 % with the finer shapes).  A small scene (its
+        // BVH lives in L1/L2: the walk is issue-bound, not latency-bound) traced in flight runs 3 % faster with 448 threads x
+        // 2 CTAs, which leaves 72 registers per thread (C4 scene: -3.5 %, filtered toy-scene stream: -5 %: those keep 512 x 2).
+        if (opx_status st = configure_device()) return st;
         // measured crossover (kernel time vs n, both tile sizes): on a small scene the 512-photon tiles win while they
         // number at most one per SM (n < 148 x 512), on a large scene (longer, latency-bound packets) up to about 2e5 photons
         const uint64_t small_below = s.dev.n_tri < (1u << 18) ? 148ull * Small::kTile : 100ull * Big::kTile;
@@ -62,6 +76,9 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
         else if (mid) k_propagate_packet<256, 4, 4, false><<<(unsigned)tiles, 256, sizeof(Mid), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
         else if (small) k_propagate_packet<512, 1, 2, false><<<(unsigned)tiles, 512, sizeof(Small), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
         else k_propagate_packet<512, 4, 2, false><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
+        // the names ncu prints for these instantiations
+        set_last_kernel(packet_stats ? "k_propagate_packet<512, 4, 2, 1>" : lean ? "k_propagate_packet<448, 4, 2, 0>" : mid ? "k_propagate_packet<256, 4, 4, 0>"
+                        : small ? "k_propagate_packet<512, 1, 2, 0>" : "k_propagate_packet<512, 4, 2, 0>");
         binned = !packet_stats;
     }
     count_launch(1);
@@ -76,16 +93,16 @@ static opx_status launch_propagate_impl(const SceneHost& s, bool brute, uint64_t
     return check_cuda(cudaGetLastError(), "propagate launch");
 }
 
-opx_status launch_propagate(const SceneHost& s, bool brute, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
+opx_status launch_propagate(const SceneHost& s, WalkMode mode, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
                             const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_hits& out, uint32_t* hitmap,
                             uint64_t* counters, cudaStream_t stream) {
-    return launch_propagate_impl(s, brute, n, d_n, id_base, o, d, wl, seed, flags, out, hitmap, counters, nullptr, stream);
+    return launch_propagate_impl(s, mode, n, d_n, id_base, o, d, wl, seed, flags, out, hitmap, counters, nullptr, stream);
 }
 
 opx_status launch_packet_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,
                                const float* wl, uint64_t seed, const opx_hits& out, uint64_t* stats, cudaStream_t stream) {
     if (s.dev.n_tri < 2) return fail(OPX_ERR_BAD_STATE, "no hierarchy to instrument (fewer than two triangles)");
-    return launch_propagate_impl(s, false, n, nullptr, id_base, o, d, wl, seed, 0u, out, nullptr, nullptr, stats, stream);
+    return launch_propagate_impl(s, kWalkProduct, n, nullptr, id_base, o, d, wl, seed, 0u, out, nullptr, nullptr, stats, stream);
 }
 
 opx_status launch_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d, const float* wl,

@@ -21,12 +21,14 @@ OPX_OK, OPX_ERR_INVALID_ARG, OPX_ERR_BAD_STATE, OPX_ERR_WORKSPACE_TOO_SMALL, OPX
 FLAG_NO_EFFICIENCY = 1                   # opx_flags
 TABLE_LINEAR, TABLE_HISTOGRAM = 0, 1     # opx_table_interp
 
+# the product boundary (include/opx.h) ...
 EXPORTS = ("opx_scene_create", "opx_scene_workspace_bytes", "opx_bvh_build", "opx_propagate",
-           "opx_propagate_flags", "opx_prefilter_workspace_bytes", "opx_prefilter", "opx_emit_cherenkov", "opx_emit_cherenkov_filtered", "opx_propagate_brute", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
-           "opx_profile_begin", "opx_profile_end", "opx_propagate_stats", "opx_propagate_packet_stats",
-           "opx_scene_wide_info", "opx_measure_fp32_peak",
-           "opx_scene_info", "opx_scene_get_layout", "opx_launch_count", "opx_scene_destroy",
-           "opx_last_error", "opx_version")
+           "opx_propagate_flags", "opx_prefilter_workspace_bytes", "opx_prefilter", "opx_emit_cherenkov",
+           "opx_emit_cherenkov_filtered", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
+           "opx_scene_info", "opx_scene_get_layout", "opx_scene_destroy", "opx_last_error", "opx_version")
+# ... and the debugging / measurement exports (include/opx_debug.h) that tests and bench.py use
+DEBUG_EXPORTS = ("opx_propagate_brute", "opx_propagate_binary", "opx_profile_begin", "opx_profile_end", "opx_propagate_stats",
+                 "opx_propagate_packet_stats", "opx_scene_wide_info", "opx_measure_fp32_peak", "opx_launch_count", "opx_last_kernel")
 
 
 class OpxError(RuntimeError):
@@ -88,17 +90,18 @@ def load_library(path=LIB_PATH):
     lib.opx_last_error.restype = C.c_char_p
     lib.opx_version.restype = C.c_char_p
     lib.opx_launch_count.restype = u64
+    lib.opx_last_kernel.restype = C.c_char_p
     lib.opx_scene_create.argtypes = [vp, vp, u32, vp, u32, vp, u32, vp]
     lib.opx_scene_workspace_bytes.argtypes = [vp, vp, vp]
     lib.opx_bvh_build.argtypes = [vp, vp, C.c_size_t, vp, C.c_size_t, vp]
-    for f in (lib.opx_propagate, lib.opx_propagate_brute):
+    for f in (lib.opx_propagate, lib.opx_propagate_brute, lib.opx_propagate_binary):
         f.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp, vp, vp]
     lib.opx_propagate_flags.argtypes = [vp, u64, vp, u64, vp, vp, vp, u64, u32, vp, vp, vp, vp]
     lib.opx_prefilter_workspace_bytes.argtypes = [u64, vp]
-    lib.opx_prefilter.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, u32, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    lib.opx_prefilter.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, u32, vp, vp, vp, vp, u64, vp, vp, C.c_size_t, vp]
     lib.opx_emit_cherenkov.argtypes = [vp, u64, C.c_float, C.c_float, C.c_float, u64, u64, u64, vp, vp, vp, vp]
     lib.opx_emit_cherenkov_filtered.argtypes = [vp, vp, u64, C.c_float, C.c_float, C.c_float, u64, u64, u64, vp, u32,
-                                                vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+                                                vp, vp, vp, vp, u64, vp, vp, C.c_size_t, vp]
     lib.opx_propagate_host_workspace_bytes.argtypes = [vp, u64, vp]
     lib.opx_propagate_host.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp, vp, vp, C.c_size_t, u64, vp]
     lib.opx_profile_begin.argtypes = [vp, u32]
@@ -158,6 +161,11 @@ def emit_cherenkov(dev_steps, n, photon_id_base=0, seed=0, n_index=1.0014, lambd
 
 def launch_count():
     return int(load_library().opx_launch_count())
+
+
+def last_kernel():
+    """opx_last_kernel: the propagation-kernel instantiation the last propagate call of this thread launched."""
+    return load_library().opx_last_kernel().decode()
 
 
 def _np_ptr(a):
@@ -254,11 +262,11 @@ class Scene:
                 torch.zeros(8, dtype=torch.int64, device=device))
 
     def propagate(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, records=None, hitmap=None,
-                  counters=None, stream=None, brute=False, flags=0, n_dev=None):
+                  counters=None, stream=None, brute=False, flags=0, n_dev=None, binary=False):
         """opx_propagate on device tensors.  hitmap (int32 view of uint32) and counters (int64 view of
         uint64) are accumulated into; pass zeroed tensors or None to have them created.
         flags / n_dev (int64 CUDA tensor of one element: photon count left on the device by prefilter)
-        select opx_propagate_flags."""
+        select opx_propagate_flags.  brute / binary select the debug walks of include/opx_debug.h."""
         import torch
         n = int(wavelengths.shape[0])
         for t, shape in ((origins, (n, 3)), (dirs, (n, 3)), (wavelengths, (n,))):
@@ -274,32 +282,35 @@ class Scene:
         h = Hits(*(records[k].data_ptr() for k in ("pos", "dir", "pixel", "surface", "state", "bounces")))
         st = stream if stream is not None else torch.cuda.current_stream(dev)
         if flags or n_dev is not None:
-            if brute:
-                raise OpxError(OPX_ERR_INVALID_ARG, "opx_propagate_brute takes no flags")
+            if brute or binary:
+                raise OpxError(OPX_ERR_INVALID_ARG, "the debug walks take no flags")
             _check(load_library().opx_propagate_flags(
                 self._h, n, None if n_dev is None else n_dev.data_ptr(), int(photon_id_base), origins.data_ptr(),
                 dirs.data_ptr(), wavelengths.data_ptr(), int(seed), int(flags), C.byref(h), hitmap.data_ptr(),
                 counters.data_ptr(), C.c_void_p(st.cuda_stream)))
         else:
-            fn = load_library().opx_propagate_brute if brute else load_library().opx_propagate
+            lib = load_library()
+            fn = lib.opx_propagate_brute if brute else (lib.opx_propagate_binary if binary else lib.opx_propagate)
             _check(fn(self._h, n, int(photon_id_base), origins.data_ptr(), dirs.data_ptr(), wavelengths.data_ptr(),
                       int(seed), C.byref(h), hitmap.data_ptr(), counters.data_ptr(), C.c_void_p(st.cuda_stream)))
         out = dict(records)
         out["hitmap"], out["counters"] = hitmap[:self.n_pixels], counters
         return out
 
-    def prefilter(self, origins, dirs, wavelengths, factors, seed=0, photon_id_base=0, out=None, stream=None):
+    def prefilter(self, origins, dirs, wavelengths, factors, seed=0, photon_id_base=0, out=None, stream=None, capacity=None):
         """opx_prefilter on device tensors -> dict(origins, dirs, wavelengths, index (int32 view of uint32),
         n_kept (int64 CUDA tensor of one element)); the first n_kept entries of the arrays are the survivors in
-        input order.  No host synchronisation: pass out["n_kept"] as `n_dev` to propagate()."""
+        input order.  No host synchronisation: pass out["n_kept"] as `n_dev` to propagate().  capacity (default n)
+        sizes the output arrays; n_kept > capacity means the list was truncated."""
         import torch
         n = int(wavelengths.shape[0])
         dev = wavelengths.device
         if out is None:
-            out = dict(origins=torch.empty((n, 3), dtype=torch.float32, device=dev),
-                       dirs=torch.empty((n, 3), dtype=torch.float32, device=dev),
-                       wavelengths=torch.empty(n, dtype=torch.float32, device=dev),
-                       index=torch.empty(n, dtype=torch.int32, device=dev),
+            cap = int(n if capacity is None else capacity)
+            out = dict(origins=torch.empty((cap, 3), dtype=torch.float32, device=dev),
+                       dirs=torch.empty((cap, 3), dtype=torch.float32, device=dev),
+                       wavelengths=torch.empty(cap, dtype=torch.float32, device=dev),
+                       index=torch.empty(cap, dtype=torch.int32, device=dev),
                        n_kept=torch.zeros(1, dtype=torch.int64, device=dev))
         need = C.c_size_t()
         _check(load_library().opx_prefilter_workspace_bytes(n, C.byref(need)))
@@ -312,8 +323,8 @@ class Scene:
         _check(load_library().opx_prefilter(
             self._h, n, int(photon_id_base), origins.data_ptr(), dirs.data_ptr(), wavelengths.data_ptr(), int(seed),
             fac, len(factors), out["origins"].data_ptr(), out["dirs"].data_ptr(), out["wavelengths"].data_ptr(),
-            None if idx is None else idx.data_ptr(), out["n_kept"].data_ptr(), _aligned(ws), need.value,
-            C.c_void_p(st.cuda_stream)))
+            None if idx is None else idx.data_ptr(), int(out["wavelengths"].shape[0]), out["n_kept"].data_ptr(), _aligned(ws),
+            need.value, C.c_void_p(st.cuda_stream)))
         return out
 
     def emit_cherenkov_filtered(self, dev_steps, n, factors, photon_id_base=0, seed=0, n_index=1.0014, lambda1=200.0,
@@ -342,7 +353,8 @@ class Scene:
         _check(load_library().opx_emit_cherenkov_filtered(
             self._h, C.byref(st), int(dev_steps["n_total"]), n_index, lambda1, lambda2, int(n), int(photon_id_base), int(seed),
             fac, len(factors), out["origins"].data_ptr(), out["dirs"].data_ptr(), out["wavelengths"].data_ptr(),
-            None if idx is None else idx.data_ptr(), out["n_kept"].data_ptr(), _aligned(ws), need.value, C.c_void_p(s.cuda_stream)))
+            None if idx is None else idx.data_ptr(), int(out["wavelengths"].shape[0]), out["n_kept"].data_ptr(), _aligned(ws),
+            need.value, C.c_void_p(s.cuda_stream)))
         return out
 
     def profile_begin(self, max_calls):

@@ -26,7 +26,10 @@ def test_every_declared_symbol_is_exported(lib):
     header = open(os.path.join(ROOT, "include", "opx.h")).read()
     declared = set(re.findall(r"\b(opx_[a-z0-9_]+)\s*\(", header))
     assert declared == set(pkg.EXPORTS)
-    for name in declared:
+    # the debugging / measurement exports live in their own header, outside the product boundary
+    debug = set(re.findall(r"\b(opx_[a-z0-9_]+)\s*\(", open(os.path.join(ROOT, "include", "opx_debug.h")).read()))
+    assert debug == set(pkg.DEBUG_EXPORTS) and not (debug & declared)
+    for name in declared | debug:
         assert hasattr(lib, name), name
     assert lib.opx_version().decode().startswith("opx")
     assert lib.opx_last_error() is not None

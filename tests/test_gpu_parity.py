@@ -187,7 +187,7 @@ def _check_lbvh(sc, gs):
     base = (ws.data_ptr() + 255) // 256 * 256 - ws.data_ptr()
     raw = ws.cpu().numpy()[base:]
     keys = raw[lay["sorted_keys"]:lay["sorted_keys"] + 8 * T].view(np.uint64)
-    assert np.all(keys[1:] >= keys[:-1])                                      # sorted keys (63-bit Morton + size-class bit)
+    assert np.all(keys[1:] >= keys[:-1])                                      # sorted 63-bit Morton keys
     tris = raw[lay["triangles"]:lay["triangles"] + 48 * T].view(np.float32).reshape(T, 3, 4)
     gid = tris[:, 0, 3].view(np.int32)
     assert np.array_equal(np.sort(gid), np.arange(T))                          # a permutation: each triangle in one leaf
