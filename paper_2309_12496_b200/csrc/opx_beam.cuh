@@ -42,7 +42,7 @@ struct Beam {
     float tlo;
 };
 
-struct BeamStats { unsigned visits = 0, tris = 0, beam_segments = 0, fallback_segments = 0, overflows = 0, culls = 0; };
+struct BeamStats { unsigned visits = 0, tris = 0, beam_segments = 0, fallback_segments = 0, overflows = 0, culls = 0, cands = 0, pairs = 0; };
 
 __device__ __forceinline__ int f2ordi(float f) { const int i = __float_as_int(f); return i ^ ((i >> 31) & 0x7fffffff); }
 __device__ __forceinline__ float ordi2f(int i) { return __int_as_float(i ^ ((i >> 31) & 0x7fffffff)); }
@@ -162,6 +162,7 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayW&
         const unsigned mt = __ballot_sync(full, hit && cref < 0);
         if (mt) {
             unsigned mine = mt;                      // the triangle children this lane still has to test
+            if (kStats) stats.cands += __popc(mt);
             const bool culled = !kMixed && __popc(mt) >= kCullMin;       // warp-uniform
             if (culled) {
                 // per-lane cull: own ray against the candidate boxes (all member rays share the beam's sign octant, so
@@ -183,6 +184,7 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayW&
                     if (en <= exi) mine |= 1u << L;
                 } while (m);
             }
+            if (kStats) stats.pairs += __reduce_add_sync(full, alive ? (unsigned)__popc(mine) : 0u);
             if (!culled) {
                 // no per-lane cull (warp-uniform): one uniform pass over the candidates, no votes, no per-lane bit scans
                 unsigned m = mt;

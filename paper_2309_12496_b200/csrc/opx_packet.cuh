@@ -224,18 +224,7 @@ __device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW
     PacketStack st;
     int ref = 0;
     for (;;) {
-        switch (oct) {
-            case 0: ref = descend<0>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
-            case 1: ref = descend<1>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
-            case 2: ref = descend<2>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
-            case 3: ref = descend<3>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
-            case 4: ref = descend<4>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
-            case 5: ref = descend<5>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
-            case 6: ref = descend<6>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
-            case 7: ref = descend<7>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
-            case 8: ref = descend<8>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
-            default: ref = descend<9>(sc, sl, e, tcap, ref, st, lane, s_stack); break;
-        }
+        ref = oct == 9 ? descend<9>(sc, sl, e, tcap, ref, st, lane, s_stack) : descend<8>(sc, sl, e, tcap, ref, st, lane, s_stack);
         if (ref == kDone) break;
         consider(sc, rw, ~ref, tmin, last, h);
         if (alive) tcap = h.t;
@@ -450,6 +439,7 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
             atomicAdd(&stats[0], (unsigned long long)bstats.beam_segments); atomicAdd(&stats[1], (unsigned long long)bstats.fallback_segments);
             atomicAdd(&stats[2], (unsigned long long)bstats.visits); atomicAdd(&stats[3], (unsigned long long)bstats.tris);
             atomicAdd(&stats[4], (unsigned long long)bstats.overflows); atomicAdd(&stats[5], (unsigned long long)bstats.culls);
+            atomicAdd(&stats[6], (unsigned long long)bstats.cands); atomicAdd(&stats[7], (unsigned long long)bstats.pairs);
         }
     }
 
