@@ -151,7 +151,7 @@ typedef struct {
  * and copies tables and frames.  Host only; no CUDA call.
  * Errors: NULL pointers, n_lambda < 2, lambda_max <= lambda_min, max_bounces outside 1..255,
  * negative t_min, material / frame / vertex index out of range, detector mesh without a frame,
- * non-positive pitch, zero-sized pixel grid, table value outside [0,1] or NaN, more than 2^30
+ * non-positive pitch, zero-sized pixel grid, table value outside [0,1] or NaN, more than 2^28
  * triangles => OPX_ERR_INVALID_ARG.  n_meshes = 0 (an empty scene) is valid. */
 opx_status opx_scene_create(const opx_scene_params* params, const opx_mesh* meshes, uint32_t n_meshes,
                             const opx_material* materials, uint32_t n_materials,

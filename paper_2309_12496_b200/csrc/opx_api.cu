@@ -130,7 +130,7 @@ opx_status opx_scene_create(const opx_scene_params* params, const opx_mesh* mesh
     }
     uint64_t total = 0;
     for (uint32_t k = 0; k < n_meshes; ++k) total += meshes[k].n_triangles;
-    if (total > (1ull << 30)) { return bail("too many triangles (limit 2^30)"); }
+    if (total > (1ull << 28)) { return bail("too many triangles (limit 2^28: 32-bit offsets into the three rotations of the triangle array)"); }
     s->tri.reserve(total * 9);
     s->tri_surface.reserve(total);
     s->surfaces.resize(n_meshes);

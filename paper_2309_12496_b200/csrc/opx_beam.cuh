@@ -31,6 +31,10 @@ constexpr int kBeamStack = 64;            // per warp, in shared memory; overflo
 #define OPX_CULL_MIN 4
 #endif
 constexpr int kCullMin = OPX_CULL_MIN;   // per-lane cull when the beam enters at least this many triangle boxes of a node
+#ifndef OPX_CULL_SLOTS
+#define OPX_CULL_SLOTS 16
+#endif
+constexpr int kCullSlots = OPX_CULL_SLOTS;   // candidate boxes a warp stages in shared memory per culling round
 
 struct Beam {
     // entry bound of axis a: fma(near_a, rn_a, cn_a); exit bound: fma(far_a, rf_a, cf_a), where
@@ -130,10 +134,13 @@ __device__ __forceinline__ bool beam_setup(const SceneDev& sc, float ox, float o
 // stack overflowed: the caller then redoes the segment with the binary packet walk.
 // (so, sd) point at the lane's own segment in shared memory (origin, direction; not re-based): the per-lane cull
 // reads it back from there, so the segment does not occupy registers during the walk.
+// s_cb: 2 x kCullSlots float4 of the warp: the candidate boxes of the node being culled, (near planes, child ref) and
+// (far planes, -), written by the lanes that own the candidates and read back by every lane with uniform addresses
+// (two broadcast 16-byte loads per candidate instead of six shuffles).
 template <bool kMixed, bool kStats>
-__device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayW& rw, const Beam& bm, float s, float tmin, int last,
+__device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayR& rr, const Beam& bm, float s, float tmin, int last_j,
                                                  bool alive, int lane, const float* so, const float* sd,
-                                                 int* s_ref, float* s_tn, Hit& h, BeamStats& stats) {
+                                                 int* s_ref, float* s_tn, float4* s_cb, Hit& h, BeamStats& stats) {
     const unsigned full = 0xffffffffu;
     h = Hit{kInf, -1, 0x7fffffff};
     float thi = kInf;
@@ -161,49 +168,56 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayW&
         const bool hit = tn <= tf;
         const unsigned mt = __ballot_sync(full, hit && cref < 0);
         if (mt) {
-            unsigned mine = mt;                      // the triangle children this lane still has to test
             if (kStats) stats.cands += __popc(mt);
-            const bool culled = !kMixed && __popc(mt) >= kCullMin;       // warp-uniform
-            if (culled) {
-                // per-lane cull: own ray against the candidate boxes (all member rays share the beam's sign octant, so
-                // near/far are the same planes for every lane).  Approximate reciprocals: see slab_setup.
-                if (kStats) ++stats.culls;
-                const float ix = rcp_approx(sd[0]), iy = rcp_approx(sd[1]), iz = rcp_approx(sd[2]);
-                const float qx = -so[0] * ix, qy = -so[1] * iy, qz = -so[2] * iz;
-                const float cap = alive ? h.t : -1.f;
-                mine = 0u;
-                unsigned m = mt;
-                do {
-                    const int L = __ffs(m) - 1;
-                    m &= m - 1;
-                    const float e0 = __fmaf_rn(__shfl_sync(full, nx, L), ix, qx), e1 = __fmaf_rn(__shfl_sync(full, ny, L), iy, qy),
-                                e2 = __fmaf_rn(__shfl_sync(full, nz, L), iz, qz);
-                    const float x0 = __fmaf_rn(__shfl_sync(full, fx, L), ix, qx), x1 = __fmaf_rn(__shfl_sync(full, fy, L), iy, qy),
-                                x2 = __fmaf_rn(__shfl_sync(full, fz, L), iz, qz);
-                    const float en = fmaxf(fmaxf(e0, e1), fmaxf(e2, 0.f)), exi = fminf(fminf(x0, x1), fminf(x2, cap));
-                    if (en <= exi) mine |= 1u << L;
-                } while (m);
-            }
-            if (kStats) stats.pairs += __reduce_add_sync(full, alive ? (unsigned)__popc(mine) : 0u);
-            if (!culled) {
+            if (kMixed || __popc(mt) < kCullMin) {
                 // no per-lane cull (warp-uniform): one uniform pass over the candidates, no votes, no per-lane bit scans
+                if (kStats) stats.pairs += __popc(mt) * __popc(__ballot_sync(full, alive));
                 unsigned m = mt;
                 do {
                     const int L = __ffs(m) - 1;
                     m &= m - 1u;
                     const int j = ~__shfl_sync(full, cref, L);
                     if (kStats) ++stats.tris;
-                    if (alive) consider(sc, rw, j, tmin, last, h);
+                    if (alive) consider_rot(sc, rr, j, tmin, last_j, h);
                 } while (m);
             } else {
-                while (__any_sync(full, mine != 0u)) {
-                    const bool has = mine != 0u;
-                    const int L = has ? __ffs(mine) - 1 : 0;
-                    mine &= mine - 1u;
-                    const int j = ~__shfl_sync(full, cref, L);
-                    if (kStats) ++stats.tris;
-                    if (alive && has) consider(sc, rw, j, tmin, last, h);
-                }
+                // per-lane cull: own ray against the candidate boxes (all member rays share the beam's sign octant, so
+                // near/far are the same planes for every lane).  Approximate reciprocals: see slab_setup.
+                if (kStats) ++stats.culls;
+                const float ix = rcp_approx(sd[0]), iy = rcp_approx(sd[1]), iz = rcp_approx(sd[2]);
+                const float qx = -so[0] * ix, qy = -so[1] * iy, qz = -so[2] * iz;
+                unsigned rem = mt;
+                do {                                     // kCullSlots candidates at a time (one round unless the node holds more)
+                    const int rank = __popc(rem & lt);
+                    const bool put = ((rem >> lane) & 1u) && rank < kCullSlots;
+                    if (put) {
+                        s_cb[rank] = make_float4(nx, ny, nz, __int_as_float(cref));
+                        s_cb[kCullSlots + rank] = make_float4(fx, fy, fz, 0.f);
+                    }
+                    const int cnt = min(__popc(rem), kCullSlots);
+                    rem &= ~__ballot_sync(full, put);
+                    __syncwarp();
+                    const float cap = alive ? h.t : -1.f;
+                    unsigned mine = 0u;                  // the candidates (slots) this lane still has to test
+#pragma unroll 2
+                    for (int c = 0; c < cnt; ++c) {
+                        const float4 n4 = s_cb[c], f4 = s_cb[kCullSlots + c];
+                        const float e0 = __fmaf_rn(n4.x, ix, qx), e1 = __fmaf_rn(n4.y, iy, qy), e2 = __fmaf_rn(n4.z, iz, qz);
+                        const float x0 = __fmaf_rn(f4.x, ix, qx), x1 = __fmaf_rn(f4.y, iy, qy), x2 = __fmaf_rn(f4.z, iz, qz);
+                        const float en = fmaxf(fmaxf(e0, e1), fmaxf(e2, 0.f)), exi = fminf(fminf(x0, x1), fminf(x2, cap));
+                        if (en <= exi && ~__float_as_int(n4.w) != last_j) mine |= 1u << c;
+                    }
+                    if (kStats) {
+                        stats.pairs += __reduce_add_sync(full, (unsigned)__popc(mine));
+                        stats.tris += __reduce_max_sync(full, (unsigned)__popc(mine));
+                    }
+                    while (mine) {                       // per-lane trip count: the warp runs max-over-lanes iterations
+                        const int c = __ffs(mine) - 1;
+                        mine &= mine - 1u;
+                        consider_rot(sc, rr, ~__float_as_int(s_cb[c].w), tmin, last_j, h);
+                    }
+                    __syncwarp();
+                } while (rem);
             }
             thi = warp_max(alive ? h.t - s : -kInf);
         }

@@ -194,9 +194,14 @@ __global__ void __launch_bounds__(256) k_pack_tris(const float* __restrict__ tri
     const uint32_t g = idx[j];
     const float* v = tri + 9 * (size_t)g;
     const int32_t s = surf[g];
-    tris_out[3 * (size_t)j + 0] = make_float4(v[0], v[1], v[2], __int_as_float((int)g));
-    tris_out[3 * (size_t)j + 1] = make_float4(v[3], v[4], v[5], __int_as_float(s));
-    tris_out[3 * (size_t)j + 2] = make_float4(v[6], v[7], v[8], 0.f);
+    // three rotations of the record, one array after the other (SceneDev::tris): (x, y, z), (y, z, x), (z, x, y)
+    for (uint32_t r = 0; r < 3; ++r) {
+        float4* o = tris_out + 3 * ((size_t)r * T + j);
+        const uint32_t c0 = r, c1 = (r + 1) % 3, c2 = (r + 2) % 3;
+        o[0] = make_float4(v[c0], v[c1], v[c2], __int_as_float((int)g));
+        o[1] = make_float4(v[3 + c0], v[3 + c1], v[3 + c2], __int_as_float(s));
+        o[2] = make_float4(v[6 + c0], v[6 + c1], v[6 + c2], 0.f);
+    }
     normals_out[j] = make_float4(nrm[3 * (size_t)g], nrm[3 * (size_t)g + 1], nrm[3 * (size_t)g + 2], __int_as_float(s));
 }
 
@@ -376,7 +381,7 @@ void compute_layout(const SceneHost& s, opx_scene_layout* lay, size_t* tmp_bytes
     size_t off = 0;
     auto take = [&](size_t bytes) { const size_t r = off; off += align_up(bytes ? bytes : 16, 256); return r; };
     lay->nodes = take(n_nodes * sizeof(NodeDev));
-    lay->triangles = take((T ? T : 1) * 48);
+    lay->triangles = take((T ? T : 1) * 48 * 3);      // three rotations of the record (opx_device.cuh: RayR)
     lay->normals = take((T ? T : 1) * 16);
     lay->surfaces = take(s.surfaces.size() * 8);
     lay->mat_kinds = take(s.mat_kinds.size() * 4);

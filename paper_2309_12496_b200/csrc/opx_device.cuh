@@ -124,9 +124,59 @@ __device__ __forceinline__ RayW ray_setup_mem(const float* o, const float* d) {
     return r;
 }
 
+// Packet kernels: the same constants WITHOUT the exchange of kx and ky for a negative d[kz], and with the triangle record
+// read from the copy whose components are already rotated to (kx, ky, kz) = (kz+1, kz+2, kz) mod 3 (SceneDev::tris holds the
+// three rotations one after the other), so that a vertex is one 16-byte load and no component is ever selected.
+// Dropping the exchange changes no result bit: with kx and ky exchanged, Sx <-> Sy and (Ax, Ay) <-> (Ay, Ax) for every
+// vertex, so each edge function U = Cx By - Cy Bx (two rounded products, one rounded difference) turns into exactly -U;
+// likewise det -> -det and T -> -T (every fma operand pair changes one sign), so t = T / det, the zero tests, the
+// both-signs rejection and the fp64 branch are unchanged; the shading normal m -> -m gives n -> -n, and the reflection
+// fma(-2 (d.n), n, d) is even in n operation by operation.  tests/test_gpu_parity.py compares this path with the oracle, which
+// does exchange, and with the per-lane kernel of opx_lane.cuh, which does too.
+struct RayR {
+    float okx, oky, okz;      // origin permuted to (kx, ky, kz)
+    float Sx, Sy, Sz;
+    uint32_t toff;            // float4 offset of the rotation of the triangle array this ray reads: kx * 3 * n_tri
+};
+
+__device__ __forceinline__ RayR ray_setup_rot(const float* o, const float* d, uint32_t n_tri) {
+    RayR r;
+    const float dx = d[0], dy = d[1], dz = d[2];
+    int kz = 0;
+    float best = fabsf(dx);
+    if (fabsf(dy) > best) { kz = 1; best = fabsf(dy); }
+    if (fabsf(dz) > best) { kz = 2; }
+    const int kx = kz == 2 ? 0 : kz + 1;
+    const int ky = kx == 2 ? 0 : kx + 1;
+    const float dkz = d[kz];
+    r.Sx = __fdiv_rn(d[kx], dkz);
+    r.Sy = __fdiv_rn(d[ky], dkz);
+    r.Sz = __fdiv_rn(1.f, dkz);
+    r.okx = o[kx]; r.oky = o[ky]; r.okz = o[kz];
+    r.toff = (uint32_t)kx * 3u * n_tri;      // rotation 0 = (x, y, z) for kz = 2, 1 = (y, z, x) for kz = 0, 2 = (z, x, y) for kz = 1
+    return r;
+}
+
+// The exact-zero branch of the contract test: all three edge functions recomputed as differences of exact
+// fp64 products, sign test, determinant and T in fp64.  Out of line on purpose: it runs for rays through a vertex or along
+// an edge only, and inlined into every leaf loop it was a third of their code.
+static __device__ __noinline__ bool tri_test_exact(float Ax, float Ay, float Bx, float By, float Cx, float Cy, float Az, float Bz, float Cz, float& t) {
+    const double Ud = __dsub_rn(__dmul_rn((double)Cx, (double)By), __dmul_rn((double)Cy, (double)Bx));
+    const double Vd = __dsub_rn(__dmul_rn((double)Ax, (double)Cy), __dmul_rn((double)Ay, (double)Cx));
+    const double Wd = __dsub_rn(__dmul_rn((double)Bx, (double)Ay), __dmul_rn((double)By, (double)Ax));
+    if ((Ud < 0.0 || Vd < 0.0 || Wd < 0.0) && (Ud > 0.0 || Vd > 0.0 || Wd > 0.0)) return false;
+    const double det = __dadd_rn(__dadd_rn(Ud, Vd), Wd);
+    if (det == 0.0) return false;
+    const double T = __fma_rn(Wd, (double)Cz, __fma_rn(Vd, (double)Bz, __dmul_rn(Ud, (double)Az)));
+    t = __double2float_rn(__ddiv_rn(T, det));
+    return true;
+}
+
 // Contract triangle test on vertex components already permuted to (kx, ky, kz) and shifted to the ray
 // origin (A = a - o, ...).  Returns true with t when the triangle is hit at finite t > tmin.
-__device__ __forceinline__ bool tri_test(const RayW& r, float Akx, float Aky, float Akz, float Bkx, float Bky, float Bkz,
+// Ray: RayW or RayR (only Sx, Sy, Sz are read).
+template <class Ray>
+__device__ __forceinline__ bool tri_test(const Ray& r, float Akx, float Aky, float Akz, float Bkx, float Bky, float Bkz,
                                          float Ckx, float Cky, float Ckz, float tmin, float& t_out) {
     const float Ax = __fmaf_rn(-r.Sx, Akz, Akx), Ay = __fmaf_rn(-r.Sy, Akz, Aky);
     const float Bx = __fmaf_rn(-r.Sx, Bkz, Bkx), By = __fmaf_rn(-r.Sy, Bkz, Bky);
@@ -136,15 +186,7 @@ __device__ __forceinline__ bool tri_test(const RayW& r, float Akx, float Aky, fl
     const float W = __fsub_rn(__fmul_rn(Bx, Ay), __fmul_rn(By, Ax));
     float t;
     if (U == 0.f || V == 0.f || W == 0.f) {
-        const double Ud = __dsub_rn(__dmul_rn((double)Cx, (double)By), __dmul_rn((double)Cy, (double)Bx));
-        const double Vd = __dsub_rn(__dmul_rn((double)Ax, (double)Cy), __dmul_rn((double)Ay, (double)Cx));
-        const double Wd = __dsub_rn(__dmul_rn((double)Bx, (double)Ay), __dmul_rn((double)By, (double)Ax));
-        if ((Ud < 0.0 || Vd < 0.0 || Wd < 0.0) && (Ud > 0.0 || Vd > 0.0 || Wd > 0.0)) return false;
-        const double det = __dadd_rn(__dadd_rn(Ud, Vd), Wd);
-        if (det == 0.0) return false;
-        const double Az = (double)__fmul_rn(r.Sz, Akz), Bz = (double)__fmul_rn(r.Sz, Bkz), Cz = (double)__fmul_rn(r.Sz, Ckz);
-        const double T = __fma_rn(Wd, Cz, __fma_rn(Vd, Bz, __dmul_rn(Ud, Az)));
-        t = __double2float_rn(__ddiv_rn(T, det));
+        if (!tri_test_exact(Ax, Ay, Bx, By, Cx, Cy, __fmul_rn(r.Sz, Akz), __fmul_rn(r.Sz, Bkz), __fmul_rn(r.Sz, Ckz), t)) return false;
     } else {
         // (U<0 || V<0 || W<0) && (U>0 || V>0 || W>0): fminf/fmaxf skip a NaN operand exactly as the comparisons do
         if (fminf(fminf(U, V), W) < 0.f && fmaxf(fmaxf(U, V), W) > 0.f) return false;
@@ -176,6 +218,19 @@ __device__ __forceinline__ void consider(const SceneDev& sc, const RayW& rw, int
     if (tt < h.t || (tt == h.t && gid < h.gid)) { h.t = tt; h.j = j; h.gid = gid; }
 }
 
+// The same for a packet kernel's ray: three 16-byte loads from the ray's rotation of the triangle array; the triangle just
+// left is recognised by its leaf-order index, so no load sits in front of the test.
+__device__ __forceinline__ void consider_rot(const SceneDev& sc, const RayR& r, int j, float tmin, int last_j, Hit& h) {
+    const float4* t = sc.tris + (r.toff + 3u * (uint32_t)j);
+    const float4 a = __ldg(t), b = __ldg(t + 1), c = __ldg(t + 2);
+    if (j == last_j) return;
+    float tt;
+    if (!tri_test(r, __fsub_rn(a.x, r.okx), __fsub_rn(a.y, r.oky), __fsub_rn(a.z, r.okz), __fsub_rn(b.x, r.okx), __fsub_rn(b.y, r.oky),
+                  __fsub_rn(b.z, r.okz), __fsub_rn(c.x, r.okx), __fsub_rn(c.y, r.oky), __fsub_rn(c.z, r.okz), tmin, tt)) return;
+    const int gid = __float_as_int(a.w);
+    if (tt < h.t || (tt == h.t && gid < h.gid)) { h.t = tt; h.j = j; h.gid = gid; }
+}
+
 // Shading normal of DESIGN.md 3.11 for the hit on leaf-order triangle j (global id gid): the vertex normals weighted by
 // the fp32 edge functions U, V, W of 3.3, recomputed here for the one winning triangle (same operations on the same
 // inputs as tri_test, hence the same bits) so that the traversal loop does not have to carry them.  Returns false when
@@ -185,6 +240,29 @@ __device__ __forceinline__ bool shading_normal(const SceneDev& sc, const RayW& r
     const float Akx = __fsub_rn(__ldg(t + r.kx), r.okx), Aky = __fsub_rn(__ldg(t + r.ky), r.oky), Akz = __fsub_rn(__ldg(t + r.kz), r.okz);
     const float Bkx = __fsub_rn(__ldg(t + 4 + r.kx), r.okx), Bky = __fsub_rn(__ldg(t + 4 + r.ky), r.oky), Bkz = __fsub_rn(__ldg(t + 4 + r.kz), r.okz);
     const float Ckx = __fsub_rn(__ldg(t + 8 + r.kx), r.okx), Cky = __fsub_rn(__ldg(t + 8 + r.ky), r.oky), Ckz = __fsub_rn(__ldg(t + 8 + r.kz), r.okz);
+    const float Ax = __fmaf_rn(-r.Sx, Akz, Akx), Ay = __fmaf_rn(-r.Sy, Akz, Aky);
+    const float Bx = __fmaf_rn(-r.Sx, Bkz, Bkx), By = __fmaf_rn(-r.Sy, Bkz, Bky);
+    const float Cx = __fmaf_rn(-r.Sx, Ckz, Ckx), Cy = __fmaf_rn(-r.Sy, Ckz, Cky);
+    const float U = __fsub_rn(__fmul_rn(Cx, By), __fmul_rn(Cy, Bx));
+    const float V = __fsub_rn(__fmul_rn(Ax, Cy), __fmul_rn(Ay, Cx));
+    const float W = __fsub_rn(__fmul_rn(Bx, Ay), __fmul_rn(By, Ax));
+    const float* vn = sc.vnormals + 9 * (size_t)gid;
+    const float mx = __fmaf_rn(W, __ldg(vn + 6), __fmaf_rn(V, __ldg(vn + 3), __fmul_rn(U, __ldg(vn + 0))));
+    const float my = __fmaf_rn(W, __ldg(vn + 7), __fmaf_rn(V, __ldg(vn + 4), __fmul_rn(U, __ldg(vn + 1))));
+    const float mz = __fmaf_rn(W, __ldg(vn + 8), __fmaf_rn(V, __ldg(vn + 5), __fmul_rn(U, __ldg(vn + 2))));
+    const float len2 = __fmaf_rn(mz, mz, __fmaf_rn(my, my, __fmul_rn(mx, mx)));
+    if (!(len2 > 0.f) || !(len2 < kInf)) return false;
+    const float inv = __fdiv_rn(1.f, __fsqrt_rn(len2));
+    nx = __fmul_rn(mx, inv); ny = __fmul_rn(my, inv); nz = __fmul_rn(mz, inv);
+    return true;
+}
+
+__device__ __forceinline__ bool shading_normal(const SceneDev& sc, const RayR& r, int j, int gid, float& nx, float& ny, float& nz) {
+    const float4* t = sc.tris + (r.toff + 3u * (uint32_t)j);
+    const float4 a = __ldg(t), b = __ldg(t + 1), c = __ldg(t + 2);
+    const float Akx = __fsub_rn(a.x, r.okx), Aky = __fsub_rn(a.y, r.oky), Akz = __fsub_rn(a.z, r.okz);
+    const float Bkx = __fsub_rn(b.x, r.okx), Bky = __fsub_rn(b.y, r.oky), Bkz = __fsub_rn(b.z, r.okz);
+    const float Ckx = __fsub_rn(c.x, r.okx), Cky = __fsub_rn(c.y, r.oky), Ckz = __fsub_rn(c.z, r.okz);
     const float Ax = __fmaf_rn(-r.Sx, Akz, Akx), Ay = __fmaf_rn(-r.Sy, Akz, Aky);
     const float Bx = __fmaf_rn(-r.Sx, Bkz, Bkx), By = __fmaf_rn(-r.Sy, Bkz, Bky);
     const float Cx = __fmaf_rn(-r.Sx, Ckz, Ckx), Cy = __fmaf_rn(-r.Sy, Ckz, Cky);
@@ -221,7 +299,8 @@ __device__ __forceinline__ void photon_init(Photon& p, float ox, float oy, float
 // Applies the outcome of one closest-hit query.  Returns true when the photon
 // was reflected and continues with a new segment; otherwise p.state holds the terminal state.
 // rw: the watertight-test constants of the segment that produced h (needed for the shading normal only).
-__device__ __forceinline__ bool interact(const SceneDev& sc, const Hit& h, const RayW& rw, Photon& p, uint64_t seed) {
+template <class Ray>
+__device__ __forceinline__ bool interact(const SceneDev& sc, const Hit& h, const Ray& rw, Photon& p, uint64_t seed) {
     if (h.j < 0) { p.state = OPX_ESCAPED; p.px = p.ox; p.py = p.oy; p.pz = p.oz; p.surface = -1; return false; }
     p.px = __fmaf_rn(h.t, p.dx, p.ox); p.py = __fmaf_rn(h.t, p.dy, p.oy); p.pz = __fmaf_rn(h.t, p.dz, p.oz);   // 3.7
     const float4 nrm = __ldg(sc.normals + h.j);

@@ -38,7 +38,8 @@ constexpr int kWOffLo = 0, kWOffHi = 3 * kWide, kWOffRef = 6 * kWide;      // wo
 struct SceneDev {
     const NodeDev* nodes;      // n_nodes
     const WNodeDev* wnodes;    // n_wnodes (0: the wide tree is not available, packets walk the binary tree)
-    const float4* tris;        // 3 per triangle, leaf order: (a.xyz, id bits) (b.xyz, surface bits) (c.xyz, 0)
+    const float4* tris;        // 3 per triangle, leaf order: (a.xyz, id bits) (b.xyz, surface bits) (c.xyz, 0); then the same array with
+                               // the components rotated to (y, z, x), then to (z, x, y)   (packet kernels: RayR::toff)
     const float4* normals;     // leaf order: n.xyz, surface id bits
     const float* vnormals;     // 9 per triangle (na, nb, nc), GLOBAL id order; NULL when no mesh carries vertex normals (3.11)
     const int2* surfaces;      // (material, frame)

@@ -45,6 +45,7 @@ struct PacketSmemT {
         uint32_t cnt[kRadix][kPktWarps];         // sort: radix counters [digit][warp]
     };
     float beam_tn[kPktWarps][kBeamStack];        // beam traversal: entry bounds of the stacked wide nodes (refs alias `stack`)
+    float4 cull[kPktWarps][2 * kCullSlots];      // beam traversal: candidate boxes of the node a warp is culling (opx_beam.cuh)
     float red[kPktWarps][3];
     float bcast[3];
     uint32_t scan_tot[kPktWarps < 8 ? 8 : kPktWarps];    // sort: per-warp totals; store phase: the 8 state counters
@@ -217,7 +218,7 @@ __device__ __forceinline__ int descend(const SceneDev& sc, const Slab& sl, float
 
 // `oct` (warp-uniform) = 0..7: every alive lane's direction lies in that sign octant; 8: mixed signs; 9: mixed signs and
 // per-ray slack e (an origin beyond SceneDev::origin_limit).
-__device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW& rw, const Slab& sl, float e, float tmin, int last,
+__device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayR& rw, const Slab& sl, float e, float tmin, int last_j,
                                                   bool alive, int lane, int* s_stack, int oct) {
     Hit h{kInf, -1, 0x7fffffff};
     float tcap = alive ? kInf : -1.f;
@@ -226,7 +227,7 @@ __device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayW
     for (;;) {
         ref = oct == 9 ? descend<9>(sc, sl, e, tcap, ref, st, lane, s_stack) : descend<8>(sc, sl, e, tcap, ref, st, lane, s_stack);
         if (ref == kDone) break;
-        consider(sc, rw, ~ref, tmin, last, h);
+        consider_rot(sc, rw, ~ref, tmin, last_j, h);
         if (alive) tcap = h.t;
         if (st.sp == 0) break;
         --st.sp;
@@ -373,21 +374,21 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
         const float* so = sm.o + 3 * i;
         const float* sd = sm.d + 3 * i;
         uint32_t nb = 0;
-        int last = -1;
+        int last = -1, last_j = -1;      // the triangle just left: global id (the record's) and leaf-order index (the walk's)
         while (__any_sync(0xffffffffu, alive)) {
             const float tmin = nb == 0 ? 0.f : sc.t_min;
             Hit h;
-            RayW rw;
+            RayR rw;
             bool done = false;
             {
                 const float ox = so[0], oy = so[1], oz = so[2], dx = sd[0], dy = sd[1], dz = sd[2];
-                rw = ray_setup_mem(so, sd);
+                rw = ray_setup_rot(so, sd, sc.n_tri);
                 Beam bm;
                 float s;
                 const unsigned tris_before = bstats.tris, visits_before = bstats.visits;
                 if (sc.n_wnodes && beam_setup(sc, ox, oy, oz, dx, dy, dz, tmin, alive, bm, s)) {     // coherent packet: one beam through the 32-wide tree
-                    done = bm.mixed ? closest_hit_beam<true, kStats>(sc, rw, bm, s, tmin, last, alive, lane, so, sd, sm.stack[w], sm.beam_tn[w], h, bstats)
-                                    : closest_hit_beam<false, kStats>(sc, rw, bm, s, tmin, last, alive, lane, so, sd, sm.stack[w], sm.beam_tn[w], h, bstats);
+                    done = bm.mixed ? closest_hit_beam<true, kStats>(sc, rw, bm, s, tmin, last_j, alive, lane, so, sd, sm.stack[w], sm.beam_tn[w], sm.cull[w], h, bstats)
+                                    : closest_hit_beam<false, kStats>(sc, rw, bm, s, tmin, last_j, alive, lane, so, sd, sm.stack[w], sm.beam_tn[w], sm.cull[w], h, bstats);
                     if (kStats && done) {
                         ++bstats.beam_segments;
                         const unsigned dt = bstats.tris - tris_before, dv = bstats.visits - visits_before;
@@ -405,15 +406,10 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
                 if (kStats) ++bstats.fallback_segments;
                 const float ox = so[0], oy = so[1], oz = so[2], dx = sd[0], dy = sd[1], dz = sd[2];
                 const Slab sl = slab_setup(ox, oy, oz, dx, dy, dz);
-                // sign octant of the packet (from the sign bits, as slab_rcp keeps them): specialised traversal when all alive
-                // lanes agree; an origin beyond origin_limit widens every box by its own rounding slack instead (8.2)
-                const int oct = dir_octant(dx, dy, dz);
-                const unsigned am = __ballot_sync(0xffffffffu, alive);
-                const int oct0 = __shfl_sync(0xffffffffu, oct, __ffs(am) - 1);
-                const bool uni = __all_sync(0xffffffffu, !alive || oct == oct0);
+                // an origin beyond origin_limit widens every box by its own rounding slack (8.2)
                 const float far_o = fmaxf(fmaxf(fabsf(ox), fabsf(oy)), fabsf(oz));
                 const bool far = __any_sync(0xffffffffu, alive && !(far_o < sc.origin_limit));
-                h = closest_hit_packet(sc, rw, sl, far_o * 9.5367431640625e-7f, tmin, last, alive, lane, sm.stack[w], far ? 9 : (uni ? oct0 : 8));
+                h = closest_hit_packet(sc, rw, sl, far_o * 9.5367431640625e-7f, tmin, last_j, alive, lane, sm.stack[w], far ? 9 : 8);
             }
             if (alive) {
                 Photon p;
@@ -423,7 +419,7 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
                 sm.d[3 * i] = p.dx; sm.d[3 * i + 1] = p.dy; sm.d[3 * i + 2] = p.dz;
                 if (alive) {
                     sm.o[3 * i] = p.ox; sm.o[3 * i + 1] = p.oy; sm.o[3 * i + 2] = p.oz;
-                    nb = p.b; last = p.last;
+                    nb = p.b; last = p.last; last_j = h.j;
                 } else {
                     sm.o[3 * i] = p.px; sm.o[3 * i + 1] = p.py; sm.o[3 * i + 2] = p.pz;
                     sm.wl[i] = __int_as_float(p.pixel);
