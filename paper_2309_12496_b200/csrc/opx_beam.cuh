@@ -26,7 +26,8 @@
 namespace opx {
 namespace {
 
-constexpr int kBeamStack = 64;            // per warp, in shared memory; overflow => fall back to the binary walk
+constexpr int kBeamStack = 56;            // per warp, in shared memory; overflow => fall back to the binary walk
+constexpr int kBeamStackWords = 64;       // words reserved per array: the last 8 of each hold the parked beam (closest_hit_beam)
 #ifndef OPX_CULL_MIN
 #define OPX_CULL_MIN 4
 #endif
@@ -138,7 +139,7 @@ __device__ __forceinline__ bool beam_setup(const SceneDev& sc, float ox, float o
 // (far planes, -), written by the lanes that own the candidates and read back by every lane with uniform addresses
 // (two broadcast 16-byte loads per candidate instead of six shuffles).
 template <bool kMixed, bool kStats>
-__device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayR& rr, const Beam& bm, float s, float tmin, int last_j,
+__device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayR& rr, Beam bm, float s, float tmin, int last_j,
                                                  bool alive, int lane, const float* so, const float* sd,
                                                  int* s_ref, float* s_tn, float4* s_cb, Hit& h, BeamStats& stats) {
     const unsigned full = 0xffffffffu;
@@ -146,8 +147,20 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayR&
     float thi = kInf;
     int sp = 0, ref = 0;
     const unsigned lt = (1u << lane) - 1u;
-    const bool ngx = bm.neg & 1u, ngy = bm.neg & 2u, ngz = bm.neg & 4u;
+    // The beam is read at every node and in no leaf phase, and the leaf phases need many registers of their own: it is parked
+    // in shared memory (the 8 words behind each stack array) and read back after every leaf phase, so that it occupies no
+    // register while triangles are tested -- left to itself the compiler kept it in local memory and re-read it at EVERY node.
+    float4* s_beam = reinterpret_cast<float4*>(s_ref + kBeamStack);
+    float4* s_beam2 = reinterpret_cast<float4*>(s_tn + kBeamStack);
+    if (lane == 0) {
+        s_beam[0] = make_float4(bm.rn[0], bm.rn[1], bm.rn[2], bm.tlo);
+        s_beam[1] = make_float4(bm.cn[0], bm.cn[1], bm.cn[2], __uint_as_float(bm.neg | (bm.mixed << 3)));
+        s_beam2[0] = make_float4(bm.rf[0], bm.rf[1], bm.rf[2], 0.f);
+        s_beam2[1] = make_float4(bm.cf[0], bm.cf[1], bm.cf[2], 0.f);
+    }
+    __syncwarp();
     for (;;) {
+        const bool ngx = bm.neg & 1u, ngy = bm.neg & 2u, ngz = bm.neg & 4u;
         if (kStats) ++stats.visits;
         const float* nd = reinterpret_cast<const float*>(sc.wnodes + ref) + lane;
         const float lox = __ldg(nd + kWOffLo), loy = __ldg(nd + kWOffLo + kWide), loz = __ldg(nd + kWOffLo + 2 * kWide);
@@ -199,8 +212,9 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayR&
                     __syncwarp();
                     const float cap = alive ? h.t : -1.f;
                     unsigned mine = 0u;                  // the candidates (slots) this lane still has to test
-#pragma unroll 2
-                    for (int c = 0; c < cnt; ++c) {
+#pragma unroll
+                    for (int c = 0; c < kCullSlots; ++c) {       // unrolled: slot addresses and mask bits are immediates
+                        if (c >= cnt) break;
                         const float4 n4 = s_cb[c], f4 = s_cb[kCullSlots + c];
                         const float e0 = __fmaf_rn(n4.x, ix, qx), e1 = __fmaf_rn(n4.y, iy, qy), e2 = __fmaf_rn(n4.z, iz, qz);
                         const float x0 = __fmaf_rn(f4.x, ix, qx), x1 = __fmaf_rn(f4.y, iy, qy), x2 = __fmaf_rn(f4.z, iz, qz);
@@ -220,6 +234,12 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayR&
                 } while (rem);
             }
             thi = warp_max(alive ? h.t - s : -kInf);
+            {
+                const float4 a = s_beam[0], b = s_beam[1], c = s_beam2[0], d = s_beam2[1];
+                bm.rn[0] = a.x; bm.rn[1] = a.y; bm.rn[2] = a.z; bm.tlo = a.w;
+                bm.cn[0] = b.x; bm.cn[1] = b.y; bm.cn[2] = b.z; bm.neg = __float_as_uint(b.w) & 7u; bm.mixed = __float_as_uint(b.w) >> 3;
+                bm.rf[0] = c.x; bm.rf[1] = c.y; bm.rf[2] = c.z; bm.cf[0] = d.x; bm.cf[1] = d.y; bm.cf[2] = d.z;
+            }
         }
         const bool go = hit && cref >= 0 && tn <= thi;
         const unsigned mn = __ballot_sync(full, go);

@@ -44,7 +44,7 @@ struct PacketSmemT {
         int stack[kPktWarps][kStackSmem];        // traversal: stack entries >= 32 of each warp
         uint32_t cnt[kRadix][kPktWarps];         // sort: radix counters [digit][warp]
     };
-    float beam_tn[kPktWarps][kBeamStack];        // beam traversal: entry bounds of the stacked wide nodes (refs alias `stack`)
+    float beam_tn[kPktWarps][kBeamStackWords];        // beam traversal: entry bounds of the stacked wide nodes (refs alias `stack`)
     float4 cull[kPktWarps][2 * kCullSlots];      // beam traversal: candidate boxes of the node a warp is culling (opx_beam.cuh)
     float red[kPktWarps][3];
     float bcast[3];
@@ -53,7 +53,7 @@ struct PacketSmemT {
     alignas(8) unsigned long long mbar;          // completion barrier of the bulk loads of the staging phase
 };
 static_assert(sizeof(int) * kStackSmem >= sizeof(uint32_t) * kRadix, "radix counters alias the stack overflow area");
-static_assert(kBeamStack <= kStackSmem, "the beam stack refs alias the binary walk's overflow area");
+static_assert(kBeamStackWords <= kStackSmem && kBeamStack + 8 <= kBeamStackWords, "the beam stack refs (and the parked beam behind them) alias the binary walk's overflow area");
 
 // ---- TMA bulk copies (cp.async.bulk, 1-D): a full tile's inputs and records are contiguous 16-byte-aligned blocks, so one
 // elected thread moves them between global and shared memory instead of 512 threads looping over float4s.
