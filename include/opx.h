@@ -260,6 +260,38 @@ opx_status opx_emit_cherenkov_filtered(const opx_scene* scene, const opx_track_s
                                        float* d_out_wavelengths, uint32_t* d_out_index, uint64_t out_capacity,
                                        uint64_t* d_n_kept, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* List of DETECTED photons, DEVICE pointers, each array of `capacity` entries (pos, dir: capacity x 3 packed): what the paper
+ * asks the emitter-to-detector loop to produce, "the position of the ray in a list when it interacts with the detector"
+ * (PAPER.md:195).  Entry r: global photon id, detector pixel id, hit position, direction of arrival - the fields of the
+ * photon's hit record (opx_hits), for photons whose state is OPX_DETECTED only. */
+typedef struct {
+    uint64_t* id;
+    int32_t* pixel;
+    float* pos;
+    float* dir;
+} opx_detected;
+
+/* opx_propagate_flags with a compacted output: instead of one hit record per photon, the photons that end DETECTED are
+ * APPENDED to the list `out`, in increasing photon id (stable: the result does not depend on scheduling, two runs give
+ * identical bytes).  *d_n_detected (DEVICE uint64) is the list's length: on entry the number of entries already in it
+ * (the caller zeroes it once), on exit increased by the number of photons this call detected.  While *d_n_detected <=
+ * capacity the list is complete.  Entries that do not fit are dropped but still counted, so *d_n_detected > capacity
+ * reports a truncated list; a truncated list holds `capacity` entries in increasing id, not necessarily those with
+ * the smallest ids.  Calls that append to the same list must be ordered (same stream, or events): a later call reads
+ * the length an earlier one wrote.  Hit-map and counters as in opx_propagate (every photon is counted, whatever its state).  The per-photon
+ * results are those of opx_propagate_flags bit for bit: this call only leaves out the 34 B/photon of records
+ * nobody asked for.  Three launches and one memset, no host round trip: the propagation kernel stages each tile's
+ * detected photons in the workspace in the order the tiles finish, a scan and a gather kernel move them to the list in
+ * photon-id order.  d_workspace: opx_propagate_detected_workspace_bytes(n, capacity) device bytes, 256-byte aligned, used
+ * while the call's kernels run.  Needs a scene of two triangles or more (OPX_ERR_BAD_STATE otherwise).  Other arguments
+ * and errors as in opx_propagate_flags. */
+opx_status opx_propagate_detected_workspace_bytes(uint64_t n, uint64_t capacity, size_t* bytes);
+opx_status opx_propagate_detected(const opx_scene* scene, uint64_t n, const uint64_t* d_n, uint64_t photon_id_base,
+                                  const float* d_origins, const float* d_dirs, const float* d_wavelengths,
+                                  uint64_t seed, uint32_t flags, const opx_detected* out, uint64_t capacity,
+                                  uint64_t* d_n_detected, void* d_workspace, size_t workspace_bytes,
+                                  uint32_t* d_hitmap, uint64_t* d_counters, void* cuda_stream);
+
 /* Size of the device staging workspace opx_propagate_host needs for chunks of `chunk` photons. */
 opx_status opx_propagate_host_workspace_bytes(const opx_scene* scene, uint64_t chunk, size_t* bytes);
 
@@ -275,6 +307,19 @@ opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photo
                               uint64_t seed, const opx_hits* h_out, uint32_t* h_hitmap,
                               uint64_t* h_counters, void* d_workspace, size_t workspace_bytes,
                               uint64_t chunk, void* cuda_stream);
+
+/* opx_propagate_host with the detected-only output of opx_propagate_detected: photons are uploaded in chunks as in
+ * opx_propagate_host, nothing but the list of detected photons (HOST arrays of `capacity` entries in h_out), the hit-map
+ * and the counters comes back - 28 B per photon up, 36 B per DETECTED photon down.  *h_n_detected receives the number of
+ * detected photons of this call (entries beyond capacity are dropped but counted); the list starts at entry 0.
+ * d_workspace: opx_propagate_host_detected_workspace_bytes(scene, chunk, capacity) device bytes, 256-byte aligned.
+ * Synchronises `cuda_stream` before returning. */
+opx_status opx_propagate_host_detected_workspace_bytes(const opx_scene* scene, uint64_t chunk, uint64_t capacity, size_t* bytes);
+opx_status opx_propagate_host_detected(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,
+                                       const float* h_origins, const float* h_dirs, const float* h_wavelengths,
+                                       uint64_t seed, uint32_t flags, const opx_detected* h_out, uint64_t capacity,
+                                       uint64_t* h_n_detected, uint32_t* h_hitmap, uint64_t* h_counters,
+                                       void* d_workspace, size_t workspace_bytes, uint64_t chunk, void* cuda_stream);
 
 opx_status opx_scene_info(const opx_scene* scene, uint64_t* n_triangles, uint64_t* n_nodes,
                           uint64_t* n_pixels, uint64_t* n_surfaces);

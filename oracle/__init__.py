@@ -237,6 +237,15 @@ def trace_mesh_arrays(tri, tri_surface, surf_mat, surf_frame, mat_kind, mat_tabl
     return r
 
 
+def detected_list(result, id_base=0, ids=None):
+    """The list PAPER.md:195 asks for ("writes the position of the ray in a list when it interacts with the detector"): the
+    records of the photons whose state is DETECTED, in photon order.  `result` is what trace_mesh returned for photons
+    id_base + i (or ids[i]).  Returns Result(id (k,) uint64, pixel (k,) int32, pos, dir (k,3))."""
+    idx = np.nonzero(np.asarray(result["state"]) == DETECTED)[0]
+    gid = (np.uint64(id_base) + idx.astype(np.uint64)) if ids is None else np.asarray(ids, dtype=np.uint64)[idx]
+    return Result(id=gid, pixel=result["pixel"][idx].copy(), pos=result["pos"][idx].copy(), dir=result["dir"][idx].copy(), index=idx)
+
+
 def trace_analytic_toy(scene, origins, dirs, wavelengths, seed=0, id_base=0, with_box=True,
                        det_half=300.0):
     """Config 0 with the mirror as an exact sphere (fp64).  `scene` is workloads.toy_rich_scene():

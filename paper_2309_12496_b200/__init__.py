@@ -5,5 +5,5 @@ opx.py  thin ctypes/torch binding with the same names
 
 Nothing here imports the oracle, and there is no CPU fallback.
 """
-from .opx import (DEBUG_EXPORTS, EXPORTS, FLAG_NO_EFFICIENCY, LIB_PATH, STATE_NAMES, TABLE_HISTOGRAM, TABLE_LINEAR, OpxError, Scene, alloc_host_records,  # noqa: F401
+from .opx import (DEBUG_EXPORTS, EXPORTS, FLAG_NO_EFFICIENCY, LIB_PATH, STATE_NAMES, TABLE_HISTOGRAM, TABLE_LINEAR, OpxError, Scene, alloc_host_detected, alloc_host_records,  # noqa: F401
                   emit_cherenkov, last_kernel, launch_count, load_library, measure_fp32_peak, upload_track_steps)

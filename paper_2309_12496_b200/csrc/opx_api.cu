@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 
 #include "opx_internal.cuh"
 
@@ -298,6 +299,38 @@ opx_status opx_emit_cherenkov_filtered(const opx_scene* scene, const opx_track_s
                                 d_out_origins, d_out_dirs, d_out_wavelengths, d_out_index, out_capacity, d_n_kept, d_workspace, (cudaStream_t)cuda_stream);
 }
 
+// ------------------------------------------------------------------------- detected-only output
+opx_status opx_propagate_detected_workspace_bytes(uint64_t n, uint64_t capacity, size_t* bytes) {
+    if (!bytes) return fail(OPX_ERR_INVALID_ARG, "bytes is NULL");
+    *bytes = detected_workspace_bytes(n, capacity);
+    return OPX_OK;
+}
+
+opx_status opx_propagate_detected(const opx_scene* scene, uint64_t n, const uint64_t* d_n, uint64_t photon_id_base,
+                                  const float* d_origins, const float* d_dirs, const float* d_wavelengths, uint64_t seed,
+                                  uint32_t flags, const opx_detected* out, uint64_t capacity, uint64_t* d_n_detected,
+                                  void* d_workspace, size_t workspace_bytes, uint32_t* d_hitmap, uint64_t* d_counters,
+                                  void* cuda_stream) {
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate_detected before opx_bvh_build");
+    if (flags & ~(uint32_t)OPX_FLAG_NO_EFFICIENCY) return fail(OPX_ERR_INVALID_ARG, "unknown flag");
+    if (!d_n_detected || misaligned(d_n_detected, 8)) return fail(OPX_ERR_INVALID_ARG, "d_n_detected is NULL or misaligned");
+    if (n == 0) return OPX_OK;
+    if (!d_origins || !d_dirs || !d_wavelengths || !out || !d_workspace) return fail(OPX_ERR_INVALID_ARG, "NULL photon/list/workspace pointer");
+    if (capacity && (!out->id || !out->pixel || !out->pos || !out->dir)) return fail(OPX_ERR_INVALID_ARG, "NULL list array");
+    if (!capacity) return fail(OPX_ERR_INVALID_ARG, "capacity = 0");
+    if (!d_hitmap && scene->n_pixels) return fail(OPX_ERR_INVALID_ARG, "d_hitmap is NULL but the scene has pixels");
+    if (misaligned(d_origins, 4) || misaligned(d_dirs, 4) || misaligned(d_wavelengths, 4) || misaligned(out->id, 8) ||
+        misaligned(out->pixel, 4) || misaligned(out->pos, 4) || misaligned(out->dir, 4) || misaligned(d_hitmap, 4) ||
+        misaligned(d_counters, 8) || misaligned(d_n, 8) || misaligned(d_workspace, 256))
+        return fail(OPX_ERR_INVALID_ARG, "misaligned pointer");
+    if (workspace_bytes < detected_workspace_bytes(n, capacity)) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_propagate_detected_workspace_bytes)");
+    if (scene->tri_surface.size() < 2) return fail(OPX_ERR_BAD_STATE, "the detected-only output needs a scene of two triangles or more");
+    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_propagate_detected")) return st;
+    return launch_propagate_detected(*scene, n, d_n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, flags, *out, capacity,
+                                     d_n_detected, d_workspace, d_hitmap, d_counters, (cudaStream_t)cuda_stream);
+}
+
 // ------------------------------------------------------------------------- host-buffer streaming
 // Device staging per slot (kSlots slots, one stream each): inputs 28 B/photon, records 34 B/photon.  Three slots let the
 // upload of chunk k+2 run while chunk k+1 computes and chunk k downloads, so neither copy engine waits for a buffer.
@@ -305,17 +338,184 @@ opx_status opx_emit_cherenkov_filtered(const opx_scene* scene, const opx_track_s
 #define OPX_HOST_SLOTS 3
 #endif
 static constexpr int kSlots = OPX_HOST_SLOTS;
-static size_t slot_bytes(uint64_t chunk) {
+}  // extern "C"
+
+namespace opx {
+struct HostPipe {
+    cudaStream_t st[kSlots]{};
+    cudaEvent_t done[kSlots]{}, kernel[kSlots]{}, start{};
+    int device = -1;
+    std::mutex busy;              // one host-buffer call per scene at a time (the calls synchronise anyway)
+};
+void destroy_host_pipe(HostPipe* p) {
+    if (!p) return;
+    for (int k = 0; k < kSlots; ++k) {
+        if (p->st[k]) cudaStreamDestroy(p->st[k]);
+        if (p->done[k]) cudaEventDestroy(p->done[k]);
+        if (p->kernel[k]) cudaEventDestroy(p->kernel[k]);
+    }
+    if (p->start) cudaEventDestroy(p->start);
+    delete p;
+}
+static std::mutex g_pipe_mutex;
+// The scene's pipe, created on its first host-buffer call (streams and events are not created per call).
+static opx_status host_pipe(const SceneHost& s, HostPipe** out) {
+    std::lock_guard<std::mutex> lock(g_pipe_mutex);
+    int dev = 0;
+    if (opx_status st = check_cuda(cudaGetDevice(&dev), "cudaGetDevice")) return st;
+    if (s.pipe && s.pipe->device != dev) { destroy_host_pipe(s.pipe); s.pipe = nullptr; }
+    if (!s.pipe) {
+        HostPipe* p = new HostPipe;
+        p->device = dev;
+        cudaError_t e = cudaEventCreateWithFlags(&p->start, cudaEventDisableTiming);
+        for (int k = 0; k < kSlots && e == cudaSuccess; ++k) {
+            e = cudaStreamCreateWithFlags(&p->st[k], cudaStreamNonBlocking);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->done[k], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->kernel[k], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) { destroy_host_pipe(p); return check_cuda(e, "creating the streams of the host-buffer path"); }
+        s.pipe = p;
+    }
+    *out = s.pipe;
+    return OPX_OK;
+}
+
+static size_t slot_bytes(uint64_t chunk, bool records) {
     size_t b = 0;
-    b += align_up(chunk * 12, 256) * 4;   // origins, dirs, pos, dir
-    b += align_up(chunk * 4, 256) * 3;    // wavelengths, pixel, surface
-    b += align_up(chunk, 256) * 2;        // state, bounces
+    b += align_up(chunk * 12, 256) * (records ? 4 : 2);   // origins, dirs (, pos, dir)
+    b += align_up(chunk * 4, 256) * (records ? 3 : 1);    // wavelengths (, pixel, surface)
+    if (records) b += align_up(chunk, 256) * 2;           // state, bounces
+    return b;
+}
+static size_t host_workspace_bytes(const SceneHost& s, uint64_t chunk, bool records, uint64_t capacity) {
+    size_t b = kSlots * slot_bytes(chunk, records) + align_up(s.n_pixels * 4 + 4, 256) + 256;
+    // the device copy of the list + the workspace of the detected-only launches (one: the chunks' kernels run one after another)
+    if (!records) b += align_up(capacity * 8, 256) + align_up(capacity * 4, 256) + 2 * align_up(capacity * 12, 256) + 256 + detected_workspace_bytes(chunk, capacity);
     return b;
 }
 
+// Both host-buffer calls: h_out (per-photon records) or h_det (detected-only list), never both.
+static opx_status propagate_host_impl(const SceneHost& scene, uint64_t n, uint64_t photon_id_base, const float* h_origins,
+                                      const float* h_dirs, const float* h_wavelengths, uint64_t seed, uint32_t flags,
+                                      const opx_hits* h_out, const opx_detected* h_det, uint64_t capacity, uint64_t* h_n_detected,
+                                      uint32_t* h_hitmap, uint64_t* h_counters, void* d_workspace, uint64_t chunk, cudaStream_t main) {
+    const bool records = h_out != nullptr;
+    HostPipe* pipe = nullptr;
+    if (opx_status st = host_pipe(scene, &pipe)) return st;
+    std::lock_guard<std::mutex> lock(pipe->busy);
+    struct Slot { float *o, *d, *wl, *pos, *dir; int32_t *pixel, *surface; uint8_t *state, *bounces; };
+    Slot slot[kSlots];
+    char* p = (char*)d_workspace;
+    auto take = [&](size_t bytes) { char* r = p; p += align_up(bytes, 256); return r; };
+    for (int k = 0; k < kSlots; ++k) {
+        Slot& s = slot[k];
+        s = Slot{};
+        s.o = (float*)take(chunk * 12); s.d = (float*)take(chunk * 12); s.wl = (float*)take(chunk * 4);
+        if (records) {
+            s.pos = (float*)take(chunk * 12); s.dir = (float*)take(chunk * 12);
+            s.pixel = (int32_t*)take(chunk * 4); s.surface = (int32_t*)take(chunk * 4);
+            s.state = (uint8_t*)take(chunk); s.bounces = (uint8_t*)take(chunk);
+        }
+    }
+    uint32_t* d_hitmap = (uint32_t*)take(scene.n_pixels * 4 + 4);
+    uint64_t* d_counters = (uint64_t*)take(64);           // [0..7] counters, then the detected list's length
+    uint64_t* d_n_det = d_counters + 8;
+    take(64);
+    opx_detected det{};
+    void* det_ws = nullptr;
+    if (!records) {
+        det.id = (uint64_t*)take(capacity * 8); det.pixel = (int32_t*)take(capacity * 4);
+        det.pos = (float*)take(capacity * 12); det.dir = (float*)take(capacity * 12);
+        det_ws = take(detected_workspace_bytes(chunk, capacity));
+    }
+
+    cudaError_t err = cudaSuccess;
+    auto ck = [&](cudaError_t e) { if (e != cudaSuccess && err == cudaSuccess) err = e; };
+    opx_status st = OPX_OK;
+    // fork: the slot streams wait for whatever preceded on the caller's stream
+    ck(cudaMemsetAsync(d_hitmap, 0, scene.n_pixels * 4 + 4, main));
+    ck(cudaMemsetAsync(d_counters, 0, 128, main));
+    ck(cudaEventRecord(pipe->start, main));
+    for (int k = 0; k < kSlots; ++k) ck(cudaStreamWaitEvent(pipe->st[k], pipe->start, 0));
+
+    uint64_t done = 0;
+    int k = 0, prev = -1;
+    // Chunk schedule: the first upload and the last download cannot overlap anything, so the stream is ramped up
+    // (chunk/8, chunk/8, chunk/4, chunk/2, then full chunks) and ramped down (halving the remainder, floor chunk/8).
+    const uint64_t small = chunk >= 8 ? chunk / 8 : 1;
+    uint32_t issued = 0;
+    while (done < n && st == OPX_OK && err == cudaSuccess) {
+        uint64_t m = chunk;
+        if (issued < 2) m = small; else if (issued == 2) m = chunk / 4 ? chunk / 4 : 1; else if (issued == 3) m = chunk / 2 ? chunk / 2 : 1;
+        const uint64_t left = n - done;
+        if (left < 2 * m) { const uint64_t half = (left + 1) / 2; m = half > small ? half : (left < small ? left : small); }
+        if (m > left) m = left;
+        ++issued;
+        Slot& s = slot[k];
+        cudaStream_t sst = pipe->st[k];
+        ck(cudaMemcpyAsync(s.o, h_origins + 3 * done, m * 12, cudaMemcpyHostToDevice, sst));
+        ck(cudaMemcpyAsync(s.d, h_dirs + 3 * done, m * 12, cudaMemcpyHostToDevice, sst));
+        ck(cudaMemcpyAsync(s.wl, h_wavelengths + done, m * 4, cudaMemcpyHostToDevice, sst));
+        if (records) {
+            opx_hits dev_out{s.pos, s.dir, s.pixel, s.surface, s.state, s.bounces};
+            st = launch_propagate(scene, kWalkProduct, m, nullptr, photon_id_base + done, s.o, s.d, s.wl, seed, flags, dev_out, d_hitmap,
+                                  d_counters, sst);
+            ck(cudaMemcpyAsync(h_out->pos + 3 * done, s.pos, m * 12, cudaMemcpyDeviceToHost, sst));
+            ck(cudaMemcpyAsync(h_out->dir + 3 * done, s.dir, m * 12, cudaMemcpyDeviceToHost, sst));
+            ck(cudaMemcpyAsync(h_out->pixel + done, s.pixel, m * 4, cudaMemcpyDeviceToHost, sst));
+            ck(cudaMemcpyAsync(h_out->surface + done, s.surface, m * 4, cudaMemcpyDeviceToHost, sst));
+            ck(cudaMemcpyAsync(h_out->state + done, s.state, m, cudaMemcpyDeviceToHost, sst));
+            ck(cudaMemcpyAsync(h_out->bounces + done, s.bounces, m, cudaMemcpyDeviceToHost, sst));
+        } else {
+            // the chunks append to one list: a chunk's kernel starts after the previous chunk's (they would not overlap much
+            // anyway: the uploads are what the pipeline waits for)
+            if (prev >= 0) ck(cudaStreamWaitEvent(sst, pipe->kernel[prev], 0));
+            st = launch_propagate_detected(scene, m, nullptr, photon_id_base + done, s.o, s.d, s.wl, seed, flags, det, capacity, d_n_det, det_ws,
+                                           d_hitmap, d_counters, sst);
+            ck(cudaEventRecord(pipe->kernel[k], sst));
+            prev = k;
+        }
+        done += m;
+        k = (k + 1) % kSlots;
+    }
+    // join
+    for (int j = 0; j < kSlots; ++j) { ck(cudaEventRecord(pipe->done[j], pipe->st[j])); ck(cudaStreamWaitEvent(main, pipe->done[j], 0)); }
+    std::vector<uint32_t> hm(scene.n_pixels);
+    uint64_t cnt[9] = {0};
+    if (scene.n_pixels) ck(cudaMemcpyAsync(hm.data(), d_hitmap, scene.n_pixels * 4, cudaMemcpyDeviceToHost, main));
+    ck(cudaMemcpyAsync(cnt, d_counters, 72, cudaMemcpyDeviceToHost, main));
+    ck(cudaStreamSynchronize(main));
+    if (!records && st == OPX_OK && err == cudaSuccess) {
+        const uint64_t have = cnt[8] < capacity ? cnt[8] : capacity;
+        if (have) {
+            ck(cudaMemcpyAsync(h_det->id, det.id, have * 8, cudaMemcpyDeviceToHost, main));
+            ck(cudaMemcpyAsync(h_det->pixel, det.pixel, have * 4, cudaMemcpyDeviceToHost, main));
+            ck(cudaMemcpyAsync(h_det->pos, det.pos, have * 12, cudaMemcpyDeviceToHost, main));
+            ck(cudaMemcpyAsync(h_det->dir, det.dir, have * 12, cudaMemcpyDeviceToHost, main));
+            ck(cudaStreamSynchronize(main));
+        }
+        *h_n_detected = cnt[8];
+    }
+    if (st != OPX_OK) { cudaStreamSynchronize(main); return st; }
+    if (err != cudaSuccess) { cudaStreamSynchronize(main); return check_cuda(err, "opx_propagate_host"); }
+    for (uint64_t i = 0; i < scene.n_pixels; ++i) h_hitmap[i] += hm[i];
+    if (h_counters) for (int i = 0; i < 8; ++i) h_counters[i] += cnt[i];
+    return OPX_OK;
+}
+}  // namespace opx
+
+extern "C" {
+using namespace opx;
+
 opx_status opx_propagate_host_workspace_bytes(const opx_scene* scene, uint64_t chunk, size_t* bytes) {
     if (!scene || !bytes || chunk == 0) return fail(OPX_ERR_INVALID_ARG, "NULL argument or chunk = 0");
-    *bytes = kSlots * slot_bytes(chunk) + align_up(scene->n_pixels * 4 + 4, 256) + 256;
+    *bytes = host_workspace_bytes(*scene, chunk, true, 0);
+    return OPX_OK;
+}
+
+opx_status opx_propagate_host_detected_workspace_bytes(const opx_scene* scene, uint64_t chunk, uint64_t capacity, size_t* bytes) {
+    if (!scene || !bytes || chunk == 0 || capacity == 0) return fail(OPX_ERR_INVALID_ARG, "NULL argument, chunk = 0 or capacity = 0");
+    *bytes = host_workspace_bytes(*scene, chunk, false, capacity);
     return OPX_OK;
 }
 
@@ -332,80 +532,34 @@ opx_status opx_propagate_host(const opx_scene* scene, uint64_t n, uint64_t photo
         return fail(OPX_ERR_INVALID_ARG, "NULL hit-record array");
     if (!h_hitmap && scene->n_pixels) return fail(OPX_ERR_INVALID_ARG, "h_hitmap is NULL but the scene has pixels");
     if (misaligned(d_workspace, 256)) return fail(OPX_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
-    size_t need = 0;
-    opx_propagate_host_workspace_bytes(scene, chunk, &need);
-    if (workspace_bytes < need) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_propagate_host_workspace_bytes)");
+    if (workspace_bytes < host_workspace_bytes(*scene, chunk, true, 0)) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_propagate_host_workspace_bytes)");
+    if (opx_status st = device_ok()) return st;
+    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_propagate_host")) return st;
+    return propagate_host_impl(*scene, n, photon_id_base, h_origins, h_dirs, h_wavelengths, seed, 0u, h_out, nullptr, 0, nullptr, h_hitmap,
+                               h_counters, d_workspace, chunk, (cudaStream_t)cuda_stream);
+}
 
-    cudaStream_t main = (cudaStream_t)cuda_stream;
-    struct Slot { float *o, *d, *wl, *pos, *dir; int32_t *pixel, *surface; uint8_t *state, *bounces; cudaStream_t st; cudaEvent_t done; };
-    Slot slot[kSlots];
-    char* p = (char*)d_workspace;
-    auto take = [&](size_t bytes) { char* r = p; p += align_up(bytes, 256); return r; };
-    for (int k = 0; k < kSlots; ++k) {
-        Slot& s = slot[k];
-        s.o = (float*)take(chunk * 12); s.d = (float*)take(chunk * 12); s.pos = (float*)take(chunk * 12); s.dir = (float*)take(chunk * 12);
-        s.wl = (float*)take(chunk * 4); s.pixel = (int32_t*)take(chunk * 4); s.surface = (int32_t*)take(chunk * 4);
-        s.state = (uint8_t*)take(chunk); s.bounces = (uint8_t*)take(chunk);
-    }
-    uint32_t* d_hitmap = (uint32_t*)take(scene->n_pixels * 4 + 4);
-    uint64_t* d_counters = (uint64_t*)take(64);
-
-    opx_status st = OPX_OK;
-    cudaEvent_t start;
-    if ((st = check_cuda(cudaEventCreateWithFlags(&start, cudaEventDisableTiming), "cudaEventCreate"))) return st;
-    for (int k = 0; k < kSlots; ++k) {
-        cudaStreamCreateWithFlags(&slot[k].st, cudaStreamNonBlocking);
-        cudaEventCreateWithFlags(&slot[k].done, cudaEventDisableTiming);
-    }
-    // fork: both slot streams wait for whatever preceded on the caller's stream
-    cudaMemsetAsync(d_hitmap, 0, scene->n_pixels * 4 + 4, main);
-    cudaMemsetAsync(d_counters, 0, 64, main);
-    cudaEventRecord(start, main);
-    for (int k = 0; k < kSlots; ++k) cudaStreamWaitEvent(slot[k].st, start, 0);
-
-    uint64_t done = 0;
-    int k = 0;
-    // Chunk schedule: the first upload and the last download cannot overlap anything, so the stream is ramped up
-    // (chunk/8, chunk/8, chunk/4, chunk/2, then full chunks) and ramped down (halving the remainder, floor chunk/8).
-    const uint64_t small = chunk >= 8 ? chunk / 8 : 1;
-    uint32_t issued = 0;
-    while (done < n && st == OPX_OK) {
-        uint64_t m = chunk;
-        if (issued < 2) m = small; else if (issued == 2) m = chunk / 4 ? chunk / 4 : 1; else if (issued == 3) m = chunk / 2 ? chunk / 2 : 1;
-        const uint64_t left = n - done;
-        if (left < 2 * m) { const uint64_t half = (left + 1) / 2; m = half > small ? half : (left < small ? left : small); }
-        if (m > left) m = left;
-        ++issued;
-        Slot& s = slot[k];
-        cudaMemcpyAsync(s.o, h_origins + 3 * done, m * 12, cudaMemcpyHostToDevice, s.st);
-        cudaMemcpyAsync(s.d, h_dirs + 3 * done, m * 12, cudaMemcpyHostToDevice, s.st);
-        cudaMemcpyAsync(s.wl, h_wavelengths + done, m * 4, cudaMemcpyHostToDevice, s.st);
-        opx_hits dev_out{s.pos, s.dir, s.pixel, s.surface, s.state, s.bounces};
-        st = launch_propagate(*scene, kWalkProduct, m, nullptr, photon_id_base + done, s.o, s.d, s.wl, seed, 0u, dev_out, d_hitmap,
-                              d_counters, s.st);
-        cudaMemcpyAsync(h_out->pos + 3 * done, s.pos, m * 12, cudaMemcpyDeviceToHost, s.st);
-        cudaMemcpyAsync(h_out->dir + 3 * done, s.dir, m * 12, cudaMemcpyDeviceToHost, s.st);
-        cudaMemcpyAsync(h_out->pixel + done, s.pixel, m * 4, cudaMemcpyDeviceToHost, s.st);
-        cudaMemcpyAsync(h_out->surface + done, s.surface, m * 4, cudaMemcpyDeviceToHost, s.st);
-        cudaMemcpyAsync(h_out->state + done, s.state, m, cudaMemcpyDeviceToHost, s.st);
-        cudaMemcpyAsync(h_out->bounces + done, s.bounces, m, cudaMemcpyDeviceToHost, s.st);
-        done += m;
-        k = (k + 1) % kSlots;
-    }
-    // join
-    for (int j = 0; j < kSlots; ++j) { cudaEventRecord(slot[j].done, slot[j].st); cudaStreamWaitEvent(main, slot[j].done, 0); }
-    std::vector<uint32_t> hm(scene->n_pixels);
-    uint64_t cnt[8] = {0};
-    if (scene->n_pixels) cudaMemcpyAsync(hm.data(), d_hitmap, scene->n_pixels * 4, cudaMemcpyDeviceToHost, main);
-    cudaMemcpyAsync(cnt, d_counters, 64, cudaMemcpyDeviceToHost, main);
-    cudaError_t e = cudaStreamSynchronize(main);
-    for (int j = 0; j < kSlots; ++j) { cudaStreamDestroy(slot[j].st); cudaEventDestroy(slot[j].done); }
-    cudaEventDestroy(start);
-    if (st != OPX_OK) return st;
-    if (e != cudaSuccess) return check_cuda(e, "opx_propagate_host");
-    for (uint64_t i = 0; i < scene->n_pixels; ++i) h_hitmap[i] += hm[i];
-    if (h_counters) for (int i = 0; i < 8; ++i) h_counters[i] += cnt[i];
-    return OPX_OK;
+opx_status opx_propagate_host_detected(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* h_origins,
+                                       const float* h_dirs, const float* h_wavelengths, uint64_t seed, uint32_t flags,
+                                       const opx_detected* h_out, uint64_t capacity, uint64_t* h_n_detected, uint32_t* h_hitmap,
+                                       uint64_t* h_counters, void* d_workspace, size_t workspace_bytes, uint64_t chunk, void* cuda_stream) {
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate_host_detected before opx_bvh_build");
+    if (flags & ~(uint32_t)OPX_FLAG_NO_EFFICIENCY) return fail(OPX_ERR_INVALID_ARG, "unknown flag");
+    if (!h_n_detected) return fail(OPX_ERR_INVALID_ARG, "h_n_detected is NULL");
+    *h_n_detected = 0;
+    if (n == 0) return OPX_OK;
+    if (!h_origins || !h_dirs || !h_wavelengths || !h_out || !d_workspace || chunk == 0 || capacity == 0)
+        return fail(OPX_ERR_INVALID_ARG, "NULL argument, chunk = 0 or capacity = 0");
+    if (!h_out->id || !h_out->pixel || !h_out->pos || !h_out->dir) return fail(OPX_ERR_INVALID_ARG, "NULL list array");
+    if (!h_hitmap && scene->n_pixels) return fail(OPX_ERR_INVALID_ARG, "h_hitmap is NULL but the scene has pixels");
+    if (scene->tri_surface.size() < 2) return fail(OPX_ERR_BAD_STATE, "the detected-only output needs a scene of two triangles or more");
+    if (misaligned(d_workspace, 256)) return fail(OPX_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    if (workspace_bytes < host_workspace_bytes(*scene, chunk, false, capacity)) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_propagate_host_detected_workspace_bytes)");
+    if (opx_status st = device_ok()) return st;
+    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_propagate_host_detected")) return st;
+    return propagate_host_impl(*scene, n, photon_id_base, h_origins, h_dirs, h_wavelengths, seed, flags, nullptr, h_out, capacity,
+                               h_n_detected, h_hitmap, h_counters, d_workspace, chunk, (cudaStream_t)cuda_stream);
 }
 
 opx_status opx_scene_info(const opx_scene* scene, uint64_t* n_triangles, uint64_t* n_nodes, uint64_t* n_pixels,

@@ -245,8 +245,11 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayR&
         const unsigned mn = __ballot_sync(full, go);
         if (mn) {
             // nearest child next, the others onto the stack with their entry bounds (tn >= 0: bit patterns order like values)
-            const int kmin = __reduce_min_sync(full, go ? __float_as_int(tn) : 0x7fffffff);
-            const int L = __ffs(__ballot_sync(full, go && __float_as_int(tn) == kmin)) - 1;
+            int L = __ffs(mn) - 1;
+            if (mn & (mn - 1u)) {          // several children: the one the beam enters first
+                const int kmin = __reduce_min_sync(full, go ? __float_as_int(tn) : 0x7fffffff);
+                L = __ffs(__ballot_sync(full, go && __float_as_int(tn) == kmin)) - 1;
+            }
             const unsigned rest = mn & ~(1u << L);
             if (rest) {
                 const int k = __popc(rest);

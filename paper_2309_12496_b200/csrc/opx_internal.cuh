@@ -57,6 +57,23 @@ struct SceneDev {
 
 struct Layout : opx_scene_layout {};
 
+// A list of detected photons (opx_detected) as the kernels see it.  Inside a detected-only launch of the propagation kernel
+// it describes the STAGING list of that launch (opx_packet.cuh, step 4b): tiles append their chunks at offsets taken from
+// *stage_count and note them in tile_table.
+struct DetOut {
+    unsigned long long* id;      // NULL: this launch writes no detected list
+    int32_t* pixel;
+    float* pos;
+    float* dir;
+    unsigned long long capacity;
+    unsigned long long* stage_count;   // entries handed out so far (zero at launch)
+    ulonglong2* tile_table;            // (staging offset, count) per tile
+};
+
+// Streams and events of the host-buffer calls (opx_propagate_host*), created once per scene at the first such call.
+struct HostPipe;
+void destroy_host_pipe(HostPipe* p);
+
 // ------------------------------------------------------------------------------ host-side scene
 struct SceneHost {
     opx_scene_params params{};
@@ -80,7 +97,8 @@ struct SceneHost {
     // opx_profile_begin/end: event triples (start, after propagate, after bin), one per call
     mutable std::vector<cudaEvent_t> prof_events;
     mutable uint32_t prof_max = 0, prof_used = 0;
-    ~SceneHost() { for (cudaEvent_t e : prof_events) cudaEventDestroy(e); }
+    mutable HostPipe* pipe = nullptr;
+    ~SceneHost() { for (cudaEvent_t e : prof_events) cudaEventDestroy(e); destroy_host_pipe(pipe); }
 };
 
 // error plumbing (opx_api.cu)
@@ -106,6 +124,12 @@ opx_status device_ok();
 opx_status launch_propagate(const SceneHost& s, WalkMode mode, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
                             const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_hits& out,
                             uint32_t* hitmap, uint64_t* counters, cudaStream_t stream);
+// the same launch writing the detected photons only, appended to a list in photon-id order (DetOut above)
+opx_status launch_propagate_detected(const SceneHost& s, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
+                                     const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_detected& list,
+                                     uint64_t capacity, uint64_t* d_n_detected, void* workspace, uint32_t* hitmap, uint64_t* counters,
+                                     cudaStream_t stream);
+size_t detected_workspace_bytes(uint64_t n, uint64_t capacity);
 // pre-propagation filter (opx_prefilter.cu)
 size_t prefilter_workspace_bytes(uint64_t n);
 opx_status launch_prefilter(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d, const float* wl,

@@ -91,6 +91,58 @@ __device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t by
 }
 __device__ __forceinline__ bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
+// Second and third step of a detected-only launch (the first is the store phase of k_propagate_packet).  `stage` holds the
+// detected photons tile by tile in the order the tiles finished, table[b] = (offset, count) of tile b.
+// k_det_scan (one CTA): exclusive prefix of the staged counts in tile order -> table[b].x becomes the tile's position in the
+// caller's list (after the entries already there), table[b].y keeps the staged count, the staging offset moves to src[b];
+// *n_detected grows by the TRUE number of detections.  A tile's chunk is staged only as far as the staging area reaches
+// (capacity entries, like the list): an overflow therefore implies *n_detected > capacity, which is how the caller learns
+// that the list is incomplete.
+__global__ void __launch_bounds__(1024) k_det_scan(ulonglong2* table, unsigned long long* src, unsigned long long tiles,
+                                                   unsigned long long stage_capacity, unsigned long long* n_detected,
+                                                   unsigned long long* stage_count) {
+    __shared__ unsigned long long s_warp[32];
+    __shared__ unsigned long long s_run;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_run = 0ull;
+    __syncthreads();
+    const unsigned long long list_base = *n_detected;
+    for (unsigned long long b0 = 0; b0 < tiles; b0 += 1024) {
+        const unsigned long long b = b0 + threadIdx.x;
+        ulonglong2 e = make_ulonglong2(0ull, 0ull);
+        if (b < tiles) e = table[b];
+        const unsigned long long staged = e.x >= stage_capacity ? 0ull : (e.x + e.y > stage_capacity ? stage_capacity - e.x : e.y);
+        unsigned long long inc = staged;
+        for (int o2 = 1; o2 < 32; o2 <<= 1) { const unsigned long long y = __shfl_up_sync(0xffffffffu, inc, o2); if (lane >= o2) inc += y; }
+        if (lane == 31) s_warp[w] = inc;
+        __syncthreads();
+        unsigned long long before = s_run;
+        for (int k = 0; k < w; ++k) before += s_warp[k];
+        if (b < tiles) { src[b] = e.x; table[b] = make_ulonglong2(list_base + before + inc - staged, staged); }
+        __syncthreads();
+        if (threadIdx.x == 1023) s_run = before + inc;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { *n_detected = list_base + *stage_count; *stage_count = 0ull; }
+}
+
+// One warp per tile: copies the tile's staged chunk to its place in the caller's list (entries beyond the capacity dropped).
+__global__ void __launch_bounds__(256) k_det_gather(const ulonglong2* __restrict__ table, const unsigned long long* __restrict__ src,
+                                                    unsigned long long tiles, DetOut stage, DetOut out) {
+    const unsigned long long b = (blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x) >> 5;
+    if (b >= tiles) return;
+    const int lane = threadIdx.x & 31;
+    const ulonglong2 e = table[b];
+    const unsigned long long from = src[b];
+    for (unsigned long long k = lane; k < e.y; k += 32) {
+        const unsigned long long r = e.x + k, q = from + k;
+        if (r >= out.capacity) break;
+        out.id[r] = stage.id[q]; out.pixel[r] = stage.pixel[q];
+        out.pos[3 * r] = stage.pos[3 * q]; out.pos[3 * r + 1] = stage.pos[3 * q + 1]; out.pos[3 * r + 2] = stage.pos[3 * q + 2];
+        out.dir[3 * r] = stage.dir[3 * q]; out.dir[3 * r + 1] = stage.dir[3 * q + 1]; out.dir[3 * r + 2] = stage.dir[3 * q + 2];
+    }
+}
+
 // Octahedral map of a direction to [-1,1]^2 (NaN-safe: garbage maps to 0,0).
 __device__ __forceinline__ void octa(float dx, float dy, float dz, float& u, float& v) {
     const float s = fabsf(dx) + fabsf(dy) + fabsf(dz);
@@ -242,7 +294,7 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
                                                                      const float* __restrict__ dirs,
                                                                      const float* __restrict__ wl, uint64_t seed, opx_hits out,
                                                                      uint32_t* hitmap, unsigned long long* counters,
-                                                                     unsigned long long* stats) {
+                                                                     unsigned long long* stats, const DetOut det) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     using PacketSmem = PacketSmemT<kPktThreads, kItems>;
     constexpr int kPktWarps = PacketSmem::kPktWarps, kTile = PacketSmem::kTile;
@@ -478,6 +530,51 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
             __syncthreads();
             if (threadIdx.x < 8 && s_cnt[threadIdx.x]) atomicAdd(&counters[threadIdx.x], (unsigned long long)s_cnt[threadIdx.x]);
         }
+    }
+
+    // 4b. detected-only output (opx_propagate_detected): the tile's DETECTED photons go, in id order, to a staging list at an
+    //     offset taken from a global counter (so tiles land in the order they finish and nobody waits for anybody), and the
+    //     tile notes (offset, count) in a table; k_det_scan / k_det_gather then move the chunks to the caller's list in tile
+    //     order = photon-id order.  (A single-pass look-back scan inside this kernel was measured first: on the C4 scene,
+    //     where tile times differ by a factor of several, finished CTAs spinning for their predecessors halved the rate.)
+    if (det.id) {
+        constexpr int kChunks = kTile / 32;                  // <= 64: two per lane of warp 0
+        static_assert(kChunks <= 64 && kTile % 32 == 0, "chunk scan layout");
+        uint32_t* s_chunk = &sm.cnt[0][0];                   // free since the traversal ended (aliases the warps' stacks)
+        unsigned long long* s_base = reinterpret_cast<unsigned long long*>(s_chunk + 64);
+        __syncthreads();
+        for (int k = threadIdx.x; k < kTile; k += kPktThreads) {
+            const unsigned dm = __ballot_sync(0xffffffffu, k < m && sm.state[k] == OPX_DETECTED);
+            if (lane == 0) s_chunk[k >> 5] = __popc(dm);
+        }
+        __syncthreads();
+        if (w == 0) {
+            const uint32_t c0 = 2 * lane < kChunks ? s_chunk[2 * lane] : 0u, c1 = 2 * lane + 1 < kChunks ? s_chunk[2 * lane + 1] : 0u;
+            uint32_t inc = c0 + c1;
+            for (int o2 = 1; o2 < 32; o2 <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o2); if (lane >= o2) inc += y; }
+            const uint32_t total = __shfl_sync(0xffffffffu, inc, 31);
+            if (2 * lane < kChunks) s_chunk[2 * lane] = inc - c0 - c1;
+            if (2 * lane + 1 < kChunks) s_chunk[2 * lane + 1] = inc - c1;
+            if (lane == 0) {
+                const unsigned long long off = total ? atomicAdd(det.stage_count, (unsigned long long)total) : 0ull;
+                det.tile_table[blockIdx.x] = make_ulonglong2(off, (unsigned long long)total);
+                *s_base = off;
+            }
+        }
+        __syncthreads();
+        const unsigned long long base = *s_base;
+        for (int k = threadIdx.x; k < kTile; k += kPktThreads) {
+            const bool isdet = k < m && sm.state[k] == OPX_DETECTED;
+            const unsigned dm = __ballot_sync(0xffffffffu, isdet);
+            const unsigned long long r = base + s_chunk[k >> 5] + __popc(dm & ((1u << lane) - 1u));
+            if (isdet && r < det.capacity) {
+                det.id[r] = id_base + tile_base + (uint64_t)k;
+                det.pixel[r] = __float_as_int(sm.wl[k]);
+                det.pos[3 * r] = sm.o[3 * k]; det.pos[3 * r + 1] = sm.o[3 * k + 1]; det.pos[3 * r + 2] = sm.o[3 * k + 2];
+                det.dir[3 * r] = sm.d[3 * k]; det.dir[3 * r + 1] = sm.d[3 * k + 1]; det.dir[3 * r + 2] = sm.d[3 * k + 2];
+            }
+        }
+        return;            // a detected-only launch writes no per-photon records
     }
 
     // 4. write the tile's records: six TMA bulk stores by one thread for a full, aligned tile, else coalesced streaming stores

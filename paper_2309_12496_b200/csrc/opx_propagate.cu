@@ -36,7 +36,8 @@ opx_status configure_device() {
 
 static opx_status launch_propagate_impl(const SceneHost& s, WalkMode mode, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
                                         const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_hits& out,
-                                        uint32_t* hitmap, uint64_t* counters, uint64_t* packet_stats, cudaStream_t stream) {
+                                        uint32_t* hitmap, uint64_t* counters, uint64_t* packet_stats, cudaStream_t stream,
+                                        DetOut det = DetOut{}, uint64_t* det_tiles = nullptr) {
     SceneDev dev = s.dev;          // per-launch copy: flags and the optional device-side count ride in the kernel parameter
     dev.flags = flags;
     dev.d_n = (const unsigned long long*)d_n;
@@ -46,6 +47,7 @@ static opx_status launch_propagate_impl(const SceneHost& s, WalkMode mode, uint6
     if (s.prof_used < s.prof_max) { ev = &s.prof_events[3 * (size_t)s.prof_used]; ++s.prof_used; }
     if (ev) cudaEventRecord(ev[0], stream);
     bool binned = false;         // A11/A12 done inside the propagation kernel
+    if (det.id && (brute || s.dev.n_tri < 2)) return fail(OPX_ERR_BAD_STATE, "the detected-only output needs a scene with a hierarchy (two triangles or more)");
     if (brute || s.dev.n_tri < 2) {
         // debug mode, or a scene with fewer than two triangles (no hierarchy): test the triangle list directly
         const uint64_t blocks = (n + 127) / 128;
@@ -71,11 +73,12 @@ static opx_status launch_propagate_impl(const SceneHost& s, WalkMode mode, uint6
         const uint64_t tile = small ? Small::kTile : (mid ? Mid::kTile : (lean ? Lean::kTile : Big::kTile));
         const uint64_t tiles = (n + tile - 1) / tile;
         if (tiles > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
-        if (packet_stats) k_propagate_packet<512, 4, 2, true><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr, nullptr, (unsigned long long*)packet_stats);
-        else if (lean) k_propagate_packet<448, 4, 2, false><<<(unsigned)tiles, 448, sizeof(Lean), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
-        else if (mid) k_propagate_packet<256, 4, 4, false><<<(unsigned)tiles, 256, sizeof(Mid), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
-        else if (small) k_propagate_packet<512, 1, 2, false><<<(unsigned)tiles, 512, sizeof(Small), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
-        else k_propagate_packet<512, 4, 2, false><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr);
+        if (det_tiles) *det_tiles = tiles;
+        if (packet_stats) k_propagate_packet<512, 4, 2, true><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr, nullptr, (unsigned long long*)packet_stats, det);
+        else if (lean) k_propagate_packet<448, 4, 2, false><<<(unsigned)tiles, 448, sizeof(Lean), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det);
+        else if (mid) k_propagate_packet<256, 4, 4, false><<<(unsigned)tiles, 256, sizeof(Mid), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det);
+        else if (small) k_propagate_packet<512, 1, 2, false><<<(unsigned)tiles, 512, sizeof(Small), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det);
+        else k_propagate_packet<512, 4, 2, false><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det);
         // the names ncu prints for these instantiations
         set_last_kernel(packet_stats ? "k_propagate_packet<512, 4, 2, 1>" : lean ? "k_propagate_packet<448, 4, 2, 0>" : mid ? "k_propagate_packet<256, 4, 4, 0>"
                         : small ? "k_propagate_packet<512, 1, 2, 0>" : "k_propagate_packet<512, 4, 2, 0>");
@@ -97,6 +100,42 @@ opx_status launch_propagate(const SceneHost& s, WalkMode mode, uint64_t n, const
                             const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_hits& out, uint32_t* hitmap,
                             uint64_t* counters, cudaStream_t stream) {
     return launch_propagate_impl(s, mode, n, d_n, id_base, o, d, wl, seed, flags, out, hitmap, counters, nullptr, stream);
+}
+
+// Workspace of a detected-only launch: the counter of the staging list, the tile table (16 B) and the staging offsets (8 B)
+// per tile of the smallest tile size, and a staging list of `capacity` entries.
+struct DetWorkspace { unsigned long long* count; ulonglong2* table; unsigned long long* src; DetOut stage; size_t bytes; };
+static DetWorkspace det_workspace(void* ws, uint64_t n, uint64_t capacity) {
+    const uint64_t tiles = (n + Small::kTile - 1) / Small::kTile + 1;
+    char* p = (char*)ws;
+    auto take = [&](size_t bytes) { char* r = p; p += align_up(bytes, 256); return r; };
+    DetWorkspace w{};
+    w.count = (unsigned long long*)take(256);
+    w.table = (ulonglong2*)take(tiles * 16);
+    w.src = (unsigned long long*)take(tiles * 8);
+    w.stage.id = (unsigned long long*)take(capacity * 8); w.stage.pixel = (int32_t*)take(capacity * 4);
+    w.stage.pos = (float*)take(capacity * 12); w.stage.dir = (float*)take(capacity * 12);
+    w.stage.capacity = capacity; w.stage.stage_count = w.count; w.stage.tile_table = w.table;
+    w.bytes = (size_t)(p - (char*)ws);
+    return w;
+}
+size_t detected_workspace_bytes(uint64_t n, uint64_t capacity) { return det_workspace(nullptr, n, capacity).bytes; }
+
+opx_status launch_propagate_detected(const SceneHost& s, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
+                                     const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_detected& list,
+                                     uint64_t capacity, uint64_t* d_n_detected, void* workspace, uint32_t* hitmap, uint64_t* counters,
+                                     cudaStream_t stream) {
+    const DetWorkspace w = det_workspace(workspace, n, capacity);
+    // the counter and the whole tile table start at zero: tiles beyond a device-side photon count never run and must read (0, 0)
+    if (opx_status st = check_cuda(cudaMemsetAsync(w.count, 0, (size_t)((char*)w.src - (char*)w.count), stream), "cudaMemsetAsync")) return st;
+    uint64_t tiles = 0;
+    if (opx_status st = launch_propagate_impl(s, kWalkProduct, n, d_n, id_base, o, d, wl, seed, flags, opx_hits{}, hitmap, counters, nullptr,
+                                              stream, w.stage, &tiles)) return st;
+    k_det_scan<<<1, 1024, 0, stream>>>(w.table, w.src, tiles, capacity, (unsigned long long*)d_n_detected, w.count);
+    DetOut out{(unsigned long long*)list.id, list.pixel, list.pos, list.dir, capacity, nullptr, nullptr};
+    k_det_gather<<<(unsigned)((tiles * 32 + 255) / 256), 256, 0, stream>>>(w.table, w.src, tiles, w.stage, out);
+    count_launch(2);
+    return check_cuda(cudaGetLastError(), "detected-list launch");
 }
 
 opx_status launch_packet_stats(const SceneHost& s, uint64_t n, uint64_t id_base, const float* o, const float* d,

@@ -25,6 +25,8 @@ TABLE_LINEAR, TABLE_HISTOGRAM = 0, 1     # opx_table_interp
 EXPORTS = ("opx_scene_create", "opx_scene_workspace_bytes", "opx_bvh_build", "opx_propagate",
            "opx_propagate_flags", "opx_prefilter_workspace_bytes", "opx_prefilter", "opx_emit_cherenkov",
            "opx_emit_cherenkov_filtered", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
+           "opx_propagate_detected_workspace_bytes", "opx_propagate_detected",
+           "opx_propagate_host_detected_workspace_bytes", "opx_propagate_host_detected",
            "opx_scene_info", "opx_scene_get_layout", "opx_scene_destroy", "opx_last_error", "opx_version")
 # ... and the debugging / measurement exports (include/opx_debug.h) that tests and bench.py use
 DEBUG_EXPORTS = ("opx_propagate_brute", "opx_propagate_binary", "opx_profile_begin", "opx_profile_end", "opx_propagate_stats",
@@ -61,6 +63,10 @@ class Mesh(C.Structure):
 class Hits(C.Structure):
     _fields_ = [("pos", C.c_void_p), ("dir", C.c_void_p), ("pixel", C.c_void_p), ("surface", C.c_void_p),
                 ("state", C.c_void_p), ("bounces", C.c_void_p)]
+
+
+class Detected(C.Structure):
+    _fields_ = [("id", C.c_void_p), ("pixel", C.c_void_p), ("pos", C.c_void_p), ("dir", C.c_void_p)]
 
 
 class TrackSteps(C.Structure):
@@ -104,6 +110,10 @@ def load_library(path=LIB_PATH):
                                                 vp, vp, vp, vp, u64, vp, vp, C.c_size_t, vp]
     lib.opx_propagate_host_workspace_bytes.argtypes = [vp, u64, vp]
     lib.opx_propagate_host.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp, vp, vp, C.c_size_t, u64, vp]
+    lib.opx_propagate_detected_workspace_bytes.argtypes = [u64, u64, vp]
+    lib.opx_propagate_detected.argtypes = [vp, u64, vp, u64, vp, vp, vp, u64, u32, vp, u64, vp, vp, C.c_size_t, vp, vp, vp]
+    lib.opx_propagate_host_detected_workspace_bytes.argtypes = [vp, u64, u64, vp]
+    lib.opx_propagate_host_detected.argtypes = [vp, u64, u64, vp, vp, vp, u64, u32, vp, u64, vp, vp, vp, vp, C.c_size_t, u64, vp]
     lib.opx_profile_begin.argtypes = [vp, u32]
     lib.opx_profile_end.argtypes = [vp, vp, vp, vp]
     lib.opx_propagate_stats.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp]
@@ -215,6 +225,7 @@ class Scene:
         self.n_triangles, self.n_nodes, self.n_pixels, self.n_surfaces = nt.value, nn.value, npix.value, ns.value
         self.workspace = None
         self._host_ws = None
+        self._det_ws = None
 
     def __del__(self):
         if getattr(self, "_h", None) and _lib is not None:
@@ -295,6 +306,68 @@ class Scene:
                       int(seed), C.byref(h), hitmap.data_ptr(), counters.data_ptr(), C.c_void_p(st.cuda_stream)))
         out = dict(records)
         out["hitmap"], out["counters"] = hitmap[:self.n_pixels], counters
+        return out
+
+    def alloc_detected(self, capacity, device="cuda"):
+        """Device arrays of an opx_detected list + its length (int64 view of uint64, zero)."""
+        import torch
+        return dict(id=torch.empty(capacity, dtype=torch.int64, device=device), pixel=torch.empty(capacity, dtype=torch.int32, device=device),
+                    pos=torch.empty((capacity, 3), dtype=torch.float32, device=device),
+                    dir=torch.empty((capacity, 3), dtype=torch.float32, device=device),
+                    n_detected=torch.zeros(1, dtype=torch.int64, device=device))
+
+    def propagate_detected(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, capacity=None, out=None, hitmap=None,
+                           counters=None, stream=None, flags=0, n_dev=None):
+        """opx_propagate_detected: the DETECTED photons appended to `out` (alloc_detected) in photon-id order; out["n_detected"]
+        is the running length on the device.  No per-photon records are written."""
+        import torch
+        n = int(wavelengths.shape[0])
+        dev = wavelengths.device
+        if out is None:
+            out = self.alloc_detected(n if capacity is None else int(capacity), dev)
+        cap = int(out["id"].shape[0])
+        if hitmap is None or counters is None:
+            hm, ct = self.alloc_accumulators(dev)
+            hitmap = hm if hitmap is None else hitmap
+            counters = ct if counters is None else counters
+        lib = load_library()
+        need = C.c_size_t()
+        _check(lib.opx_propagate_detected_workspace_bytes(n, cap, C.byref(need)))
+        if self._det_ws is None or self._det_ws.numel() < need.value + 256 or self._det_ws.device != dev:
+            self._det_ws = torch.empty(need.value + 256, dtype=torch.uint8, device=dev)
+        d = Detected(*(out[k].data_ptr() for k in ("id", "pixel", "pos", "dir")))
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        _check(lib.opx_propagate_detected(self._h, n, None if n_dev is None else n_dev.data_ptr(), int(photon_id_base),
+                                          origins.data_ptr(), dirs.data_ptr(), wavelengths.data_ptr(), int(seed), int(flags),
+                                          C.byref(d), cap, out["n_detected"].data_ptr(), _aligned(self._det_ws), need.value,
+                                          hitmap.data_ptr(), counters.data_ptr(), C.c_void_p(st.cuda_stream)))
+        res = dict(out)
+        res["hitmap"], res["counters"] = hitmap[:self.n_pixels], counters
+        return res
+
+    def propagate_host_detected(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, capacity=None, chunk=1 << 20, out=None,
+                                stream=None, device="cuda", flags=0):
+        """opx_propagate_host_detected: host photon buffers in, the list of detected photons (host) + hit-map + counters out."""
+        import torch
+        lib = load_library()
+        n = int(wavelengths.shape[0])
+        chunk = max(1, min(int(chunk), max(n, 1)))
+        if out is None:
+            out = alloc_host_detected(max(1, n if capacity is None else int(capacity)), self.n_pixels)
+        cap = int(out["id"].shape[0])
+        need = C.c_size_t()
+        _check(lib.opx_propagate_host_detected_workspace_bytes(self._h, chunk, cap, C.byref(need)))
+        if self._host_ws is None or self._host_ws.numel() < need.value + 256:
+            self._host_ws = torch.empty(need.value + 256, dtype=torch.uint8, device=device)
+        ptr = (lambda t: t.data_ptr()) if isinstance(wavelengths, torch.Tensor) else (lambda a: a.ctypes.data)
+        d = Detected(*(out[k].data_ptr() for k in ("id", "pixel", "pos", "dir")))
+        nd = C.c_uint64(0)
+        st = stream if stream is not None else torch.cuda.current_stream(device)
+        _check(lib.opx_propagate_host_detected(self._h, n, int(photon_id_base), ptr(origins), ptr(dirs), ptr(wavelengths), int(seed),
+                                               int(flags), C.byref(d), cap, C.byref(nd), out["hitmap"].data_ptr(),
+                                               out["counters"].data_ptr(), _aligned(self._host_ws), need.value, chunk,
+                                               C.c_void_p(st.cuda_stream)))
+        out["n_detected"] = int(nd.value)
         return out
 
     def prefilter(self, origins, dirs, wavelengths, factors, seed=0, photon_id_base=0, out=None, stream=None, capacity=None):
@@ -438,6 +511,16 @@ def alloc_host_records(n, n_pixels):
                hitmap=torch.zeros(max(1, n_pixels), dtype=torch.int32, pin_memory=pin),
                counters=torch.zeros(8, dtype=torch.int64, pin_memory=pin))
     return out
+
+
+def alloc_host_detected(capacity, n_pixels):
+    """Pinned host buffers for opx_propagate_host_detected (hitmap and counters zeroed)."""
+    import torch
+    pin = torch.cuda.is_available()
+    mk = lambda shape, dt: torch.empty(shape, dtype=dt, pin_memory=pin)
+    return dict(id=mk((capacity,), torch.int64), pixel=mk((capacity,), torch.int32), pos=mk((capacity, 3), torch.float32),
+                dir=mk((capacity, 3), torch.float32), hitmap=torch.zeros(max(1, n_pixels), dtype=torch.int32, pin_memory=pin),
+                counters=torch.zeros(8, dtype=torch.int64, pin_memory=pin))
 
 
 def _aligned(t, a=256):
