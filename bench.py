@@ -444,30 +444,71 @@ def main():
     value = world * n * args.steps / (ms_total * 1e-3)
     cnt = counters.cpu().numpy()
 
-    # ---- end to end through the C ABI with host buffers (copies inside the timed region)
+    # ---- end to end through the C ABI with host buffers (copies inside the timed region).  The headline form returns what the
+    #      paper asks for: the list of DETECTED photons + hit-map + counters; `records` is the same call returning
+    #      every photon's 34-byte record; `tracks` starts from the track steps in host memory, so that the photons
+    #      never cross the link at all.
     e2e = None
     if rank == 0 or dist is not None:
-        host_out = pkg.alloc_host_records(n, scene.n_pixels)
-        chunk = min(n, 1 << 20)
-        scene.propagate_host(*pin, seed=args.seed, photon_id_base=id_base, chunk=chunk, out=host_out, stream=stream)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for _ in range(args.e2e_steps):
-            host_out["hitmap"].zero_(); host_out["counters"].zero_()
-            scene.propagate_host(*pin, seed=args.seed, photon_id_base=id_base, chunk=chunk, out=host_out, stream=stream)
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": world * n * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": BYTES_IN * n,
-               "d2h_bytes_per_step": BYTES_OUT * n + 4 * scene.n_pixels + 64, "chunk_photons": chunk,
-               "ms_per_step": 1e3 * dt / args.e2e_steps,
-               "what": "opx_propagate_host: pinned host photon arrays in, every photon's hit record + hit-map + counters out"}
-        if dist is None and not np.array_equal(host_out["counters"].numpy(), cnt):
+        def wall(fn, k):
+            fn()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(k):
+                fn()
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            if dist is not None:
+                t = torch.tensor([dt], device=dev, dtype=torch.float64)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                dt = float(t.item())
+            return dt / k
+        chunk = min(n, 1 << 21)
+        cap = max(4096, int(1.25 * int(cnt[0])) + 4096)
+        host_det = pkg.alloc_host_detected(cap, scene.n_pixels)
+
+        def e2e_step():
+            host_det["hitmap"].zero_(); host_det["counters"].zero_()
+            scene.propagate_host_detected(*pin, seed=args.seed, photon_id_base=id_base, chunk=chunk, out=host_det, stream=stream)
+        dt = wall(e2e_step, args.e2e_steps)
+        n_det = int(host_det["n_detected"])
+        e2e = {"value": world * n / dt, "unit": UNIT, "h2d_bytes_per_step": BYTES_IN * n,
+               "d2h_bytes_per_step": 36 * n_det + 4 * scene.n_pixels + 72, "chunk_photons": chunk, "ms_per_step": 1e3 * dt,
+               "detected_per_step": n_det,
+               "what": "opx_propagate_host_detected: pinned host photon arrays in (28 B/photon), the list of detected photons "
+                       "(id, pixel, position, direction: 36 B each) + hit-map + counters out"}
+        if dist is None and (n_det != int(cnt[0]) or not np.array_equal(host_det["counters"].numpy(), cnt)):
             raise SystemExit("bench: host path and device path disagree")
-        del host_out
+        del host_det
+        if dist is None:
+            host_out = pkg.alloc_host_records(n, scene.n_pixels)
+            chunk_r = min(n, 1 << 20)
+
+            def rec_step():
+                host_out["hitmap"].zero_(); host_out["counters"].zero_()
+                scene.propagate_host(*pin, seed=args.seed, photon_id_base=id_base, chunk=chunk_r, out=host_out, stream=stream)
+            dt = wall(rec_step, args.e2e_steps)
+            e2e["records"] = {"value": n / dt, "unit": UNIT, "h2d_bytes_per_step": BYTES_IN * n,
+                              "d2h_bytes_per_step": BYTES_OUT * n + 4 * scene.n_pixels + 64, "chunk_photons": chunk_r, "ms_per_step": 1e3 * dt,
+                              "what": "opx_propagate_host: the same with every photon's 34-byte hit record brought back"}
+            if not np.array_equal(host_out["counters"].numpy(), cnt):
+                raise SystemExit("bench: host record path and device path disagree")
+            del host_out
+            if w.track_source is not None and id_base == 0:
+                steps_h = w.track_source.steps()
+                kinds_ = [m["kind"] for m in w.scene.materials]
+                fac_ = [kinds_.index(2)] + [kinds_.index(1)] * (2 if args.config in ("C4", "C5") else 1)
+                tr = {}
+                for name, fac in (("in_flight", ()), ("paper_filter", fac_)):
+                    hd = pkg.alloc_host_detected(cap, scene.n_pixels)
+                    dt = wall(lambda: scene.tracks_host_detected(steps_h, n, factors=fac, seed=args.seed, out=hd, chunk=min(n, 1 << 26), stream=stream),
+                              args.e2e_steps)
+                    tr[name] = {"value": n / dt, "unit": UNIT, "ms_per_step": 1e3 * dt, "detected_per_step": int(hd["n_detected"]),
+                                "h2d_bytes_per_step": 40 * len(steps_h["length"]) + 8, "d2h_bytes_per_step": 36 * int(hd["n_detected"]) + 4 * scene.n_pixels + 72}
+                    del hd
+                e2e["tracks"] = dict(tr, what="opx_tracks_host_detected: track steps in host memory in (40 B/step), photons generated and "
+                                              "propagated on the device, list of detected photons out; in_flight = efficiencies drawn per "
+                                              "interaction, paper_filter = the paper's pre-propagation filter fused with the emission")
 
     if rank != 0:
         if dist is not None:

@@ -283,13 +283,16 @@ typedef struct {
  * nobody asked for.  Three launches and one memset, no host round trip: the propagation kernel stages each tile's
  * detected photons in the workspace in the order the tiles finish, a scan and a gather kernel move them to the list in
  * photon-id order.  d_workspace: opx_propagate_detected_workspace_bytes(n, capacity) device bytes, 256-byte aligned, used
- * while the call's kernels run.  Needs a scene of two triangles or more (OPX_ERR_BAD_STATE otherwise).  Other arguments
+ * while the call's kernels run.  d_index (DEVICE, n entries, may be NULL): when the inputs are the survivors of
+ * opx_prefilter / opx_emit_cherenkov_filtered, the index array that call wrote - the list then carries the ORIGINAL
+ * photon ids photon_id_base + d_index[i] (increasing, the filters being stable) instead of photon_id_base + i; it
+ * changes nothing else.  Needs a scene of two triangles or more (OPX_ERR_BAD_STATE otherwise).  Other arguments
  * and errors as in opx_propagate_flags. */
 opx_status opx_propagate_detected_workspace_bytes(uint64_t n, uint64_t capacity, size_t* bytes);
 opx_status opx_propagate_detected(const opx_scene* scene, uint64_t n, const uint64_t* d_n, uint64_t photon_id_base,
                                   const float* d_origins, const float* d_dirs, const float* d_wavelengths,
-                                  uint64_t seed, uint32_t flags, const opx_detected* out, uint64_t capacity,
-                                  uint64_t* d_n_detected, void* d_workspace, size_t workspace_bytes,
+                                  uint64_t seed, uint32_t flags, const uint32_t* d_index, const opx_detected* out,
+                                  uint64_t capacity, uint64_t* d_n_detected, void* d_workspace, size_t workspace_bytes,
                                   uint32_t* d_hitmap, uint64_t* d_counters, void* cuda_stream);
 
 /* Size of the device staging workspace opx_propagate_host needs for chunks of `chunk` photons. */
@@ -320,6 +323,24 @@ opx_status opx_propagate_host_detected(const opx_scene* scene, uint64_t n, uint6
                                        uint64_t seed, uint32_t flags, const opx_detected* h_out, uint64_t capacity,
                                        uint64_t* h_n_detected, uint32_t* h_hitmap, uint64_t* h_counters,
                                        void* d_workspace, size_t workspace_bytes, uint64_t chunk, void* cuda_stream);
+
+/* The paper's whole loop, memory-resident (photons are written to a file by Geant4 today, "the rendering
+ * loop" should run from memory): track steps in HOST memory in, the list of detected photons in HOST memory out; the photons
+ * themselves never exist outside the device.  h_steps holds HOST pointers (opx_track_steps); photons photon_id_base ..
+ * photon_id_base + n - 1 of its first[] are generated (opx_emit_cherenkov) and propagated in chunks of `chunk`, the
+ * detected ones appended to h_out as in opx_propagate_host_detected.  n_factors = 0: efficiencies drawn in flight
+ * (opx_emit_cherenkov then opx_propagate_detected).  n_factors > 0: the paper's own pipeline - the pre-propagation filter
+ * on `factors` fused with the emission (opx_emit_cherenkov_filtered), the survivors traced with OPX_FLAG_NO_EFFICIENCY; the
+ * list carries the original photon ids either way.  By definition the result is that of those calls.  Moves 40 B per track
+ * step up and 36 B per detected photon down.  d_workspace: opx_tracks_host_detected_workspace_bytes(...) device bytes,
+ * 256-byte aligned.  chunk <= 2^32 - 1.  Synchronises `cuda_stream` before returning. */
+opx_status opx_tracks_host_detected_workspace_bytes(const opx_scene* scene, uint64_t n_steps, uint64_t chunk, uint64_t capacity,
+                                                    size_t* bytes);
+opx_status opx_tracks_host_detected(const opx_scene* scene, const opx_track_steps* h_steps, uint64_t n_total, float n_index,
+                                    float lambda1_nm, float lambda2_nm, uint64_t n, uint64_t photon_id_base, uint64_t seed,
+                                    const uint32_t* factors, uint32_t n_factors, const opx_detected* h_out, uint64_t capacity,
+                                    uint64_t* h_n_detected, uint32_t* h_hitmap, uint64_t* h_counters, void* d_workspace,
+                                    size_t workspace_bytes, uint64_t chunk, void* cuda_stream);
 
 opx_status opx_scene_info(const opx_scene* scene, uint64_t* n_triangles, uint64_t* n_nodes,
                           uint64_t* n_pixels, uint64_t* n_surfaces);

@@ -308,9 +308,9 @@ opx_status opx_propagate_detected_workspace_bytes(uint64_t n, uint64_t capacity,
 
 opx_status opx_propagate_detected(const opx_scene* scene, uint64_t n, const uint64_t* d_n, uint64_t photon_id_base,
                                   const float* d_origins, const float* d_dirs, const float* d_wavelengths, uint64_t seed,
-                                  uint32_t flags, const opx_detected* out, uint64_t capacity, uint64_t* d_n_detected,
-                                  void* d_workspace, size_t workspace_bytes, uint32_t* d_hitmap, uint64_t* d_counters,
-                                  void* cuda_stream) {
+                                  uint32_t flags, const uint32_t* d_index, const opx_detected* out, uint64_t capacity,
+                                  uint64_t* d_n_detected, void* d_workspace, size_t workspace_bytes, uint32_t* d_hitmap,
+                                  uint64_t* d_counters, void* cuda_stream) {
     if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
     if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_propagate_detected before opx_bvh_build");
     if (flags & ~(uint32_t)OPX_FLAG_NO_EFFICIENCY) return fail(OPX_ERR_INVALID_ARG, "unknown flag");
@@ -322,13 +322,13 @@ opx_status opx_propagate_detected(const opx_scene* scene, uint64_t n, const uint
     if (!d_hitmap && scene->n_pixels) return fail(OPX_ERR_INVALID_ARG, "d_hitmap is NULL but the scene has pixels");
     if (misaligned(d_origins, 4) || misaligned(d_dirs, 4) || misaligned(d_wavelengths, 4) || misaligned(out->id, 8) ||
         misaligned(out->pixel, 4) || misaligned(out->pos, 4) || misaligned(out->dir, 4) || misaligned(d_hitmap, 4) ||
-        misaligned(d_counters, 8) || misaligned(d_n, 8) || misaligned(d_workspace, 256))
+        misaligned(d_counters, 8) || misaligned(d_n, 8) || misaligned(d_index, 4) || misaligned(d_workspace, 256))
         return fail(OPX_ERR_INVALID_ARG, "misaligned pointer");
     if (workspace_bytes < detected_workspace_bytes(n, capacity)) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_propagate_detected_workspace_bytes)");
     if (scene->tri_surface.size() < 2) return fail(OPX_ERR_BAD_STATE, "the detected-only output needs a scene of two triangles or more");
     if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_propagate_detected")) return st;
     return launch_propagate_detected(*scene, n, d_n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, flags, *out, capacity,
-                                     d_n_detected, d_workspace, d_hitmap, d_counters, (cudaStream_t)cuda_stream);
+                                     d_n_detected, d_index, d_workspace, d_hitmap, d_counters, (cudaStream_t)cuda_stream);
 }
 
 // ------------------------------------------------------------------------- host-buffer streaming
@@ -470,8 +470,8 @@ static opx_status propagate_host_impl(const SceneHost& scene, uint64_t n, uint64
             // the chunks append to one list: a chunk's kernel starts after the previous chunk's (they would not overlap much
             // anyway: the uploads are what the pipeline waits for)
             if (prev >= 0) ck(cudaStreamWaitEvent(sst, pipe->kernel[prev], 0));
-            st = launch_propagate_detected(scene, m, nullptr, photon_id_base + done, s.o, s.d, s.wl, seed, flags, det, capacity, d_n_det, det_ws,
-                                           d_hitmap, d_counters, sst);
+            st = launch_propagate_detected(scene, m, nullptr, photon_id_base + done, s.o, s.d, s.wl, seed, flags, det, capacity, d_n_det, nullptr,
+                                           det_ws, d_hitmap, d_counters, sst);
             ck(cudaEventRecord(pipe->kernel[k], sst));
             prev = k;
         }
@@ -560,6 +560,117 @@ opx_status opx_propagate_host_detected(const opx_scene* scene, uint64_t n, uint6
     if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_propagate_host_detected")) return st;
     return propagate_host_impl(*scene, n, photon_id_base, h_origins, h_dirs, h_wavelengths, seed, flags, nullptr, h_out, capacity,
                                h_n_detected, h_hitmap, h_counters, d_workspace, chunk, (cudaStream_t)cuda_stream);
+}
+
+// ------------------------------------------------------------------------- from track steps (host) to detected photons (host)
+static size_t tracks_workspace_bytes(const SceneHost& s, uint64_t n_steps, uint64_t chunk, uint64_t capacity) {
+    size_t b = 2 * align_up(n_steps * 12, 256) + 2 * align_up(n_steps * 4, 256) + align_up((n_steps + 1) * 8, 256);     // step table
+    b += 2 * align_up(chunk * 12, 256) + 2 * align_up(chunk * 4, 256) + 256;                                          // photons of a chunk, index, count
+    b += prefilter_workspace_bytes(chunk) + detected_workspace_bytes(chunk, capacity);
+    b += align_up(capacity * 8, 256) + align_up(capacity * 4, 256) + 2 * align_up(capacity * 12, 256);               // the list on the device
+    b += align_up(s.n_pixels * 4 + 4, 256) + 256;
+    return b;
+}
+
+opx_status opx_tracks_host_detected_workspace_bytes(const opx_scene* scene, uint64_t n_steps, uint64_t chunk, uint64_t capacity, size_t* bytes) {
+    if (!scene || !bytes || chunk == 0 || capacity == 0 || chunk > 0xffffffffull) return fail(OPX_ERR_INVALID_ARG, "NULL argument, chunk = 0, chunk > 2^32 - 1 or capacity = 0");
+    *bytes = tracks_workspace_bytes(*scene, n_steps, chunk, capacity);
+    return OPX_OK;
+}
+
+opx_status opx_tracks_host_detected(const opx_scene* scene, const opx_track_steps* h_steps, uint64_t n_total, float n_index, float lambda1_nm,
+                                    float lambda2_nm, uint64_t n, uint64_t photon_id_base, uint64_t seed, const uint32_t* factors,
+                                    uint32_t n_factors, const opx_detected* h_out, uint64_t capacity, uint64_t* h_n_detected,
+                                    uint32_t* h_hitmap, uint64_t* h_counters, void* d_workspace, size_t workspace_bytes, uint64_t chunk,
+                                    void* cuda_stream) {
+    if (!scene || !h_steps) return fail(OPX_ERR_INVALID_ARG, "scene/steps is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_tracks_host_detected before opx_bvh_build");
+    if (!h_n_detected) return fail(OPX_ERR_INVALID_ARG, "h_n_detected is NULL");
+    *h_n_detected = 0;
+    if (!(lambda1_nm > 0.f) || !(lambda2_nm > lambda1_nm) || !std::isfinite(lambda2_nm) || !std::isfinite(n_index))
+        return fail(OPX_ERR_INVALID_ARG, "need 0 < lambda1 < lambda2 and a finite refractive index");
+    if (n_factors > 8 || (n_factors && !factors)) return fail(OPX_ERR_INVALID_ARG, "n_factors must be <= 8 and factors non-NULL");
+    for (uint32_t k = 0; k < n_factors; ++k) {
+        if (factors[k] >= scene->mat_kinds.size()) return fail(OPX_ERR_INVALID_ARG, "factor material index out of range");
+        if ((scene->mat_kinds[factors[k]] & 0xffu) == OPX_MAT_ABSORBER) return fail(OPX_ERR_INVALID_ARG, "an absorber has no efficiency table");
+    }
+    if (n == 0) return OPX_OK;
+    const uint64_t S = h_steps->n_steps;
+    if (S == 0 || !h_steps->x || !h_steps->w || !h_steps->length || !h_steps->beta || !h_steps->first)
+        return fail(OPX_ERR_INVALID_ARG, "empty or NULL step table");
+    if (photon_id_base > n_total || n > n_total - photon_id_base) return fail(OPX_ERR_INVALID_ARG, "photon ids beyond first[n_steps]");
+    if (!h_out || !h_out->id || !h_out->pixel || !h_out->pos || !h_out->dir || !d_workspace || chunk == 0 || capacity == 0 || chunk > 0xffffffffull)
+        return fail(OPX_ERR_INVALID_ARG, "NULL argument, chunk = 0, chunk > 2^32 - 1 or capacity = 0");
+    if (!h_hitmap && scene->n_pixels) return fail(OPX_ERR_INVALID_ARG, "h_hitmap is NULL but the scene has pixels");
+    if (scene->tri_surface.size() < 2) return fail(OPX_ERR_BAD_STATE, "the detected-only output needs a scene of two triangles or more");
+    if (misaligned(d_workspace, 256)) return fail(OPX_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    if (workspace_bytes < tracks_workspace_bytes(*scene, S, chunk, capacity)) return fail(OPX_ERR_WORKSPACE_TOO_SMALL, "workspace too small (see opx_tracks_host_detected_workspace_bytes)");
+    if (opx_status st = device_ok()) return st;
+    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_tracks_host_detected")) return st;
+
+    cudaStream_t main = (cudaStream_t)cuda_stream;
+    char* p = (char*)d_workspace;
+    auto take = [&](size_t bytes) { char* r = p; p += align_up(bytes, 256); return r; };
+    float* dx = (float*)take(S * 12); float* dw = (float*)take(S * 12); float* dl = (float*)take(S * 4); float* db = (float*)take(S * 4);
+    uint64_t* df = (uint64_t*)take((S + 1) * 8);
+    float* po = (float*)take(chunk * 12); float* pd = (float*)take(chunk * 12); float* pw = (float*)take(chunk * 4);
+    uint32_t* pidx = (uint32_t*)take(chunk * 4);
+    uint64_t* d_n_kept = (uint64_t*)take(256);
+    void* pf_ws = take(prefilter_workspace_bytes(chunk));
+    void* det_ws = take(detected_workspace_bytes(chunk, capacity));
+    opx_detected det{(uint64_t*)take(capacity * 8), (int32_t*)take(capacity * 4), (float*)take(capacity * 12), (float*)take(capacity * 12)};
+    uint32_t* d_hitmap = (uint32_t*)take(scene->n_pixels * 4 + 4);
+    uint64_t* d_counters = (uint64_t*)take(128);
+    uint64_t* d_n_det = d_counters + 8;
+
+    cudaError_t err = cudaSuccess;
+    auto ck = [&](cudaError_t e) { if (e != cudaSuccess && err == cudaSuccess) err = e; };
+    ck(cudaMemcpyAsync(dx, h_steps->x, S * 12, cudaMemcpyHostToDevice, main));
+    ck(cudaMemcpyAsync(dw, h_steps->w, S * 12, cudaMemcpyHostToDevice, main));
+    ck(cudaMemcpyAsync(dl, h_steps->length, S * 4, cudaMemcpyHostToDevice, main));
+    ck(cudaMemcpyAsync(db, h_steps->beta, S * 4, cudaMemcpyHostToDevice, main));
+    ck(cudaMemcpyAsync(df, h_steps->first, (S + 1) * 8, cudaMemcpyHostToDevice, main));
+    ck(cudaMemsetAsync(d_hitmap, 0, scene->n_pixels * 4 + 4, main));
+    ck(cudaMemsetAsync(d_counters, 0, 128, main));
+    const opx_track_steps dsteps{dx, dw, dl, db, df, S};
+    opx_status st = OPX_OK;
+    for (uint64_t done = 0; done < n && st == OPX_OK && err == cudaSuccess; done += chunk) {
+        const uint64_t m = n - done < chunk ? n - done : chunk;
+        const uint64_t base = photon_id_base + done;
+        if (n_factors) {
+            st = launch_emit_filtered(*scene, dsteps, n_index, lambda1_nm, lambda2_nm, m, base, seed, factors, n_factors, po, pd, pw, pidx, m,
+                                      d_n_kept, pf_ws, main);
+            if (st == OPX_OK)
+                st = launch_propagate_detected(*scene, m, d_n_kept, base, po, pd, pw, seed, OPX_FLAG_NO_EFFICIENCY, det, capacity, d_n_det, pidx,
+                                               det_ws, d_hitmap, d_counters, main);
+        } else {
+            st = launch_emit(dsteps, n_index, lambda1_nm, lambda2_nm, m, base, seed, po, pd, pw, main);
+            if (st == OPX_OK)
+                st = launch_propagate_detected(*scene, m, nullptr, base, po, pd, pw, seed, 0u, det, capacity, d_n_det, nullptr, det_ws, d_hitmap,
+                                               d_counters, main);
+        }
+    }
+    std::vector<uint32_t> hm(scene->n_pixels);
+    uint64_t cnt[9] = {0};
+    if (scene->n_pixels) ck(cudaMemcpyAsync(hm.data(), d_hitmap, scene->n_pixels * 4, cudaMemcpyDeviceToHost, main));
+    ck(cudaMemcpyAsync(cnt, d_counters, 72, cudaMemcpyDeviceToHost, main));
+    ck(cudaStreamSynchronize(main));
+    if (st == OPX_OK && err == cudaSuccess) {
+        const uint64_t have = cnt[8] < capacity ? cnt[8] : capacity;
+        if (have) {
+            ck(cudaMemcpyAsync(h_out->id, det.id, have * 8, cudaMemcpyDeviceToHost, main));
+            ck(cudaMemcpyAsync(h_out->pixel, det.pixel, have * 4, cudaMemcpyDeviceToHost, main));
+            ck(cudaMemcpyAsync(h_out->pos, det.pos, have * 12, cudaMemcpyDeviceToHost, main));
+            ck(cudaMemcpyAsync(h_out->dir, det.dir, have * 12, cudaMemcpyDeviceToHost, main));
+            ck(cudaStreamSynchronize(main));
+        }
+        *h_n_detected = cnt[8];
+    }
+    if (st != OPX_OK) return st;
+    if (err != cudaSuccess) return check_cuda(err, "opx_tracks_host_detected");
+    for (uint64_t i = 0; i < scene->n_pixels; ++i) h_hitmap[i] += hm[i];
+    if (h_counters) for (int i = 0; i < 8; ++i) h_counters[i] += cnt[i];
+    return OPX_OK;
 }
 
 opx_status opx_scene_info(const opx_scene* scene, uint64_t* n_triangles, uint64_t* n_nodes, uint64_t* n_pixels,

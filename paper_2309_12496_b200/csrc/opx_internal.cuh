@@ -68,6 +68,7 @@ struct DetOut {
     unsigned long long capacity;
     unsigned long long* stage_count;   // entries handed out so far (zero at launch)
     ulonglong2* tile_table;            // (staging offset, count) per tile
+    const uint32_t* index;             // optional: entry i of this launch is photon id_base + index[i] (the survivors of a filter)
 };
 
 // Streams and events of the host-buffer calls (opx_propagate_host*), created once per scene at the first such call.
@@ -127,8 +128,8 @@ opx_status launch_propagate(const SceneHost& s, WalkMode mode, uint64_t n, const
 // the same launch writing the detected photons only, appended to a list in photon-id order (DetOut above)
 opx_status launch_propagate_detected(const SceneHost& s, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
                                      const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_detected& list,
-                                     uint64_t capacity, uint64_t* d_n_detected, void* workspace, uint32_t* hitmap, uint64_t* counters,
-                                     cudaStream_t stream);
+                                     uint64_t capacity, uint64_t* d_n_detected, const uint32_t* d_index, void* workspace, uint32_t* hitmap,
+                                     uint64_t* counters, cudaStream_t stream);
 size_t detected_workspace_bytes(uint64_t n, uint64_t capacity);
 // pre-propagation filter (opx_prefilter.cu)
 size_t prefilter_workspace_bytes(uint64_t n);

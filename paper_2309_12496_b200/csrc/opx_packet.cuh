@@ -568,7 +568,7 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
             const unsigned dm = __ballot_sync(0xffffffffu, isdet);
             const unsigned long long r = base + s_chunk[k >> 5] + __popc(dm & ((1u << lane) - 1u));
             if (isdet && r < det.capacity) {
-                det.id[r] = id_base + tile_base + (uint64_t)k;
+                det.id[r] = id_base + (det.index ? (uint64_t)__ldg(det.index + tile_base + k) : tile_base + (uint64_t)k);
                 det.pixel[r] = __float_as_int(sm.wl[k]);
                 det.pos[3 * r] = sm.o[3 * k]; det.pos[3 * r + 1] = sm.o[3 * k + 1]; det.pos[3 * r + 2] = sm.o[3 * k + 2];
                 det.dir[3 * r] = sm.d[3 * k]; det.dir[3 * r + 1] = sm.d[3 * k + 1]; det.dir[3 * r + 2] = sm.d[3 * k + 2];

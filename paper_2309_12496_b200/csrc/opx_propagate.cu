@@ -123,16 +123,17 @@ size_t detected_workspace_bytes(uint64_t n, uint64_t capacity) { return det_work
 
 opx_status launch_propagate_detected(const SceneHost& s, uint64_t n, const uint64_t* d_n, uint64_t id_base, const float* o,
                                      const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_detected& list,
-                                     uint64_t capacity, uint64_t* d_n_detected, void* workspace, uint32_t* hitmap, uint64_t* counters,
-                                     cudaStream_t stream) {
-    const DetWorkspace w = det_workspace(workspace, n, capacity);
+                                     uint64_t capacity, uint64_t* d_n_detected, const uint32_t* d_index, void* workspace, uint32_t* hitmap,
+                                     uint64_t* counters, cudaStream_t stream) {
+    DetWorkspace w = det_workspace(workspace, n, capacity);
+    w.stage.index = d_index;
     // the counter and the whole tile table start at zero: tiles beyond a device-side photon count never run and must read (0, 0)
     if (opx_status st = check_cuda(cudaMemsetAsync(w.count, 0, (size_t)((char*)w.src - (char*)w.count), stream), "cudaMemsetAsync")) return st;
     uint64_t tiles = 0;
     if (opx_status st = launch_propagate_impl(s, kWalkProduct, n, d_n, id_base, o, d, wl, seed, flags, opx_hits{}, hitmap, counters, nullptr,
                                               stream, w.stage, &tiles)) return st;
     k_det_scan<<<1, 1024, 0, stream>>>(w.table, w.src, tiles, capacity, (unsigned long long*)d_n_detected, w.count);
-    DetOut out{(unsigned long long*)list.id, list.pixel, list.pos, list.dir, capacity, nullptr, nullptr};
+    DetOut out{(unsigned long long*)list.id, list.pixel, list.pos, list.dir, capacity, nullptr, nullptr, nullptr};
     k_det_gather<<<(unsigned)((tiles * 32 + 255) / 256), 256, 0, stream>>>(w.table, w.src, tiles, w.stage, out);
     count_launch(2);
     return check_cuda(cudaGetLastError(), "detected-list launch");

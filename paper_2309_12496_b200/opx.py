@@ -27,6 +27,7 @@ EXPORTS = ("opx_scene_create", "opx_scene_workspace_bytes", "opx_bvh_build", "op
            "opx_emit_cherenkov_filtered", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
            "opx_propagate_detected_workspace_bytes", "opx_propagate_detected",
            "opx_propagate_host_detected_workspace_bytes", "opx_propagate_host_detected",
+           "opx_tracks_host_detected_workspace_bytes", "opx_tracks_host_detected",
            "opx_scene_info", "opx_scene_get_layout", "opx_scene_destroy", "opx_last_error", "opx_version")
 # ... and the debugging / measurement exports (include/opx_debug.h) that tests and bench.py use
 DEBUG_EXPORTS = ("opx_propagate_brute", "opx_propagate_binary", "opx_profile_begin", "opx_profile_end", "opx_propagate_stats",
@@ -111,7 +112,10 @@ def load_library(path=LIB_PATH):
     lib.opx_propagate_host_workspace_bytes.argtypes = [vp, u64, vp]
     lib.opx_propagate_host.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, vp, vp, vp, C.c_size_t, u64, vp]
     lib.opx_propagate_detected_workspace_bytes.argtypes = [u64, u64, vp]
-    lib.opx_propagate_detected.argtypes = [vp, u64, vp, u64, vp, vp, vp, u64, u32, vp, u64, vp, vp, C.c_size_t, vp, vp, vp]
+    lib.opx_propagate_detected.argtypes = [vp, u64, vp, u64, vp, vp, vp, u64, u32, vp, vp, u64, vp, vp, C.c_size_t, vp, vp, vp]
+    lib.opx_tracks_host_detected_workspace_bytes.argtypes = [vp, u64, u64, u64, vp]
+    lib.opx_tracks_host_detected.argtypes = [vp, vp, u64, C.c_float, C.c_float, C.c_float, u64, u64, u64, vp, u32, vp, u64, vp, vp, vp,
+                                             vp, C.c_size_t, u64, vp]
     lib.opx_propagate_host_detected_workspace_bytes.argtypes = [vp, u64, u64, vp]
     lib.opx_propagate_host_detected.argtypes = [vp, u64, u64, vp, vp, vp, u64, u32, vp, u64, vp, vp, vp, vp, C.c_size_t, u64, vp]
     lib.opx_profile_begin.argtypes = [vp, u32]
@@ -317,7 +321,7 @@ class Scene:
                     n_detected=torch.zeros(1, dtype=torch.int64, device=device))
 
     def propagate_detected(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, capacity=None, out=None, hitmap=None,
-                           counters=None, stream=None, flags=0, n_dev=None):
+                           counters=None, stream=None, flags=0, n_dev=None, index=None):
         """opx_propagate_detected: the DETECTED photons appended to `out` (alloc_detected) in photon-id order; out["n_detected"]
         is the running length on the device.  No per-photon records are written."""
         import torch
@@ -339,7 +343,7 @@ class Scene:
         st = stream if stream is not None else torch.cuda.current_stream(dev)
         _check(lib.opx_propagate_detected(self._h, n, None if n_dev is None else n_dev.data_ptr(), int(photon_id_base),
                                           origins.data_ptr(), dirs.data_ptr(), wavelengths.data_ptr(), int(seed), int(flags),
-                                          C.byref(d), cap, out["n_detected"].data_ptr(), _aligned(self._det_ws), need.value,
+                                          None if index is None else index.data_ptr(), C.byref(d), cap, out["n_detected"].data_ptr(), _aligned(self._det_ws), need.value,
                                           hitmap.data_ptr(), counters.data_ptr(), C.c_void_p(st.cuda_stream)))
         res = dict(out)
         res["hitmap"], res["counters"] = hitmap[:self.n_pixels], counters
@@ -367,6 +371,37 @@ class Scene:
                                                int(flags), C.byref(d), cap, C.byref(nd), out["hitmap"].data_ptr(),
                                                out["counters"].data_ptr(), _aligned(self._host_ws), need.value, chunk,
                                                C.c_void_p(st.cuda_stream)))
+        out["n_detected"] = int(nd.value)
+        return out
+
+    def tracks_host_detected(self, steps, n, factors=(), photon_id_base=0, seed=0, n_index=1.0014, lambda1=200.0, lambda2=600.0,
+                             capacity=None, chunk=1 << 24, out=None, stream=None, device="cuda"):
+        """opx_tracks_host_detected: `steps` = dict of HOST numpy arrays (x, w (S,3), length, beta (S,) float32, first (S+1,) uint64)
+        in, list of detected photons (host) + hit-map + counters out.  factors: () = efficiencies in flight, else the paper's
+        pre-propagation filter on those materials."""
+        import torch
+        lib = load_library()
+        x, w = np.ascontiguousarray(steps["x"], np.float32), np.ascontiguousarray(steps["w"], np.float32)
+        ln, be = np.ascontiguousarray(steps["length"], np.float32), np.ascontiguousarray(steps["beta"], np.float32)
+        first = np.ascontiguousarray(steps["first"], np.uint64)
+        S = len(ln)
+        ts = TrackSteps(x.ctypes.data, w.ctypes.data, ln.ctypes.data, be.ctypes.data, first.ctypes.data, S)
+        chunk = max(1, min(int(chunk), max(int(n), 1)))
+        if out is None:
+            out = alloc_host_detected(max(1, int(n) if capacity is None else int(capacity)), self.n_pixels)
+        cap = int(out["id"].shape[0])
+        need = C.c_size_t()
+        _check(lib.opx_tracks_host_detected_workspace_bytes(self._h, S, chunk, cap, C.byref(need)))
+        if self._host_ws is None or self._host_ws.numel() < need.value + 256:
+            self._host_ws = torch.empty(need.value + 256, dtype=torch.uint8, device=device)
+        fac = (C.c_uint32 * max(1, len(factors)))(*factors)
+        d = Detected(*(out[k].data_ptr() for k in ("id", "pixel", "pos", "dir")))
+        nd = C.c_uint64(0)
+        st = stream if stream is not None else torch.cuda.current_stream(device)
+        _check(lib.opx_tracks_host_detected(self._h, C.byref(ts), int(first[-1]), n_index, lambda1, lambda2, int(n), int(photon_id_base),
+                                            int(seed), fac, len(factors), C.byref(d), cap, C.byref(nd), out["hitmap"].data_ptr(),
+                                            out["counters"].data_ptr(), _aligned(self._host_ws), need.value, chunk,
+                                            C.c_void_p(st.cuda_stream)))
         out["n_detected"] = int(nd.value)
         return out
 

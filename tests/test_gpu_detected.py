@@ -108,12 +108,43 @@ def test_filtered_chain_and_device_side_count(toy):
     a, m = 40_000, 50_000
     pre = gs.emit_cherenkov_filtered(pkg.upload_track_steps(steps), m, fac, photon_id_base=a, seed=7)
     out = gs.propagate_detected(pre["origins"], pre["dirs"], pre["wavelengths"], flags=pkg.FLAG_NO_EFFICIENCY, n_dev=pre["n_kept"])
+    # the same with the filter's index array: the list then names the ORIGINAL photons
+    out2 = gs.propagate_detected(pre["origins"], pre["dirs"], pre["wavelengths"], flags=pkg.FLAG_NO_EFFICIENCY, n_dev=pre["n_kept"],
+                                 index=pre["index"], photon_id_base=a)
     torch.cuda.synchronize()
     ro, rd, rl = oracle.emit_cherenkov(steps, m, id_base=a, seed=7)
     f = oracle.prefilter(w.scene, rl, fac, seed=7, id_base=a)
     ref = oracle.trace_mesh(w.scene, ro[f.index], rd[f.index], rl[f.index], flags=oracle.NO_EFFICIENCY)
     det = oracle.detected_list(ref)
     _check_list(out, int(out["n_detected"].item()), det)
+    _check_list(out2, int(out2["n_detected"].item()), oracle.detected_list(ref, ids=np.uint64(a) + f.index.astype(np.uint64)))
+
+
+@pytest.mark.parametrize("filtered", [False, True])
+def test_from_track_steps_in_host_memory_to_the_detected_list(toy, filtered):
+    """opx_tracks_host_detected (the loop memory-resident): step table in host memory in, detected list out,
+    in chunks that split tiles and steps; == the oracle's chain emit (-> prefilter) -> trace -> detected_list, original ids."""
+    w, gs = toy
+    steps = w.track_source.steps()
+    fac = [w.scene.info["m_det"], w.scene.info["m_mir"]] if filtered else []
+    a, m = 123_456, 70_001
+    got = gs.tracks_host_detected(steps, m, factors=fac, photon_id_base=a, seed=13, chunk=20_000)
+    ro, rd, rl = oracle.emit_cherenkov(steps, m, id_base=a, seed=13)
+    if filtered:
+        f = oracle.prefilter(w.scene, rl, fac, seed=13, id_base=a)
+        ref = oracle.trace_mesh(w.scene, ro[f.index], rd[f.index], rl[f.index], flags=oracle.NO_EFFICIENCY)
+        det = oracle.detected_list(ref, ids=np.uint64(a) + f.index.astype(np.uint64))
+    else:
+        ref = oracle.trace_mesh(w.scene, ro, rd, rl, seed=13, id_base=a)
+        det = oracle.detected_list(ref, id_base=a)
+    k = got["n_detected"]
+    assert k == len(det.id) > 50
+    assert np.array_equal(got["id"][:k].numpy().view(np.uint64), det.id)
+    assert np.array_equal(got["pixel"][:k].numpy(), det.pixel)
+    assert np.array_equal(got["pos"][:k].numpy().astype(np.float64), det.pos)
+    assert np.array_equal(got["dir"][:k].numpy().astype(np.float64), det.dir)
+    assert np.array_equal(got["hitmap"][:gs.n_pixels].numpy().astype(np.uint32), ref.hitmap)
+    assert np.array_equal(got["counters"].numpy().astype(np.uint64), ref.counters)
 
 
 def test_host_path_detected(toy):
@@ -148,7 +179,7 @@ def test_detected_errors(toy):
     dd = opx.Detected(*(lst[k].data_ptr() for k in ("id", "pixel", "pos", "dir")))
     hm, ct = gs.alloc_accumulators()
     ws = torch.empty(1 << 16, dtype=torch.uint8, device="cuda")
-    args = lambda cap, nd, wsb: (gs._h, 64, None, 0, o.data_ptr(), d.data_ptr(), lam.data_ptr(), 0, 0, C.byref(dd), cap, nd,
+    args = lambda cap, nd, wsb: (gs._h, 64, None, 0, o.data_ptr(), d.data_ptr(), lam.data_ptr(), 0, 0, None, C.byref(dd), cap, nd,
                                  opx._aligned(ws), wsb, hm.data_ptr(), ct.data_ptr(), None)
     assert lib.opx_propagate_detected(*args(64, None, 1 << 15)) == opx.OPX_ERR_INVALID_ARG          # no length word
     assert lib.opx_propagate_detected(*args(0, lst["n_detected"].data_ptr(), 1 << 15)) == opx.OPX_ERR_INVALID_ARG   # capacity 0
