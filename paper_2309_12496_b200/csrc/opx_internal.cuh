@@ -56,6 +56,7 @@ struct SceneDev {
 };
 
 struct Layout : opx_scene_layout {};
+constexpr uint32_t kFlagPacketWalk = 1u << 16;   // internal launch flag (debug): incoherent packets walk the binary tree as a warp, not per lane
 
 // A list of detected photons (opx_detected) as the kernels see it.  Inside a detected-only launch of the propagation kernel
 // it describes the STAGING list of that launch (opx_packet.cuh, step 4b): tiles append their chunks at offsets taken from

@@ -25,6 +25,8 @@ constexpr int kPktStack = 96;                        // depth bound of the Karra
 constexpr int kStackSmem = kPktStack - 32;
 constexpr int kRadixBits = 6, kRadix = 1 << kRadixBits;      // 2 passes over the 12-bit key
 
+// (A fifth shape, 1024 threads x 1 photon with a run-time tile stride, spreads a call of at most 148 x 1024 photons over all
+// SMs with every packet in flight at once: opx_propagate.cu.)
 // The kernel is compiled for two tile sizes on 512 threads: kItems = 4 photons per thread, 2048-photon tiles (the
 // product shape: the more photons of a ring a tile holds, the narrower its packets; each warp walks 4 packets), and
 // kItems = 1, 512-photon tiles where each warp walks ONE packet, for calls too small to fill the machine with large
@@ -288,22 +290,65 @@ __device__ __forceinline__ Hit closest_hit_packet(const SceneDev& sc, const RayR
     return h;
 }
 
+// Closest hit of ONE ray with a private stack (the walk of opx_lane.cuh on the packet kernels' rotated triangle records): what
+// the lanes of a packet do when the packet is too incoherent for a beam.  Lanes then walk different subtrees and most of the
+// warp idles, but each ray's walk is ~40 dependent node visits instead of the ~1000 of a warp that visits the union of 32
+// unrelated walks one node after the other -- and an incoherent packet is a matter of latency (it holds up its tile), not
+// of throughput (1 packet-segment in 250 on the C4 scene).
+__device__ __forceinline__ Hit closest_hit_own(const SceneDev& sc, const RayR& rr, const Slab& sl, float e, float tmin, int last_j) {
+    Hit h{kInf, -1, 0x7fffffff};
+    int stack_ref[kPktStack];
+    float stack_t[kPktStack];
+    int sp = 0, ref = 0;
+    for (;;) {
+        if (ref >= 0) {
+            const NodeDev* nd = sc.nodes + ref;
+            const float4 q0 = __ldg(&nd->q0), q1 = __ldg(&nd->q1), q2 = __ldg(&nd->q2);
+            const int4 q3 = __ldg(&nd->q3);
+            float n0, f0, n1, f1;
+            slab2_slack(sl, e, q0, q1, q2, h.t, n0, f0, n1, f1);
+            const bool hit0 = n0 <= f0, hit1 = n1 <= f1;
+            if (hit0 && hit1) {
+                int near = q3.x, far = q3.y;
+                float tf = n1;
+                if (n1 < n0) { near = q3.y; far = q3.x; tf = n0; }
+                stack_ref[sp] = far; stack_t[sp] = tf; ++sp;
+                ref = near;
+                continue;
+            }
+            if (hit0) { ref = q3.x; continue; }
+            if (hit1) { ref = q3.y; continue; }
+        } else {
+            consider_rot(sc, rr, ~ref, tmin, last_j, h);
+        }
+        bool found = false;
+        while (sp > 0) {
+            --sp;
+            if (stack_t[sp] <= h.t) { ref = stack_ref[sp]; found = true; break; }
+        }
+        if (!found) break;
+    }
+    return h;
+}
+
 template <int kPktThreads, int kItems, int kPktCtas, bool kStats>
 __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(const SceneDev sc, uint64_t n, uint64_t id_base,
                                                                      const float* __restrict__ origins,
                                                                      const float* __restrict__ dirs,
                                                                      const float* __restrict__ wl, uint64_t seed, opx_hits out,
                                                                      uint32_t* hitmap, unsigned long long* counters,
-                                                                     unsigned long long* stats, const DetOut det) {
+                                                                     unsigned long long* stats, const DetOut det, uint32_t tile_stride) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     using PacketSmem = PacketSmemT<kPktThreads, kItems>;
     constexpr int kPktWarps = PacketSmem::kPktWarps, kTile = PacketSmem::kTile;
     PacketSmem& sm = *reinterpret_cast<PacketSmem*>(smem_raw);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const uint64_t tile_base = (uint64_t)blockIdx.x * kTile;
+    // photons per tile: kTile, or fewer (a multiple of 32) when a small call is spread over all SMs (launch_propagate)
+    const uint32_t stride = tile_stride ? tile_stride : (uint32_t)kTile;
+    const uint64_t tile_base = (uint64_t)blockIdx.x * stride;
     if (sc.d_n) n = min(n, (uint64_t)__ldg(sc.d_n));       // photon count left on the device by opx_prefilter
     if (tile_base >= n) return;
-    const int m = (int)min((uint64_t)kTile, n - tile_base);
+    const int m = (int)min((uint64_t)stride, n - tile_base);
     if (threadIdx.x == 0) sm.next_group = 0;
 
     // 1. stage the tile (read once).  A full tile whose three input blocks are 16-byte aligned is fetched by three TMA bulk
@@ -458,10 +503,15 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
                 if (kStats) ++bstats.fallback_segments;
                 const float ox = so[0], oy = so[1], oz = so[2], dx = sd[0], dy = sd[1], dz = sd[2];
                 const Slab sl = slab_setup(ox, oy, oz, dx, dy, dz);
-                // an origin beyond origin_limit widens every box by its own rounding slack (8.2)
+                // every box is widened by the ray's own rounding slack, which matters for an origin beyond origin_limit only (8.2)
                 const float far_o = fmaxf(fmaxf(fabsf(ox), fabsf(oy)), fabsf(oz));
-                const bool far = __any_sync(0xffffffffu, alive && !(far_o < sc.origin_limit));
-                h = closest_hit_packet(sc, rw, sl, far_o * 9.5367431640625e-7f, tmin, last_j, alive, lane, sm.stack[w], far ? 9 : 8);
+                if (sc.flags & kFlagPacketWalk) {            // debug (opx_propagate_binary): the warp walks the binary tree as one packet
+                    const bool far = __any_sync(0xffffffffu, alive && !(far_o < sc.origin_limit));
+                    h = closest_hit_packet(sc, rw, sl, far_o * 9.5367431640625e-7f, tmin, last_j, alive, lane, sm.stack[w], far ? 9 : 8);
+                } else {
+                    h = Hit{kInf, -1, 0x7fffffff};
+                    if (alive) h = closest_hit_own(sc, rw, sl, far_o * 9.5367431640625e-7f, tmin, last_j);
+                }
             }
             if (alive) {
                 Photon p;

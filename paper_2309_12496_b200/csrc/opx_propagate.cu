@@ -14,6 +14,8 @@ using Big = PacketSmemT<512, 4>;      // 2048-photon tiles, 4 packets per warp: 
 using Small = PacketSmemT<512, 1>;    // 512-photon tiles, 1 packet per warp: calls too small to fill the machine
 using Mid = PacketSmemT<256, 4>;      // 1024-photon tiles, 4 CTAs/SM: filtered streams on large scenes
 using Lean = PacketSmemT<448, 4>;     // 1792-photon tiles, 72 registers: in-flight calls on small scenes
+using Wave = PacketSmemT<1024, 1>;    // one CTA per SM, one packet per warp, run-time tile size: a small call in a single wave
+constexpr uint64_t kSMs = 148;
 
 // The dynamic shared memory limit of a kernel is an attribute per device (context): set once per device, at the first
 // opx_bvh_build or launch on it, so that a later opx_propagate performs stream operations only (CUDA-graph capturable).
@@ -29,6 +31,7 @@ opx_status configure_device() {
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 1, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Small));
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<448, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Lean));
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<256, 4, 4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Mid));
+    if (!e) e = cudaFuncSetAttribute(k_propagate_packet<1024, 1, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Wave));
     if (opx_status st = check_cuda(e, "cudaFuncSetAttribute")) return st;
     done.fetch_or(bit, std::memory_order_release);      // two threads racing here both set the same attributes: harmless
     return OPX_OK;
@@ -41,7 +44,7 @@ static opx_status launch_propagate_impl(const SceneHost& s, WalkMode mode, uint6
     SceneDev dev = s.dev;          // per-launch copy: flags and the optional device-side count ride in the kernel parameter
     dev.flags = flags;
     dev.d_n = (const unsigned long long*)d_n;
-    if (mode == kWalkBinary) dev.n_wnodes = 0;      // debug: packets walk the binary tree only
+    if (mode == kWalkBinary) { dev.n_wnodes = 0; dev.flags |= kFlagPacketWalk; }      // debug: packets walk the binary tree only, as warps
     const bool brute = mode == kWalkBrute;
     cudaEvent_t* ev = nullptr;
     if (s.prof_used < s.prof_max) { ev = &s.prof_events[3 * (size_t)s.prof_used]; ++s.prof_used; }
@@ -66,21 +69,33 @@ static opx_status launch_propagate_impl(const SceneHost& s, WalkMode mode, uint6
         if (opx_status st = configure_device()) return st;
         // measured crossover (kernel time vs n, both tile sizes): on a small scene the 512-photon tiles win while they
         // number at most one per SM (n < 148 x 512), on a large scene (longer, latency-bound packets) up to about 2e5 photons
-        const uint64_t small_below = s.dev.n_tri < (1u << 18) ? 148ull * Small::kTile : 100ull * Big::kTile;
-        const bool small = !packet_stats && n < small_below;
-        const bool mid = !packet_stats && !small && s.dev.n_tri >= (1u << 18) && (flags & OPX_FLAG_NO_EFFICIENCY);
-        const bool lean = !packet_stats && !small && s.dev.n_tri < (1u << 18) && !(flags & OPX_FLAG_NO_EFFICIENCY);
-        const uint64_t tile = small ? Small::kTile : (mid ? Mid::kTile : (lean ? Lean::kTile : Big::kTile));
+        // A small call (the paper's own runs are 600 ... 6e5 photons) is latency-bound: its time is the dependent
+        // chain of ONE packet times the packets a warp walks one after the other.  Up to 148 x 512 photons the 512-photon tiles
+        // (one packet per warp) already put every packet in flight at once; from there to 148 x 1024 photons the call runs as a
+        // single wave -- one CTA of up to 32 warps per SM, one packet per warp, the photons dealt out evenly over the SMs (tile
+        // size = ceil(n / 148) rounded up to whole packets): measured 64 us against 82 us at 151 000 photons on the toy scene,
+        // 74 against 81 at 1e5; below 148 x 512 photons the 1024-thread CTAs lose (80 us against 68 at 6000 photons).
+        const bool wave = !packet_stats && n > kSMs * Small::kTile && n <= kSMs * Wave::kTile;
+        uint32_t stride = 0;
+        if (wave) stride = (uint32_t)(((n + kSMs - 1) / kSMs + 31) / 32 * 32);
+        // measured crossover (kernel time vs n, both tile sizes): beyond one wave the 512-photon tiles still win on a large scene
+        // (longer, latency-bound packets) up to about 2e5 photons; on a small scene the large tiles take over
+        const uint64_t small_below = s.dev.n_tri < (1u << 18) ? kSMs * Small::kTile + 1 : 100ull * Big::kTile;
+        const bool small = !packet_stats && !wave && n < small_below;
+        const bool mid = !packet_stats && !wave && !small && s.dev.n_tri >= (1u << 18) && (flags & OPX_FLAG_NO_EFFICIENCY);
+        const bool lean = !packet_stats && !wave && !small && s.dev.n_tri < (1u << 18) && !(flags & OPX_FLAG_NO_EFFICIENCY);
+        const uint64_t tile = wave ? stride : small ? Small::kTile : (mid ? Mid::kTile : (lean ? Lean::kTile : Big::kTile));
         const uint64_t tiles = (n + tile - 1) / tile;
         if (tiles > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
         if (det_tiles) *det_tiles = tiles;
-        if (packet_stats) k_propagate_packet<512, 4, 2, true><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr, nullptr, (unsigned long long*)packet_stats, det);
-        else if (lean) k_propagate_packet<448, 4, 2, false><<<(unsigned)tiles, 448, sizeof(Lean), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det);
-        else if (mid) k_propagate_packet<256, 4, 4, false><<<(unsigned)tiles, 256, sizeof(Mid), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det);
-        else if (small) k_propagate_packet<512, 1, 2, false><<<(unsigned)tiles, 512, sizeof(Small), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det);
-        else k_propagate_packet<512, 4, 2, false><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det);
+        if (packet_stats) k_propagate_packet<512, 4, 2, true><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr, nullptr, (unsigned long long*)packet_stats, det, 0u);
+        else if (wave) k_propagate_packet<1024, 1, 1, false><<<(unsigned)tiles, 1024, sizeof(Wave), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det, stride);
+        else if (lean) k_propagate_packet<448, 4, 2, false><<<(unsigned)tiles, 448, sizeof(Lean), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det, 0u);
+        else if (mid) k_propagate_packet<256, 4, 4, false><<<(unsigned)tiles, 256, sizeof(Mid), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det, 0u);
+        else if (small) k_propagate_packet<512, 1, 2, false><<<(unsigned)tiles, 512, sizeof(Small), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det, 0u);
+        else k_propagate_packet<512, 4, 2, false><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det, 0u);
         // the names ncu prints for these instantiations
-        set_last_kernel(packet_stats ? "k_propagate_packet<512, 4, 2, 1>" : lean ? "k_propagate_packet<448, 4, 2, 0>" : mid ? "k_propagate_packet<256, 4, 4, 0>"
+        set_last_kernel(packet_stats ? "k_propagate_packet<512, 4, 2, 1>" : wave ? "k_propagate_packet<1024, 1, 1, 0>" : lean ? "k_propagate_packet<448, 4, 2, 0>" : mid ? "k_propagate_packet<256, 4, 4, 0>"
                         : small ? "k_propagate_packet<512, 1, 2, 0>" : "k_propagate_packet<512, 4, 2, 0>");
         binned = !packet_stats;
     }
@@ -106,7 +121,8 @@ opx_status launch_propagate(const SceneHost& s, WalkMode mode, uint64_t n, const
 // per tile of the smallest tile size, and a staging list of `capacity` entries.
 struct DetWorkspace { unsigned long long* count; ulonglong2* table; unsigned long long* src; DetOut stage; size_t bytes; };
 static DetWorkspace det_workspace(void* ws, uint64_t n, uint64_t capacity) {
-    const uint64_t tiles = (n + Small::kTile - 1) / Small::kTile + 1;
+    uint64_t tiles = (n + Small::kTile - 1) / Small::kTile + 1;      // the smallest fixed tile size ...
+    if (tiles < kSMs + 1) tiles = kSMs + 1;                         // ... and the single-wave shape's at most 148 tiles
     char* p = (char*)ws;
     auto take = [&](size_t bytes) { char* r = p; p += align_up(bytes, 256); return r; };
     DetWorkspace w{};
