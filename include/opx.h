@@ -143,6 +143,7 @@ typedef struct {
     uint64_t parents;     /* (2 n_triangles - 1) x 4 B: parent of internal node i / leaf T-1+i  */
     uint64_t wide_nodes;  /* (wide_node_capacity) x 896 B: 32-wide nodes collapsed from `nodes`  */
     uint64_t wide_node_capacity;
+    uint64_t wide_count;  /* uint32: number of 32-wide nodes the build produced; 0 = the wide tree did not fit or is too deep */
     uint64_t vertex_normals; /* (n_triangles) x 36 B: na, nb, nc in GLOBAL triangle-id order; 16 B if no mesh has any */
     uint64_t total_bytes;
 } opx_scene_layout;
@@ -164,9 +165,11 @@ opx_status opx_scene_workspace_bytes(const opx_scene* scene, size_t* scene_bytes
 
 /* A1-A4.  GPU LBVH build into the caller's workspaces (both 256-byte aligned device pointers):
  * scene AABB + 63-bit Morton keys of the triangle AABB centres, LSD radix sort, Karras hierarchy,
- * padded bottom-up refit, packing into 64-byte nodes and leaf-ordered triangles.  Uploads the
- * flattened scene first (the host->device copies of pageable memory make this call synchronous with
- * respect to the host up to the last upload).  May be called again to rebuild.
+ * padded bottom-up refit, packing into 64-byte nodes and leaf-ordered triangles, collapse into the 32-wide tree.
+ * Uploads the flattened scene first, then enqueues a fixed sequence of kernels on cuda_stream and returns: nothing
+ * is read back and the stream is not synchronised (the uploads leave from pageable host memory, so the call returns
+ * once the last of them has been staged; the scene's host arrays are not referenced afterwards).  Work that uses the
+ * scene must be ordered after the build (same stream, or an event).  May be called again to rebuild.
  * Errors: OPX_ERR_WORKSPACE_TOO_SMALL, OPX_ERR_INVALID_ARG (NULL / misaligned),
  * OPX_ERR_UNSUPPORTED_DEVICE, OPX_ERR_CUDA. */
 opx_status opx_bvh_build(opx_scene* scene, void* d_scene_ws, size_t scene_bytes,

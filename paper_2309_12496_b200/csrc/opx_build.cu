@@ -292,15 +292,14 @@ __device__ inline void take_child(const NodeDev* __restrict__ bn, int node, int 
     e.cnt = e.ref >= 0 ? bn[e.ref].q3.z : 1;
 }
 
-__global__ void __launch_bounds__(256) k_collapse(const NodeDev* __restrict__ bn, const int2* __restrict__ q_in,
-                                                  const uint32_t* __restrict__ n_in_ptr, int2* q_out, uint32_t* n_out,
-                                                  WNodeDev* wn, uint32_t* n_wn, uint32_t cap_wn, uint32_t* overflow) {
+__device__ __forceinline__ void collapse_level(const NodeDev* __restrict__ bn, const int2* q_in, uint32_t n_in, int2* q_out, uint32_t* n_out,
+                                               WNodeDev* wn, uint32_t* n_wn, uint32_t cap_wn, uint32_t* overflow) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    const uint32_t n_in = *n_in_ptr;
     const uint32_t warps = gridDim.x * (blockDim.x >> 5);
     for (uint32_t task = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); task < n_in; task += warps) {
-        const int b = q_in[task].x, w = q_in[task].y;
+        const int2 tk = __ldcg(&q_in[task]);      // written by other SMs one level earlier: not through L1
+        const int b = tk.x, w = tk.y;
         WEntry e; e.ref = 0x7fffffff; e.cnt = 0;
         bool valid = false;
         if (lane < 2) { take_child(bn, b, lane, e); valid = true; }
@@ -362,13 +361,49 @@ __global__ void __launch_bounds__(256) k_collapse(const NodeDev* __restrict__ bn
     }
 }
 
-__global__ void k_collapse_init(int2* q, uint32_t* counters) {
-    // counters: [0] n_in, [1] n_out, [2] n_wn, [3] overflow
-    q[0] = make_int2(0, 0);
-    counters[0] = 1u; counters[1] = 0u; counters[2] = 1u; counters[3] = 0u;
+// Barrier across the CTAs of a grid that is resident as a whole (k_collapse_all is launched with at most two CTAs per SM).
+// bar[0] counts arrivals, bar[1] is the generation.
+__device__ __forceinline__ void grid_barrier(uint32_t* bar) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const uint32_t gen = atomicAdd(&bar[1], 0u);
+        if (atomicAdd(&bar[0], 1u) == gridDim.x - 1) { atomicExch(&bar[0], 0u); __threadfence(); atomicAdd(&bar[1], 1u); }
+        else while (atomicAdd(&bar[1], 0u) == gen) { }
+        __threadfence();
+    }
+    __syncthreads();
 }
 
-__global__ void k_collapse_next(uint32_t* counters) { counters[0] = counters[1]; counters[1] = 0u; }
+// The whole collapse in ONE launch: the levels of the 32-wide tree are produced one after the other with a grid barrier in
+// between, the size of each level being known on the device only.  counters: [0] tasks of this level, [1] tasks of the next,
+// [2] wide nodes so far, [3] capacity overflow, [4..5] the barrier.  On exit *wide_count = number of wide nodes, or 0 if the
+// tree outgrew its capacity (packets then walk the binary tree).  The host reads nothing back: opx_bvh_build returns after
+// enqueueing and can be captured into a CUDA graph.
+__global__ void __launch_bounds__(256) k_collapse_all(const NodeDev* __restrict__ bn, int2* q0, int2* q1, uint32_t* counters, WNodeDev* wn,
+                                                      uint32_t cap_wn, uint32_t* wide_count) {
+    int2* q_in = q0;
+    int2* q_out = q1;
+    for (int level = 0; level < 128; ++level) {
+        const uint32_t n_in = level == 0 ? 1u : atomicAdd(&counters[0], 0u);
+        if (n_in == 0u) break;                                   // the same value in every CTA (set before the last barrier)
+        collapse_level(bn, q_in, n_in, q_out, counters + 1, wn, counters + 2, cap_wn, counters + 3);
+        grid_barrier(counters + 4);
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            const uint32_t next = atomicAdd(&counters[1], 0u);
+            atomicExch(&counters[0], atomicAdd(&counters[3], 0u) ? 0u : next);      // overflow: stop
+            atomicExch(&counters[1], 0u);
+        }
+        grid_barrier(counters + 4);
+        int2* t = q_in; q_in = q_out; q_out = t;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) *wide_count = atomicAdd(&counters[3], 0u) ? 0u : atomicAdd(&counters[2], 0u);
+}
+
+__global__ void k_collapse_init(int2* q, uint32_t* counters) {
+    q[0] = make_int2(0, 0);
+    counters[0] = 1u; counters[1] = 0u; counters[2] = 1u; counters[3] = 0u; counters[4] = 0u; counters[5] = 0u;
+}
 
 }  // namespace
 
@@ -391,6 +426,7 @@ void compute_layout(const SceneHost& s, opx_scene_layout* lay, size_t* tmp_bytes
     lay->parents = take((2 * T + 1) * 4);
     lay->wide_node_capacity = wide_node_capacity(T);
     lay->wide_nodes = take(lay->wide_node_capacity * sizeof(WNodeDev));
+    lay->wide_count = take(4);
     lay->vertex_normals = take(s.tri_vnormals.size() * 4);
     lay->total_bytes = off;
     if (tmp_bytes) {
@@ -472,7 +508,6 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
     const float pad = s.leaf_pad, tri_size = s.tri_size, scene_ext = s.scene_ext;      // scene constants (compute_scene_stats)
 
     const int Ti = (int)T;
-    uint32_t n_wide = 0;
     if (T >= 2) {
         const uint32_t nsb = (uint32_t)sort_blocks(T);
         const uint32_t g256 = (uint32_t)((T + 255) / 256);
@@ -495,41 +530,31 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
         if ((e = cudaMemsetAsync(tmp.flags, 0, T * 4, stream))) return check_cuda(e, "memset flags");
         k_refit<<<g256, 256, 0, stream>>>(tris, Ti, pad, nodes, parents, tmp.flags);
         count_launch(3);
-        // collapse into the 32-wide tree, level by level (the host reads the size of the next level)
+        // collapse into the 32-wide tree: one launch for all levels (k_collapse_all), nothing read back
         WNodeDev* wnodes = (WNodeDev*)(ws + lay.wide_nodes);
         const uint32_t cap = (uint32_t)lay.wide_node_capacity;
         k_collapse_init<<<1, 1, 0, stream>>>(tmp.queue[0], tmp.wcount);
-        count_launch(1);
-        uint32_t h_cnt[4] = {1, 0, 1, 0};
-        int qi = 0;
-        for (int level = 0; level < 128 && h_cnt[0] > 0; ++level) {
-            const uint32_t blocks = (h_cnt[0] + 7) / 8;
-            k_collapse<<<blocks < 2368u ? blocks : 2368u, 256, 0, stream>>>(nodes, tmp.queue[qi], tmp.wcount, tmp.queue[qi ^ 1], tmp.wcount + 1,
-                                                                          wnodes, tmp.wcount + 2, cap, tmp.wcount + 3);
-            k_collapse_next<<<1, 1, 0, stream>>>(tmp.wcount);
-            count_launch(2);
-            if ((e = cudaMemcpyAsync(h_cnt, tmp.wcount, 16, cudaMemcpyDeviceToHost, stream)) || (e = cudaStreamSynchronize(stream)))
-                return check_cuda(e, "wide-tree collapse");
-            if (h_cnt[3]) break;
-            qi ^= 1;
+        const uint32_t grid = (uint32_t)std::min<size_t>((lay.wide_node_capacity + 7) / 8, 296);      // resident as a whole: <= 2 CTAs per SM
+        k_collapse_all<<<grid, 256, 0, stream>>>(nodes, tmp.queue[0], tmp.queue[1], tmp.wcount, wnodes, cap, (uint32_t*)(ws + lay.wide_count));
+        count_launch(2);
+    } else {
+        if ((e = cudaMemsetAsync(ws + lay.wide_count, 0, 4, stream))) return check_cuda(e, "memset wide count");
+        if (T == 1) {
+            // a single triangle needs no hierarchy: propagate tests it directly (see launch_propagate)
+            uint64_t zero_key = 0;
+            uint32_t zero_idx = 0;
+            if ((e = up(sorted_keys, &zero_key, 8)) || (e = up(tmp.idx[0], &zero_idx, 4))) return check_cuda(e, "tiny upload");
+            k_pack_tris<<<1, 32, 0, stream>>>(tmp.tri_in, tmp.surf_in, tmp.normals_in, tmp.idx[0], 1u, tris, normals);
+            count_launch(1);
         }
-        // capacity exceeded (or a pathologically deep tree): no wide tree, packets walk the binary tree
-        n_wide = (h_cnt[3] || h_cnt[0] > 0) ? 0u : h_cnt[2];
-    } else if (T == 1) {
-        // a single triangle needs no hierarchy: propagate tests it directly (see launch_propagate)
-        uint64_t zero_key = 0;
-        uint32_t zero_idx = 0;
-        if ((e = up(sorted_keys, &zero_key, 8)) || (e = up(tmp.idx[0], &zero_idx, 4))) return check_cuda(e, "tiny upload");
-        k_pack_tris<<<1, 32, 0, stream>>>(tmp.tri_in, tmp.surf_in, tmp.normals_in, tmp.idx[0], 1u, tris, normals);
-        count_launch(1);
     }
     if ((e = cudaGetLastError())) return check_cuda(e, "BVH build launch");
-    // the uploads above read pageable host memory owned by the scene: make sure they are done
-    // before the caller can destroy or rebuild it
-    if ((e = cudaStreamSynchronize(stream))) return check_cuda(e, "BVH build");
+    // No synchronisation: the uploads above left from pageable host memory, which cudaMemcpyAsync stages before it returns,
+    // so the scene's host arrays are no longer referenced; everything else is stream-ordered.
 
     SceneDev& d = s.dev;
-    d.wnodes = (const WNodeDev*)(ws + lay.wide_nodes); d.n_wnodes = n_wide;
+    d.wnodes = (const WNodeDev*)(ws + lay.wide_nodes); d.n_wnodes = T >= 2 ? (uint32_t)lay.wide_node_capacity : 0u;
+    d.wide_count = (const uint32_t*)(ws + lay.wide_count);
     d.nodes = nodes; d.tris = tris; d.normals = normals; d.surfaces = surfaces; d.mat_kinds = mat_kinds;
     d.tables = tables; d.frames = frames;
     d.vnormals = s.tri_vnormals.empty() ? nullptr : (const float*)(ws + lay.vertex_normals);

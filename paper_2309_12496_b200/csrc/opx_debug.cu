@@ -130,7 +130,16 @@ opx_status opx_propagate_packet_stats(const opx_scene* scene, uint64_t n, uint64
 opx_status opx_scene_wide_info(const opx_scene* scene, uint64_t* n_wide_nodes, uint64_t* capacity) {
     if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
     if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_scene_wide_info before opx_bvh_build");
-    if (n_wide_nodes) *n_wide_nodes = scene->dev.n_wnodes;
+    if (n_wide_nodes) {
+        // the count lives on the device (the build does not read it back): this debug call waits for the device
+        uint32_t c = 0;
+        *n_wide_nodes = 0;
+        if (scene->dev.wide_count) {
+            if (opx_status st = check_cuda(cudaDeviceSynchronize(), "cudaDeviceSynchronize")) return st;
+            if (opx_status st = check_cuda(cudaMemcpy(&c, scene->dev.wide_count, 4, cudaMemcpyDeviceToHost), "cudaMemcpy")) return st;
+            *n_wide_nodes = c;
+        }
+    }
     if (capacity) *capacity = scene->layout.wide_node_capacity;
     return OPX_OK;
 }

@@ -37,7 +37,9 @@ constexpr int kWOffLo = 0, kWOffHi = 3 * kWide, kWOffRef = 6 * kWide;      // wo
 // Everything the propagation kernels need, passed by value as a kernel parameter.
 struct SceneDev {
     const NodeDev* nodes;      // n_nodes
-    const WNodeDev* wnodes;    // n_wnodes (0: the wide tree is not available, packets walk the binary tree)
+    const WNodeDev* wnodes;    // the 32-wide tree (n_wnodes = its capacity, 0: none was built)
+    const uint32_t* wide_count; // device word the build leaves behind: number of wide nodes, 0 = the collapse did not fit (packets then
+                               // walk the binary tree); read by the kernels, so opx_bvh_build never has to wait for it
     const float4* tris;        // 3 per triangle, leaf order: (a.xyz, id bits) (b.xyz, surface bits) (c.xyz, 0); then the same array with
                                // the components rotated to (y, z, x), then to (z, x, y)   (packet kernels: RayR::toff)
     const float4* normals;     // leaf order: n.xyz, surface id bits

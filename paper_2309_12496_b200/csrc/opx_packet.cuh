@@ -452,6 +452,7 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
         smem_radix_pass(sm, alt, sm.key, 22);
     }
 
+    const bool have_wide = sc.n_wnodes && __ldg(sc.wide_count) != 0u;      // the build's verdict on the 32-wide tree (warp-uniform)
     // 3. each warp takes groups of 32 neighbouring photons and walks them as a packet
     //    (groups are handed out dynamically so that a slow packet does not hold up its warp's share)
     const int groups = (m + 31) >> 5;
@@ -483,7 +484,7 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
                 Beam bm;
                 float s;
                 const unsigned tris_before = bstats.tris, visits_before = bstats.visits;
-                if (sc.n_wnodes && beam_setup(sc, ox, oy, oz, dx, dy, dz, tmin, alive, bm, s)) {     // coherent packet: one beam through the 32-wide tree
+                if (have_wide && beam_setup(sc, ox, oy, oz, dx, dy, dz, tmin, alive, bm, s)) {     // coherent packet: one beam through the 32-wide tree
                     done = bm.mixed ? closest_hit_beam<true, kStats>(sc, rw, bm, s, tmin, last_j, alive, lane, so, sd, sm.stack[w], sm.beam_tn[w], sm.cull[w], h, bstats)
                                     : closest_hit_beam<false, kStats>(sc, rw, bm, s, tmin, last_j, alive, lane, so, sd, sm.stack[w], sm.beam_tn[w], sm.cull[w], h, bstats);
                     if (kStats && done) {

@@ -77,7 +77,7 @@ class TrackSteps(C.Structure):
 
 class SceneLayout(C.Structure):
     _fields_ = [(k, C.c_uint64) for k in ("nodes", "triangles", "normals", "surfaces", "mat_kinds", "tables",
-                                          "frames", "sorted_keys", "parents", "wide_nodes", "wide_node_capacity",
+                                          "frames", "sorted_keys", "parents", "wide_nodes", "wide_node_capacity", "wide_count",
                                           "vertex_normals", "total_bytes")]
 
 

@@ -101,10 +101,38 @@ def test_c2_c3_sampled_parity(toy, name, stride, seed):
         assert len(np.unique(ref["state"])) >= 5        # the workload exercises the terminal states
 
 
+def test_c2_bench_launch_itself_against_the_oracle(toy):
+    """The launch bench.py times on C2 -- all 1e7 point-source photons, contiguous ids, one opx_propagate call (large tiles,
+    packets of ring neighbours) -- compared with the oracle on every 4000th of its records (the oracle traces those ids alone:
+    a photon's result depends on (scene, inputs[i], seed, id) only), plus the size-independent properties on all of them."""
+    sc, gs = toy
+    w = wl.make_config("C2")
+    pin = [torch.empty((w.n, 3), dtype=torch.float32), torch.empty((w.n, 3), dtype=torch.float32), torch.empty(w.n, dtype=torch.float32)]
+    for a in range(0, w.n, 2_000_000):
+        for dst, src in zip(pin, w.photon_range(a, a + 2_000_000)):
+            dst[a:a + 2_000_000] = torch.from_numpy(src)
+    got = gs.propagate(*(x.cuda() for x in pin), seed=0)
+    torch.cuda.synchronize()
+    ids = np.arange(0, w.n, 4000, dtype=np.uint64)
+    idx = torch.from_numpy(ids.astype(np.int64)).cuda()
+    sub = {k: got[k][idx].cpu().numpy() for k in ("state", "pixel", "surface", "bounces", "pos", "dir")}
+    o, d, lam = w.photons(ids)
+    ref = oracle.trace_mesh(sc, o, d, lam, seed=0, ids=ids)
+    for k in ("state", "pixel", "surface", "bounces"):
+        assert np.array_equal(sub[k], ref[k]), k
+    assert np.array_equal(sub["pos"].astype(np.float64), ref["pos"]) and np.array_equal(sub["dir"].astype(np.float64), ref["dir"])
+    cnt = got["counters"].cpu().numpy()
+    assert cnt[:7].sum() == w.n and int(got["hitmap"].sum().item()) == cnt[0]
+    det = got["state"] == 0
+    assert torch.equal(torch.bincount(got["pixel"][det].long(), minlength=gs.n_pixels).int(), got["hitmap"].int())
+    assert bool((got["pixel"][~(det | (got["state"] == 1))] == -1).all())
+
+
 def test_both_cta_shapes_against_the_oracle(toy):
-    """opx_propagate picks 512-photon tiles (one packet per warp) for small calls (on this scene: below 75 776 photons) and large tiles (on this
-    small scene, in flight: 448 threads x 4 photons) above: 620 000 contiguous C3 photons take the large tiles, their
-    first 50 000 alone the small ones; both must reproduce the oracle, hence each other, bit for bit.  (The 512-thread
+    """opx_propagate picks 512-photon tiles (one packet per warp) for small calls (on this scene: up to 75 776 photons), a single
+    wave of 1024-thread CTAs from there to 151 552 photons, and large tiles (on this small scene, in flight: 448 threads x 4
+    photons) above: 620 000 contiguous C3 photons take the large tiles, their first 50 000 alone the small ones, their first
+    120 000 the single wave; all must reproduce the oracle, hence each other, bit for bit.  (The 512-thread
     shape is pinned by test_no_efficiency_trace_at_scale on this scene and by tests/test_gpu_filter.py on the large one.)"""
     sc, gs = toy
     w = wl.make_config("C3", n=2_000_000)
@@ -119,6 +147,37 @@ def test_both_cta_shapes_against_the_oracle(toy):
     small = _host(gs.propagate(do[:m].contiguous(), dd[:m].contiguous(), dl[:m].contiguous(), seed=21, photon_id_base=700_000))
     for k in ("state", "pixel", "surface", "bounces", "pos", "dir"):
         assert np.array_equal(small[k], big[k][:m]), k
+    m = 120_000
+    wave = gs.propagate(do[:m].contiguous(), dd[:m].contiguous(), dl[:m].contiguous(), seed=21, photon_id_base=700_000)
+    assert pkg.last_kernel() == "k_propagate_packet<1024, 1, 1, 0>"
+    wave = _host(wave)
+    for k in ("state", "pixel", "surface", "bounces", "pos", "dir"):
+        assert np.array_equal(wave[k], big[k][:m]), k
+
+
+def test_propagate_is_cuda_graph_capturable(toy):
+    """opx_propagate performs stream operations only (kernel attributes are set at opx_bvh_build): a call captured into a CUDA
+    graph and replayed gives the records of the plain call."""
+    sc, gs = toy
+    w = wl.make_config("C3", n=300_000)
+    do, dd, dl = _dev(*w.photon_range(0, 200_000))
+    plain = _host(gs.propagate(do, dd, dl, seed=3))
+    rec = gs.alloc_records(200_000)
+    hm, ct = gs.alloc_accumulators()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        g.capture_begin()
+        gs.propagate(do, dd, dl, seed=3, records=rec, hitmap=hm, counters=ct, stream=side)
+        g.capture_end()
+    for _ in range(2):
+        hm.zero_(); ct.zero_(); rec["state"].fill_(99)
+        g.replay()
+    torch.cuda.synchronize()
+    for k in ("state", "pixel", "surface", "bounces", "pos", "dir"):
+        assert np.array_equal(rec[k].cpu().numpy(), plain[k]), k
+    assert np.array_equal(hm[:gs.n_pixels].cpu().numpy(), plain["hitmap"]) and np.array_equal(ct.cpu().numpy(), plain["counters"])
 
 
 def test_id_base_and_chunking(toy):
