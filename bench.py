@@ -36,7 +36,7 @@ BYTES_IN, BYTES_OUT = 28, 34                        # per photon: inputs, hit re
 L2_BYTES = 126e6
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the step's kernel, from the `ncu --set full` captures
 # summarised under profiles/ (per config, at the launch size this bench times; None until a capture exists)
-NCU_TRAFFIC_BYTES = {"C2": 566210304, "C4": 6683943000}
+NCU_TRAFFIC_BYTES = {"C2": (566210304, 10_000_000), "C4": (6683943000, 100_000_000)}      # (bytes, photons of the captured launch)
 NCU_TRAFFIC_SOURCE = {"C2": "profiles/r02_k_propagate_packet.md (1e7 photons per launch)", "C4": "profiles/r02_k_propagate_packet.md (1e8 photons per launch)"}
 
 
@@ -210,7 +210,9 @@ def roofline_record(pkg, scene, photons, n, id_base, seed, kernel_ms, step_ms, p
         roof = {"bound": "hbm", "achieved": hbm, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": hbm / peaks["hbm_gbs"],
                 "peak_source": peaks["source"]}
     roof.update({
-        "traffic": NCU_TRAFFIC_BYTES.get(config), "traffic_source": NCU_TRAFFIC_SOURCE.get(config),
+        # the capture's bytes, scaled when this launch has another photon count than the captured one (the default sizes match)
+        "traffic": (NCU_TRAFFIC_BYTES[config][0] * n // NCU_TRAFFIC_BYTES[config][1]) if config in NCU_TRAFFIC_BYTES else None,
+        "traffic_source": NCU_TRAFFIC_SOURCE.get(config),
         "kernel": pkg.last_kernel(), "kernel_ms": kernel_ms, "kernel_share_of_step": kernel_ms / step_ms,
         "fp32_peak_derived_tflops": derived, "frac_of_derived_peak": alu / derived,
         "fp32_peak_derivation": "148 SMs x 128 FP32 lanes x 2 FLOP x sm_max_mhz (only the clock is measured)",

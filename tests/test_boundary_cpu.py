@@ -37,7 +37,7 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_struct_sizes_match_header(lib):
     assert C.sizeof(opx.SceneParams) == 20 and C.sizeof(opx.PixelFrame) == 56
-    assert C.sizeof(opx.Mesh) == 48 and C.sizeof(opx.Hits) == 48 and C.sizeof(opx.SceneLayout) == 104
+    assert C.sizeof(opx.Mesh) == 48 and C.sizeof(opx.Hits) == 48 and C.sizeof(opx.SceneLayout) == 112 and C.sizeof(opx.Detected) == 32
 
 
 def test_scene_create_and_info(lib):
