@@ -6,12 +6,11 @@
 //   2. sort    photons are ordered by a 12-bit pseudo-angle of their direction about the tile's mean
 //              direction (Cherenkov photons of a track lie on a cone = a ring in the octahedral
 //              plane), with a 2-pass 6-bit radix sort in shared memory;
-//   3. trace   every warp takes groups of 32 neighbouring photons and walks the BVH as ONE packet:
-//              node loads are warp-uniform (one broadcast transaction instead of 32), control flow
-//              is uniform, and the traversal stack is shared by the warp and lives in the registers
-//              of its lanes (entry k in lane k, read back with a shuffle; entries >= 32 overflow to
-//              shared memory).  Each lane still intersects its own ray against every triangle the
-//              packet reaches, so results are exactly the per-photon results of DESIGN.md section 2;
+//   3. trace   every warp takes groups of 32 neighbouring photons and walks the 32-wide tree as ONE packet bounded by a
+//              beam (opx_beam.cuh): lane k tests child k of a wide node, control flow is uniform, the stack is the
+//              warp's in shared memory.  A packet too incoherent for a beam is walked per lane through the binary
+//              tree (closest_hit_own).  Each lane intersects its own ray with the contract test against the triangles
+//              its ray's box test leaves, so results are exactly the per-photon results of DESIGN.md section 2;
 //   4. store   records are written back into the photon's own shared-memory slot and the tile leaves by six TMA bulk
 //              stores (or coalesced streaming stores for a ragged / misaligned tile).
 #pragma once
