@@ -341,7 +341,10 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
     using PacketSmem = PacketSmemT<kPktThreads, kItems>;
     constexpr int kPktWarps = PacketSmem::kPktWarps, kTile = PacketSmem::kTile;
     PacketSmem& sm = *reinterpret_cast<PacketSmem*>(smem_raw);
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    // opaque to the compiler from here on: it otherwise re-derives both (and every shared-memory address built on them) from
+    // the thread id inside the node and cull loops -- S2R + shifts + address arithmetic at every node -- to save two registers
+    asm volatile("" : "+r"(lane), "+r"(w));
     // photons per tile: kTile, or fewer (a multiple of 32) when a small call is spread over all SMs (launch_propagate)
     const uint32_t stride = tile_stride ? tile_stride : (uint32_t)kTile;
     const uint64_t tile_base = (uint64_t)blockIdx.x * stride;
@@ -415,12 +418,37 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
             }
             if (threadIdx.x < 12) rs[threadIdx.x] = 0.f;
             __syncthreads();
+            {   // exclusive prefix of the kItems x kPktWarps (<= 128) jump counts, once, by warp 0
+                constexpr int kC = kItems * kPktWarps;
+                static_assert(kC <= 128, "four chunk counts per lane of warp 0");
+                if (w == 0) {
+                    uint32_t c4[4], sum = 0;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { c4[k] = 4 * lane + k < kC ? chunk[4 * lane + k] : 0u; sum += c4[k]; }
+                    uint32_t inc = sum;
+                    for (int o2 = 1; o2 < 32; o2 <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o2); if (lane >= o2) inc += y; }
+                    uint32_t runsum = inc - sum;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { if (4 * lane + k < kC) chunk[4 * lane + k] = runsum; runsum += c4[k]; }
+                }
+                __syncthreads();
+            }
 #pragma unroll
             for (int r = 0; r < kItems; ++r) {
-                uint32_t before = 0;
-                for (int c = 0; c < r * kPktWarps + w; ++c) before += chunk[c];
+                const uint32_t before = chunk[r * kPktWarps + w];
                 run[r] = min(3u, before + __popc(bal[r] & (0xffffffffu >> (31 - lane))));
-                if (r * kPktThreads + (int)threadIdx.x < m) {
+                // sums per run.  A warp's 32 photons are consecutive, so all but the warps that hold a track boundary belong to one
+                // run: those add once per warp (2048 threads adding floats to three words one by one serialise on a
+                // compare-and-swap loop)
+                const bool in = r * kPktThreads + (int)threadIdx.x < m;
+                const uint32_t run0 = __shfl_sync(0xffffffffu, run[r], 0);
+                if (__all_sync(0xffffffffu, run[r] == run0)) {
+                    float a = in ? u[r] : 0.f, b = in ? v[r] : 0.f, c = in ? 1.f : 0.f;
+                    for (int off = 16; off > 0; off >>= 1) {
+                        a += __shfl_xor_sync(0xffffffffu, a, off); b += __shfl_xor_sync(0xffffffffu, b, off); c += __shfl_xor_sync(0xffffffffu, c, off);
+                    }
+                    if (lane == 0) { atomicAdd(&rs[3 * run0], a); atomicAdd(&rs[3 * run0 + 1], b); atomicAdd(&rs[3 * run0 + 2], c); }
+                } else if (in) {
                     atomicAdd(&rs[3 * run[r]], u[r]); atomicAdd(&rs[3 * run[r] + 1], v[r]); atomicAdd(&rs[3 * run[r] + 2], 1.f);
                 }
             }
