@@ -233,7 +233,7 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayR&
                     __syncwarp();
                 } while (rem);
             }
-            thi = warp_max(alive ? h.t - s : -kInf);
+            thi = warp_max_pos(alive ? h.t - s : 0.f);            // h.t > 0 >= s: the bounds are positive, their bit patterns order like the values
             {
                 const float4 a = s_beam[0], b = s_beam[1], c = s_beam2[0], d = s_beam2[1];
                 bm.rn[0] = a.x; bm.rn[1] = a.y; bm.rn[2] = a.z; bm.tlo = a.w;
