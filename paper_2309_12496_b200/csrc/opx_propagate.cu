@@ -12,8 +12,7 @@ namespace opx {
 
 using Big = PacketSmemT<512, 4>;      // 2048-photon tiles, 4 packets per warp: the general shape
 using Small = PacketSmemT<512, 1>;    // 512-photon tiles, 1 packet per warp: calls too small to fill the machine
-using Mid = PacketSmemT<256, 4>;      // 1024-photon tiles, 4 CTAs/SM: filtered streams on large scenes
-using Lean = PacketSmemT<448, 4>;     // 1792-photon tiles, 72 registers: in-flight calls on small scenes
+using Mid = PacketSmemT<256, 4>;      // 1024-photon tiles, 4 CTAs/SM: filtered (NO_EFFICIENCY) streams
 using Wave = PacketSmemT<1024, 1>;    // one CTA per SM, one packet per warp, run-time tile size: a small call in a single wave
 constexpr uint64_t kSMs = 148;
 
@@ -29,7 +28,6 @@ opx_status configure_device() {
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 1, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Small));
-    if (!e) e = cudaFuncSetAttribute(k_propagate_packet<448, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Lean));
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<256, 4, 4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Mid));
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<1024, 1, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Wave));
     if (opx_status st = check_cuda(e, "cudaFuncSetAttribute")) return st;
@@ -58,17 +56,13 @@ static opx_status launch_propagate_impl(const SceneHost& s, WalkMode mode, uint6
         k_propagate_lane<true, false><<<(unsigned)blocks, 128, 0, stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr);
         set_last_kernel("k_propagate_lane<1, 0>");
     } else {
-        // tile size: 2048 photons (4 packets per warp) unless the call is small; then 512 photons (1 packet per warp)
-        // Shapes (defined at the top of this file).  A filtered stream (NO_EFFICIENCY: 1 photon in 7-9 survives, so packets are
-        // wide and walk more nodes) on a large scene runs 22 % faster with 4 CTAs of 256 threads per SM (1024-photon tiles) than
-        // with 2 x 512: its packets differ widely in cost, and a tile's warps wait at its barrier for the slowest packet, so
-        // finer tiles waste fewer warp slots (384 x 3: +14 %, 128 x 8: -15 %); everything else is faster with 2 x 512 (more
-        // photons per ring in a tile: C4 in flight -10 %, toy-scene pipeline -23 % with the finer shapes).  A small scene (its
-        // BVH lives in L1/L2: the walk is issue-bound, not latency-bound) traced in flight runs 3 % faster with 448 threads x
-        // 2 CTAs, which leaves 72 registers per thread (C4 scene: -3.5 %, filtered toy-scene stream: -5 %: those keep 512 x 2).
+        // Shapes (defined at the top of this file), re-measured on the final kernel of round 2: in-flight calls run fastest with
+        // 2 x 512 threads per SM and 2048-photon tiles on every scene (toy scene C2 / C3: 1.158 / 1.210 ms per 1e7 photons
+        // against 1.171 / 1.251 with 448 x 2 and 1.216 / 1.227 with 256 x 4; C4: 6.18 / 6.70 / 7.40 ms per 2e7).  A filtered
+        // stream (NO_EFFICIENCY: 1 photon in 7-9 survives, so packets are wide and differ widely in cost; a tile's warps wait at
+        // its barrier for the slowest packet) runs fastest with 4 CTAs of 256 threads and 1024-photon tiles on every scene (C4
+        // survivors of 4e7 photons: 3.38 ms against 4.12 with 2 x 512; toy scene 0.280 against 0.320).
         if (opx_status st = configure_device()) return st;
-        // measured crossover (kernel time vs n, both tile sizes): on a small scene the 512-photon tiles win while they
-        // number at most one per SM (n < 148 x 512), on a large scene (longer, latency-bound packets) up to about 2e5 photons
         // A small call (the paper's own runs are 600 ... 6e5 photons) is latency-bound: its time is the dependent
         // chain of ONE packet times the packets a warp walks one after the other.  Up to 148 x 512 photons the 512-photon tiles
         // (one packet per warp) already put every packet in flight at once; from there to 148 x 1024 photons the call runs as a
@@ -82,20 +76,18 @@ static opx_status launch_propagate_impl(const SceneHost& s, WalkMode mode, uint6
         // (longer, latency-bound packets) up to about 2e5 photons; on a small scene the large tiles take over
         const uint64_t small_below = s.dev.n_tri < (1u << 18) ? kSMs * Small::kTile + 1 : 100ull * Big::kTile;
         const bool small = !packet_stats && !wave && n < small_below;
-        const bool mid = !packet_stats && !wave && !small && s.dev.n_tri >= (1u << 18) && (flags & OPX_FLAG_NO_EFFICIENCY);
-        const bool lean = !packet_stats && !wave && !small && s.dev.n_tri < (1u << 18) && !(flags & OPX_FLAG_NO_EFFICIENCY);
-        const uint64_t tile = wave ? stride : small ? Small::kTile : (mid ? Mid::kTile : (lean ? Lean::kTile : Big::kTile));
+        const bool mid = !packet_stats && !wave && !small && (flags & OPX_FLAG_NO_EFFICIENCY);
+        const uint64_t tile = wave ? stride : small ? Small::kTile : (mid ? Mid::kTile : Big::kTile);
         const uint64_t tiles = (n + tile - 1) / tile;
         if (tiles > 0x7fffffffull) return fail(OPX_ERR_INVALID_ARG, "n too large for one launch");
         if (det_tiles) *det_tiles = tiles;
         if (packet_stats) k_propagate_packet<512, 4, 2, true><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, nullptr, nullptr, (unsigned long long*)packet_stats, det, 0u);
         else if (wave) k_propagate_packet<1024, 1, 1, false><<<(unsigned)tiles, 1024, sizeof(Wave), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det, stride);
-        else if (lean) k_propagate_packet<448, 4, 2, false><<<(unsigned)tiles, 448, sizeof(Lean), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det, 0u);
         else if (mid) k_propagate_packet<256, 4, 4, false><<<(unsigned)tiles, 256, sizeof(Mid), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det, 0u);
         else if (small) k_propagate_packet<512, 1, 2, false><<<(unsigned)tiles, 512, sizeof(Small), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det, 0u);
         else k_propagate_packet<512, 4, 2, false><<<(unsigned)tiles, 512, sizeof(Big), stream>>>(dev, n, id_base, o, d, wl, seed, out, hitmap, (unsigned long long*)counters, nullptr, det, 0u);
         // the names ncu prints for these instantiations
-        set_last_kernel(packet_stats ? "k_propagate_packet<512, 4, 2, 1>" : wave ? "k_propagate_packet<1024, 1, 1, 0>" : lean ? "k_propagate_packet<448, 4, 2, 0>" : mid ? "k_propagate_packet<256, 4, 4, 0>"
+        set_last_kernel(packet_stats ? "k_propagate_packet<512, 4, 2, 1>" : wave ? "k_propagate_packet<1024, 1, 1, 0>" : mid ? "k_propagate_packet<256, 4, 4, 0>"
                         : small ? "k_propagate_packet<512, 1, 2, 0>" : "k_propagate_packet<512, 4, 2, 0>");
         binned = !packet_stats;
     }

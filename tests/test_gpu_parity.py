@@ -130,8 +130,8 @@ def test_c2_bench_launch_itself_against_the_oracle(toy):
 
 def test_both_cta_shapes_against_the_oracle(toy):
     """opx_propagate picks 512-photon tiles (one packet per warp) for small calls (on this scene: up to 75 776 photons), a single
-    wave of 1024-thread CTAs from there to 151 552 photons, and large tiles (on this small scene, in flight: 448 threads x 4
-    photons) above: 620 000 contiguous C3 photons take the large tiles, their first 50 000 alone the small ones, their first
+    wave of 1024-thread CTAs from there to 151 552 photons, and large tiles (512 threads x 4 photons)
+    above: 620 000 contiguous C3 photons take the large tiles, their first 50 000 alone the small ones, their first
     120 000 the single wave; all must reproduce the oracle, hence each other, bit for bit.  (The 512-thread
     shape is pinned by test_no_efficiency_trace_at_scale on this scene and by tests/test_gpu_filter.py on the large one.)"""
     sc, gs = toy
