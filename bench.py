@@ -36,7 +36,7 @@ BYTES_IN, BYTES_OUT = 28, 34                        # per photon: inputs, hit re
 L2_BYTES = 126e6
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the step's kernel, from the `ncu --set full` captures
 # summarised under profiles/ (per config, at the launch size this bench times; None until a capture exists)
-NCU_TRAFFIC_BYTES = {"C2": (566210304, 10_000_000), "C4": (6683943000, 100_000_000)}      # (bytes, photons of the captured launch)
+NCU_TRAFFIC_BYTES = {"C2": (565296128, 10_000_000), "C4": (6683452000, 100_000_000)}      # (bytes, photons of the captured launch)
 NCU_TRAFFIC_SOURCE = {"C2": "profiles/r02_k_propagate_packet.md (1e7 photons per launch)", "C4": "profiles/r02_k_propagate_packet.md (1e8 photons per launch)"}
 
 

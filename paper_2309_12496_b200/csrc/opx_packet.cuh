@@ -330,6 +330,86 @@ __device__ __forceinline__ Hit closest_hit_own(const SceneDev& sc, const RayR& r
     return h;
 }
 
+// The photon arrays of a tile in shared memory (inputs, then the segment in flight, then the record: section 8.3).
+struct TileView { float* o; float* d; float* wl; int* surface; const uint32_t* key; uint8_t* state; uint8_t* bounces; };
+
+// One packet: the 32 photons at sorted positions [32 gidx, 32 gidx + 32) of tile `t` (m photons; photon i of the tile is
+// global photon id0 + i) are walked segment by segment until each has reached its terminal state; records replace the
+// photons' segments in their shared-memory slots.  s_ref / s_tn / s_cb: the warp's traversal scratch.
+template <bool kStats>
+__device__ __forceinline__ void trace_packet(const SceneDev& sc, const TileView& t, int m, int gidx, uint64_t id0, uint64_t seed, bool have_wide,
+                                             int lane, int* s_ref, float* s_tn, float4* s_cb, BeamStats& bstats, unsigned long long* stats) {
+    const int slot = gidx * 32 + lane;
+    bool alive = slot < m;
+    const int i = alive ? (int)(t.key[slot] & 0xffffu) : 0;
+    // Only the bounce count and the triangle just left stay in registers across the traversal: the segment
+    // (origin, direction) lives in the photon's own shared-memory slot (rewritten after each reflection; nobody
+    // else reads or writes that slot), wavelength and id are re-read at each interaction, and the record
+    // replaces the segment in the slot the moment the photon terminates.
+    const float* so = t.o + 3 * i;
+    const float* sd = t.d + 3 * i;
+    uint32_t nb = 0;
+    int last = -1, last_j = -1;      // the triangle just left: global id (the record's) and leaf-order index (the walk's)
+    while (__any_sync(0xffffffffu, alive)) {
+        const float tmin = nb == 0 ? 0.f : sc.t_min;
+        Hit h;
+        RayR rw;
+        bool done = false;
+        {
+            const float ox = so[0], oy = so[1], oz = so[2], dx = sd[0], dy = sd[1], dz = sd[2];
+            rw = ray_setup_rot(so, sd, sc.n_tri);
+            Beam bm;
+            float s;
+            const unsigned tris_before = bstats.tris, visits_before = bstats.visits;
+            if (have_wide && beam_setup(sc, ox, oy, oz, dx, dy, dz, tmin, alive, bm, s)) {     // coherent packet: one beam through the 32-wide tree
+                done = bm.mixed ? closest_hit_beam<true, kStats>(sc, rw, bm, s, tmin, last_j, alive, lane, so, sd, s_ref, s_tn, s_cb, h, bstats)
+                                : closest_hit_beam<false, kStats>(sc, rw, bm, s, tmin, last_j, alive, lane, so, sd, s_ref, s_tn, s_cb, h, bstats);
+                if (kStats && done) {
+                    ++bstats.beam_segments;
+                    const unsigned dt = bstats.tris - tris_before, dv = bstats.visits - visits_before;
+                    const int bucket = min(15, 32 - __clz(dt));
+                    const int bb = min(3, (int)__shfl_sync(0xffffffffu, nb, __ffs(__ballot_sync(0xffffffffu, alive)) - 1));
+                    if (lane == 0) {
+                        atomicAdd(&stats[8 + bucket], 1ull); atomicAdd(&stats[24 + bucket], (unsigned long long)dt);
+                        atomicAdd(&stats[40 + bb], 1ull); atomicAdd(&stats[44 + bb], (unsigned long long)dt);
+                        atomicAdd(&stats[48 + bb], (unsigned long long)dv);
+                    }
+                }
+            }
+        }
+        if (!done) {
+            if (kStats) ++bstats.fallback_segments;
+            const float ox = so[0], oy = so[1], oz = so[2], dx = sd[0], dy = sd[1], dz = sd[2];
+            const Slab sl = slab_setup(ox, oy, oz, dx, dy, dz);
+            // every box is widened by the ray's own rounding slack, which matters for an origin beyond origin_limit only (8.2)
+            const float far_o = fmaxf(fmaxf(fabsf(ox), fabsf(oy)), fabsf(oz));
+            if (sc.flags & kFlagPacketWalk) {            // debug (opx_propagate_binary): the warp walks the binary tree as one packet
+                const bool far = __any_sync(0xffffffffu, alive && !(far_o < sc.origin_limit));
+                h = closest_hit_packet(sc, rw, sl, far_o * 9.5367431640625e-7f, tmin, last_j, alive, lane, s_ref, far ? 9 : 8);
+            } else {
+                h = Hit{kInf, -1, 0x7fffffff};
+                if (alive) h = closest_hit_own(sc, rw, sl, far_o * 9.5367431640625e-7f, tmin, last_j);
+            }
+        }
+        if (alive) {
+            Photon p;
+            photon_init(p, so[0], so[1], so[2], sd[0], sd[1], sd[2], t.wl[i], id0 + (uint64_t)i);
+            p.b = nb; p.last = last;
+            alive = interact(sc, h, rw, p, seed);
+            t.d[3 * i] = p.dx; t.d[3 * i + 1] = p.dy; t.d[3 * i + 2] = p.dz;
+            if (alive) {
+                t.o[3 * i] = p.ox; t.o[3 * i + 1] = p.oy; t.o[3 * i + 2] = p.oz;
+                nb = p.b; last = p.last; last_j = h.j;
+            } else {
+                t.o[3 * i] = p.px; t.o[3 * i + 1] = p.py; t.o[3 * i + 2] = p.pz;
+                t.wl[i] = __int_as_float(p.pixel);
+                t.surface[i] = p.surface;
+                t.state[i] = (uint8_t)p.state; t.bounces[i] = (uint8_t)p.b;
+            }
+        }
+    }
+}
+
 template <int kPktThreads, int kItems, int kPktCtas, bool kStats>
 __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(const SceneDev sc, uint64_t n, uint64_t id_base,
                                                                      const float* __restrict__ origins,
@@ -484,80 +564,13 @@ __global__ void __launch_bounds__(kPktThreads, kPktCtas) k_propagate_packet(cons
     //    (groups are handed out dynamically so that a slow packet does not hold up its warp's share)
     const int groups = (m + 31) >> 5;
     BeamStats bstats;
+    const TileView tv{sm.o, sm.d, sm.wl, sm.surface, sm.key, sm.state, sm.bounces};
     for (;;) {
         int gidx = 0;
         if (lane == 0) gidx = atomicAdd(&sm.next_group, 1);
         gidx = __shfl_sync(0xffffffffu, gidx, 0);
         if (gidx >= groups) break;
-        const int slot = gidx * 32 + lane;
-        bool alive = slot < m;
-        const int i = alive ? (int)(sm.key[slot] & 0xffffu) : 0;
-        // Only the bounce count and the triangle just left stay in registers across the traversal: the segment
-        // (origin, direction) lives in the photon's own shared-memory slot (rewritten after each reflection; nobody
-        // else reads or writes that slot), wavelength and id are re-read at each interaction, and the record
-        // replaces the segment in the slot the moment the photon terminates.
-        const float* so = sm.o + 3 * i;
-        const float* sd = sm.d + 3 * i;
-        uint32_t nb = 0;
-        int last = -1, last_j = -1;      // the triangle just left: global id (the record's) and leaf-order index (the walk's)
-        while (__any_sync(0xffffffffu, alive)) {
-            const float tmin = nb == 0 ? 0.f : sc.t_min;
-            Hit h;
-            RayR rw;
-            bool done = false;
-            {
-                const float ox = so[0], oy = so[1], oz = so[2], dx = sd[0], dy = sd[1], dz = sd[2];
-                rw = ray_setup_rot(so, sd, sc.n_tri);
-                Beam bm;
-                float s;
-                const unsigned tris_before = bstats.tris, visits_before = bstats.visits;
-                if (have_wide && beam_setup(sc, ox, oy, oz, dx, dy, dz, tmin, alive, bm, s)) {     // coherent packet: one beam through the 32-wide tree
-                    done = bm.mixed ? closest_hit_beam<true, kStats>(sc, rw, bm, s, tmin, last_j, alive, lane, so, sd, sm.stack[w], sm.beam_tn[w], sm.cull[w], h, bstats)
-                                    : closest_hit_beam<false, kStats>(sc, rw, bm, s, tmin, last_j, alive, lane, so, sd, sm.stack[w], sm.beam_tn[w], sm.cull[w], h, bstats);
-                    if (kStats && done) {
-                        ++bstats.beam_segments;
-                        const unsigned dt = bstats.tris - tris_before, dv = bstats.visits - visits_before;
-                        const int bucket = min(15, 32 - __clz(dt));
-                        const int bb = min(3, (int)__shfl_sync(0xffffffffu, nb, __ffs(__ballot_sync(0xffffffffu, alive)) - 1));
-                        if (lane == 0) {
-                            atomicAdd(&stats[8 + bucket], 1ull); atomicAdd(&stats[24 + bucket], (unsigned long long)dt);
-                            atomicAdd(&stats[40 + bb], 1ull); atomicAdd(&stats[44 + bb], (unsigned long long)dt);
-                            atomicAdd(&stats[48 + bb], (unsigned long long)dv);
-                        }
-                    }
-                }
-            }
-            if (!done) {
-                if (kStats) ++bstats.fallback_segments;
-                const float ox = so[0], oy = so[1], oz = so[2], dx = sd[0], dy = sd[1], dz = sd[2];
-                const Slab sl = slab_setup(ox, oy, oz, dx, dy, dz);
-                // every box is widened by the ray's own rounding slack, which matters for an origin beyond origin_limit only (8.2)
-                const float far_o = fmaxf(fmaxf(fabsf(ox), fabsf(oy)), fabsf(oz));
-                if (sc.flags & kFlagPacketWalk) {            // debug (opx_propagate_binary): the warp walks the binary tree as one packet
-                    const bool far = __any_sync(0xffffffffu, alive && !(far_o < sc.origin_limit));
-                    h = closest_hit_packet(sc, rw, sl, far_o * 9.5367431640625e-7f, tmin, last_j, alive, lane, sm.stack[w], far ? 9 : 8);
-                } else {
-                    h = Hit{kInf, -1, 0x7fffffff};
-                    if (alive) h = closest_hit_own(sc, rw, sl, far_o * 9.5367431640625e-7f, tmin, last_j);
-                }
-            }
-            if (alive) {
-                Photon p;
-                photon_init(p, so[0], so[1], so[2], sd[0], sd[1], sd[2], sm.wl[i], id_base + tile_base + (uint64_t)i);
-                p.b = nb; p.last = last;
-                alive = interact(sc, h, rw, p, seed);
-                sm.d[3 * i] = p.dx; sm.d[3 * i + 1] = p.dy; sm.d[3 * i + 2] = p.dz;
-                if (alive) {
-                    sm.o[3 * i] = p.ox; sm.o[3 * i + 1] = p.oy; sm.o[3 * i + 2] = p.oz;
-                    nb = p.b; last = p.last; last_j = h.j;
-                } else {
-                    sm.o[3 * i] = p.px; sm.o[3 * i + 1] = p.py; sm.o[3 * i + 2] = p.pz;
-                    sm.wl[i] = __int_as_float(p.pixel);
-                    sm.surface[i] = p.surface;
-                    sm.state[i] = (uint8_t)p.state; sm.bounces[i] = (uint8_t)p.b;
-                }
-            }
-        }
+        trace_packet<kStats>(sc, tv, m, gidx, id_base + tile_base, seed, have_wide, lane, sm.stack[w], sm.beam_tn[w], sm.cull[w], bstats, stats);
     }
     __syncthreads();
     if (kStats) {
