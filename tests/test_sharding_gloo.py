@@ -39,6 +39,9 @@ def _worker(rank, world, port, n_total, seed, out_dir):
     counters = torch.from_numpy(r["counters"].astype(np.int64))
     allreduce_accumulators(hitmap, counters)
     np.save(os.path.join(out_dir, f"state_{rank}.npy"), r["state"])
+    det = oracle.detected_list(r, id_base=300_000 + start)               # the rank's shard of the detected list
+    np.save(os.path.join(out_dir, f"det_id_{rank}.npy"), det.id)
+    np.save(os.path.join(out_dir, f"det_pos_{rank}.npy"), det.pos)
     if rank == 0:
         np.save(os.path.join(out_dir, "hitmap.npy"), hitmap.numpy())
         np.save(os.path.join(out_dir, "counters.npy"), counters.numpy())
@@ -60,6 +63,10 @@ def test_two_rank_shards_reproduce_single_rank(tmp_path):
     assert np.array_equal(np.load(tmp_path / "hitmap.npy").astype(np.uint32), ref["hitmap"])
     assert np.array_equal(np.load(tmp_path / "counters.npy").astype(np.uint64), ref["counters"])
     assert ref["hitmap"].sum() > 0
+    # the detected lists stay sharded: concatenated in rank order they are the single-rank list (ids increasing across ranks)
+    det = oracle.detected_list(ref, id_base=300_000)
+    assert np.array_equal(np.concatenate([np.load(tmp_path / f"det_id_{r}.npy") for r in range(world)]), det.id)
+    assert np.array_equal(np.concatenate([np.load(tmp_path / f"det_pos_{r}.npy") for r in range(world)]), det.pos)
 
 
 def _worker_chain(rank, world, port, n_total, seed, out_dir):
