@@ -119,24 +119,37 @@ __global__ void __launch_bounds__(kSortBlock) k_radix_hist(const uint64_t* __res
     hist[(size_t)threadIdx.x * n_blocks + blockIdx.x] = h[threadIdx.x];
 }
 
-// One block: exclusive scan of hist[digit][block] in (digit, block) order.
-__global__ void __launch_bounds__(256) k_radix_scan(uint32_t* hist, uint32_t n_blocks) {
+// One block of 32 warps: exclusive scan of hist[digit][block] in (digit, block) order.  A warp owns 8 digits; its lanes stride
+// over the blocks (coalesced) and scan them 32 at a time.
+__global__ void __launch_bounds__(1024) k_radix_scan(uint32_t* hist, uint32_t n_blocks) {
     __shared__ uint32_t tot[256];
-    const uint32_t d = threadIdx.x;
-    uint32_t sum = 0;
-    for (uint32_t b = 0; b < n_blocks; ++b) sum += hist[(size_t)d * n_blocks + b];
-    tot[d] = sum;
-    __syncthreads();
-    if (d == 0) {
-        uint32_t run = 0;
-        for (int k = 0; k < 256; ++k) { const uint32_t t = tot[k]; tot[k] = run; run += t; }
+    const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (uint32_t d = w; d < 256; d += 32) {
+        uint32_t sum = 0;
+        for (uint32_t b = lane; b < n_blocks; b += 32) sum += hist[(size_t)d * n_blocks + b];
+        sum = __reduce_add_sync(0xffffffffu, sum);
+        if (lane == 0) tot[d] = sum;
     }
     __syncthreads();
-    uint32_t run = tot[d];
-    for (uint32_t b = 0; b < n_blocks; ++b) {
-        const uint32_t t = hist[(size_t)d * n_blocks + b];
-        hist[(size_t)d * n_blocks + b] = run;
-        run += t;
+    if (w == 0) {      // exclusive scan of the 256 digit totals: 8 per lane
+        uint32_t c[8], sum = 0;
+        for (int k = 0; k < 8; ++k) { c[k] = tot[8 * lane + k]; sum += c[k]; }
+        uint32_t inc = sum;
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= (uint32_t)o) inc += y; }
+        uint32_t run = inc - sum;
+        for (int k = 0; k < 8; ++k) { tot[8 * lane + k] = run; run += c[k]; }
+    }
+    __syncthreads();
+    for (uint32_t d = w; d < 256; d += 32) {
+        uint32_t run = tot[d];
+        for (uint32_t b0 = 0; b0 < n_blocks; b0 += 32) {
+            const uint32_t b = b0 + lane;
+            const uint32_t t = b < n_blocks ? hist[(size_t)d * n_blocks + b] : 0u;
+            uint32_t inc = t;
+            for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= (uint32_t)o) inc += y; }
+            if (b < n_blocks) hist[(size_t)d * n_blocks + b] = run + inc - t;
+            run += __shfl_sync(0xffffffffu, inc, 31);
+        }
     }
 }
 
@@ -518,7 +531,7 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
         int cur = 0;
         for (int shift = 0; shift < 64; shift += 8) {
             k_radix_hist<<<nsb, kSortBlock, 0, stream>>>(tmp.keys[cur], (uint32_t)T, shift, tmp.hist, nsb);
-            k_radix_scan<<<1, 256, 0, stream>>>(tmp.hist, nsb);
+            k_radix_scan<<<1, 1024, 0, stream>>>(tmp.hist, nsb);
             k_radix_scatter<<<nsb, kSortBlock, 0, stream>>>(tmp.keys[cur], tmp.idx[cur], tmp.keys[cur ^ 1], tmp.idx[cur ^ 1],
                                                            (uint32_t)T, shift, tmp.hist, nsb);
             count_launch(3);
