@@ -47,7 +47,7 @@ opx_status opx_propagate_stats(const opx_scene* scene, uint64_t n, uint64_t phot
 /* Work counters of the PRODUCT kernel (k_propagate_packet, instrumented instantiation): same records
  * as opx_propagate into `out` (DEVICE arrays of n), no binning, and ADDS to d_stats (8 uint64, DEVICE):
  * [0] packet-segments (one closest-hit query of a 32-photon packet) answered by beam traversal of the
- * 32-wide tree, [1] packet-segments answered by the binary packet walk (incoherent packets, stack
+ * 32-wide tree, [1] packet-segments answered by the per-lane walk of the binary tree (incoherent packets, stack
  * overflow, no wide tree), [2] wide nodes visited, [3] triangles handed to the lanes by beam traversal
  * (each is tested by every live lane), [4] beam-stack overflows, [5..7] reserved.  Never timed. */
 opx_status opx_propagate_packet_stats(const opx_scene* scene, uint64_t n, uint64_t photon_id_base,

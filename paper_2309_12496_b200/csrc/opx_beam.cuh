@@ -132,7 +132,7 @@ __device__ __forceinline__ bool beam_setup(const SceneDev& sc, float ox, float o
 }
 
 // Closest hit of the packet by beam traversal.  Returns false (warp-uniform) if the shared-memory
-// stack overflowed: the caller then redoes the segment with the binary packet walk.
+// stack overflowed: the caller then redoes the segment with the per-lane walk of the binary tree.
 // (so, sd) point at the lane's own segment in shared memory (origin, direction; not re-based): the per-lane cull
 // reads it back from there, so the segment does not occupy registers during the walk.
 // s_cb: 2 x kCullSlots float4 of the warp: the candidate boxes of the node being culled, (near planes, child ref) and

@@ -6,7 +6,7 @@ the cheap slab / beam arithmetic and the padding of the boxes are under the most
     (the reciprocal of the slab test is infinite there);
   * origins far outside the scene (the contract's vertex - origin rounds to ulps of the ORIGIN);
   * grazing incidence (1e-6 .. 1e-3 rad) on sliver triangles (aspect 1e4) and on very large triangles, at
-    coordinates near 3000 mm, in coherent bundles (beam traversal) and mixed (binary packet walk);
+    coordinates near 3000 mm, in coherent bundles (beam traversal) and mixed (per-lane walk of the binary tree);
   * bundles whose direction components straddle zero (they flip the beam's "mixed axis" handling);
   * origins lying exactly on box faces.
 
