@@ -216,3 +216,32 @@ def test_grazing_rays_on_the_c4_scene_mirrors():
     lam = rng.uniform(200, 600, len(o)).astype(np.float32)
     sample = np.sort(rng.choice(len(lam), 1500, replace=False))
     _check(sc, gs, o, d, lam, 9, "grazing on C4 mirrors", sample=sample, brute=False)
+
+
+def test_incoherent_packets_take_the_per_lane_walk(toy):
+    """Packets of unrelated rays -- isotropic directions from origins scattered through the enclosure, in an order that puts
+    no two neighbours into one packet -- are too wide for a beam: every packet-segment is walked per lane through the binary
+    tree (closest_hit_own), in all four kernel shapes' size ranges; a block of coherent cone photons in the middle of the call
+    makes the same tiles hold beam packets and per-lane packets side by side."""
+    sc, gs = toy
+    rng = np.random.default_rng(77)
+    n = 160_000
+    lo, hi = sc.meshes[-1]["vertices"].min(axis=0) + 5.0, sc.meshes[-1]["vertices"].max(axis=0) - 5.0
+    o = (lo + (hi - lo) * rng.random((n, 3))).astype(np.float32)
+    d = _unit(rng.normal(size=(n, 3))).astype(np.float32)
+    lam = rng.uniform(200.0, 600.0, n).astype(np.float32)
+    w = wl.make_config("C2", n=200_000)
+    co, cd, cl = w.photon_range(0, 40_000)
+    o[60_000:100_000], d[60_000:100_000], lam[60_000:100_000] = co, cd, cl
+    sample = np.arange(0, n, 41)
+    prod = _check(sc, gs, o, d, lam, 9, "incoherent rays", sample=sample)
+    assert len(np.unique(prod["state"])) >= 4
+    # the instrumented product kernel saw both kinds of packet-segments
+    _, st = gs.propagate_packet_stats(*_dev(o, d, lam), seed=9)
+    assert st["fallback_segments"] > 3000 and st["beam_segments"] > 1000
+    # sizes that take the 512-photon tiles, the single wave and the large tiles
+    for m in (3_000, 100_000, n):
+        do, dd, dl = _dev(o[:m], d[:m], lam[:m])
+        part = _host(gs.propagate(do, dd, dl, seed=9))
+        for k in KEYS_INT + ("pos", "dir"):
+            assert np.array_equal(part[k], prod[k][:m], equal_nan=k in ("pos", "dir")), (m, k)
