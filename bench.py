@@ -530,7 +530,8 @@ def main():
                 raise SystemExit("bench: host record path and device path disagree")
             del host_out
             if w.track_source is not None and id_base == 0:
-                steps_h = w.track_source.steps()
+                # the step table in page-locked host memory, like the photon arrays of the other legs
+                steps_h = {k: torch.from_numpy(v).pin_memory().numpy() for k, v in w.track_source.steps().items()}
                 kinds_ = [m["kind"] for m in w.scene.materials]
                 fac_ = [kinds_.index(2)] + [kinds_.index(1)] * (2 if args.config in ("C4", "C5") else 1)
                 tr = {}
