@@ -315,6 +315,45 @@ def test_c4_scene_bvh_and_sampled_parity(lhcb):
     assert a["counters"][:7].sum() == len(ids2) and a["hitmap"].sum() == a["counters"][0]
 
 
+def test_c4_bench_launch_itself_against_the_oracle(lhcb):
+    """The launch bench.py's headline times -- all 1e8 track photons of C4, contiguous ids, ONE opx_propagate call on the
+    1.01e6-triangle scene -- against the oracle on every 250 000th of its records (the oracle traces those ids alone), plus the
+    size-independent properties on all 1e8; the detected-only form of the same launch lists exactly the DETECTED records."""
+    import concurrent.futures
+    sc, gs = lhcb
+    w = wl.make_config("C4")
+    n = w.n
+    pin = [torch.empty((n, 3), dtype=torch.float32), torch.empty((n, 3), dtype=torch.float32), torch.empty(n, dtype=torch.float32)]
+    step = 2_000_000
+
+    def fill(a):
+        for dst, src in zip(pin, w.photon_range(a, min(n, a + step))):
+            dst[a:a + step] = torch.from_numpy(src)
+    with concurrent.futures.ThreadPoolExecutor(max_workers=8) as ex:
+        list(ex.map(fill, range(0, n, step)))
+    do, dd, dl = (x.cuda() for x in pin)
+    got = gs.propagate(do, dd, dl, seed=0)
+    assert pkg.last_kernel() == "k_propagate_packet<512, 4, 2, 0>"
+    torch.cuda.synchronize()
+    ids = np.arange(11, n, 250_000, dtype=np.uint64)
+    idx = torch.from_numpy(ids.astype(np.int64)).cuda()
+    sub = {k: got[k][idx].cpu().numpy() for k in ("state", "pixel", "surface", "bounces", "pos", "dir")}
+    o, d, lam = w.photons(ids)
+    ref = oracle.trace_mesh(sc, o, d, lam, seed=0, ids=ids)
+    for k in ("state", "pixel", "surface", "bounces"):
+        assert np.array_equal(sub[k], ref[k]), k
+    assert np.array_equal(sub["pos"].astype(np.float64), ref["pos"]) and np.array_equal(sub["dir"].astype(np.float64), ref["dir"])
+    cnt = got["counters"].cpu().numpy()
+    assert cnt[:7].sum() == n and int(got["hitmap"].long().sum().item()) == cnt[0]
+    det = got["state"] == 0
+    assert torch.equal(torch.bincount(got["pixel"][det].long(), minlength=gs.n_pixels).int(), got["hitmap"].int())
+    lst = gs.propagate_detected(do, dd, dl, seed=0, capacity=int(cnt[0]) + 16)
+    torch.cuda.synchronize()
+    k = int(lst["n_detected"].item())
+    assert k == cnt[0] and torch.equal(lst["id"][:k], torch.nonzero(det).flatten())
+    assert torch.equal(lst["pos"][:k], got["pos"][det]) and torch.equal(lst["pixel"][:k], got["pixel"][det])
+
+
 def test_c5_sampled_parity(lhcb):
     """Config 4 (the stress config): every 500 000th photon id of the 1e9-photon workload of mixed tracks
     (beta in [0.9999, 1], origins in a 200 mm disc) on the C4 scene against the oracle, through a chunked call
