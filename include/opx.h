@@ -219,6 +219,34 @@ opx_status opx_prefilter(const opx_scene* scene, uint64_t n, uint64_t photon_id_
                          uint64_t out_capacity, uint64_t* d_n_kept, void* d_workspace, size_t workspace_bytes,
                          void* cuda_stream);
 
+/* opx_prefilter for callers that cannot allocate device memory.  Some users of this library never get to call
+ * cudaMalloc: a plug-in inside an experiment framework (a Geant4 worker, a trigger-farm process) is handed its photon
+ * buffers by the framework's memory pool, which has reserved the whole card and forbids allocations of its own; and a
+ * worker thread in an event loop that shares the GPU with other threads' streams cannot afford cudaMalloc / cudaFree,
+ * which make every stream on the device wait.  Such a caller has input and output arrays but nowhere to put the
+ * filter's workspace.  This call needs none: the mask words and per-block counts live in a fixed array compiled into
+ * libopx.so (about 2 MiB; every GPU that loads the library's device code holds it until the process exits).
+ *   - Arguments, results and errors are those of opx_prefilter without d_workspace / workspace_bytes; the output is the
+ *     same bytes opx_prefilter produces.  The caller still owns and passes every input and output array.
+ *   - n <= OPX_PREFILTER_NOALLOC_MAX_PHOTONS, otherwise OPX_ERR_INVALID_ARG with a message naming the limit: split the
+ *     photons over several calls (photon_id_base keeps the draws identical) or use opx_prefilter.
+ *   - The call never allocates or frees device memory, neither directly nor through a library routine: it enqueues the
+ *     three kernels of opx_prefilter (for n = 0 one 8-byte memset of *d_n_kept) and returns.
+ *   - The first call with n >= 1 on each device looks up where that device keeps the array (one cudaGetSymbolAddress,
+ *     which loads the library's device code there if it is not loaded yet) and remembers the answer.  Make that first
+ *     call with the device current and before any stream capture begins; a call with n = 0 does not do the look-up.
+ *   - All calls on one device share the one array, and it keeps whatever the previous call left in it.  The kernels
+ *     overwrite every word they later read, so nothing has to be cleared between calls -- but two calls whose kernels
+ *     can run at the same time on one GPU (different streams without an event between them, or two host threads)
+ *     overwrite each other's masks and give wrong survivors.  Order such calls on one stream or with events.
+ *   - Device ordinals 0..63. */
+#define OPX_PREFILTER_NOALLOC_MAX_PHOTONS 16777216ull /* 2^24 photons per call */
+opx_status opx_prefilter_noalloc(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
+                                 const float* d_dirs, const float* d_wavelengths, uint64_t seed,
+                                 const uint32_t* factors, uint32_t n_factors,
+                                 float* d_out_origins, float* d_out_dirs, float* d_out_wavelengths, uint32_t* d_out_index,
+                                 uint64_t out_capacity, uint64_t* d_n_kept, void* cuda_stream);
+
 /* Track steps for opx_emit_cherenkov: DEVICE pointers.  Step s starts at x[s], runs along the unit vector w[s] for
  * length[s] mm with velocity beta[s]; first (n_steps + 1 entries, non-decreasing, first[0] = 0) is the exclusive
  * prefix sum of the photons emitted per step: global photon g belongs to the step with first[s] <= g < first[s+1].

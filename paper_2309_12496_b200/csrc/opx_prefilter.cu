@@ -146,3 +146,88 @@ opx_status launch_prefilter(const SceneHost& s, uint64_t n, uint64_t id_base, co
 }
 
 }  // namespace opx
+
+// ------------------------------------------------------------------ opx_prefilter_noalloc (include/opx.h)
+// The filter for callers that have no device memory to give it and may not ask the driver for any: a Geant4 worker
+// or an experiment-framework plug-in that was handed a fixed set of device buffers by the framework's own pool (the
+// pool holds the whole card, so a cudaMalloc from inside the plug-in fails or is forbidden by the host code's rules),
+// and event loops in which several worker threads keep their own streams busy on one GPU, where a cudaMalloc /
+// cudaFree would make the whole device wait.  The mask words and per-CTA counts that opx_prefilter keeps in the
+// caller's workspace live here in ONE array that is part of the library image: every GPU on which the library's code
+// gets loaded holds these bytes from then until the process exits, whether or not the entry point is ever called.
+#include <mutex>
+
+namespace opx {
+namespace {
+
+constexpr uint64_t kNoAllocMaxPhotons = OPX_PREFILTER_NOALLOC_MAX_PHOTONS;
+constexpr size_t kNoAllocBlocks = (size_t)((kNoAllocMaxPhotons + kBlk - 1) / kBlk);
+// the layout launch_prefilter() carves out of a workspace: mask words, then per-CTA counts, then one spare line
+constexpr size_t kNoAllocBytes = (kNoAllocBlocks * kWords * 4 + 255) / 256 * 256 + (kNoAllocBlocks * 4 + 255) / 256 * 256 + 256;
+static_assert(kNoAllocBytes <= (size_t)(2u << 20) + (64u << 10), "the built-in scratch is meant to stay near 2 MiB");
+
+// In HOST code this name is only a handle for the runtime's symbol table - it is not where the bytes are on the GPU,
+// and handing it to a kernel would fault (or, where the GPU can reach host memory, quietly scribble over the host-side
+// shadow).  Host code must go through noalloc_scratch() below.  Device code could name the array directly.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+constexpr int kMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+void* g_noalloc_addr[kMaxDevices] = {};   // device address of g_noalloc_scratch on device k, looked up once
+
+// Device address of the built-in scratch on the CURRENT device.  Each device has its own copy of the array at its own
+// address, so the look-up is done once per device, with that device current, and remembered.  The look-up makes the
+// runtime load this library's device code on that device if nothing has yet; it allocates nothing.
+opx_status noalloc_scratch(void** out) {
+    int dev = -1;
+    if (cudaError_t e = cudaGetDevice(&dev)) return check_cuda(e, "cudaGetDevice");
+    if (dev < 0 || dev >= kMaxDevices) return fail(OPX_ERR_UNSUPPORTED_DEVICE, "opx_prefilter_noalloc: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_addr[dev]) {
+        void* p = nullptr;
+        if (cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_scratch)) return check_cuda(e, "cudaGetSymbolAddress(built-in prefilter scratch)");
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) return fail(OPX_ERR_CUDA, "built-in prefilter scratch has no usable device address");
+        g_noalloc_addr[dev] = p;
+    }
+    *out = g_noalloc_addr[dev];
+    return OPX_OK;
+}
+
+}  // namespace
+}  // namespace opx
+
+extern "C" opx_status opx_prefilter_noalloc(const opx_scene* scene, uint64_t n, uint64_t photon_id_base, const float* d_origins,
+                                            const float* d_dirs, const float* d_wavelengths, uint64_t seed,
+                                            const uint32_t* factors, uint32_t n_factors, float* d_out_origins,
+                                            float* d_out_dirs, float* d_out_wavelengths, uint32_t* d_out_index,
+                                            uint64_t out_capacity, uint64_t* d_n_kept, void* cuda_stream) {
+    using namespace opx;
+    auto off = [](const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) != 0; };
+    if (!scene) return fail(OPX_ERR_INVALID_ARG, "scene is NULL");
+    if (!scene->built) return fail(OPX_ERR_BAD_STATE, "opx_prefilter_noalloc before opx_bvh_build");
+    if (!d_n_kept || off(d_n_kept, 8)) return fail(OPX_ERR_INVALID_ARG, "d_n_kept is NULL or misaligned");
+    if (n > kNoAllocMaxPhotons)
+        return fail(OPX_ERR_INVALID_ARG, "opx_prefilter_noalloc: n = " + std::to_string(n) + " photons is beyond the " +
+                                             std::to_string(kNoAllocMaxPhotons) + " (OPX_PREFILTER_NOALLOC_MAX_PHOTONS) the built-in " +
+                                             "scratch holds; split the call or use opx_prefilter with a workspace of your own");
+    if (n_factors > 8 || (n_factors && !factors)) return fail(OPX_ERR_INVALID_ARG, "n_factors must be <= 8 and factors non-NULL");
+    for (uint32_t k = 0; k < n_factors; ++k) {
+        if (factors[k] >= scene->mat_kinds.size()) return fail(OPX_ERR_INVALID_ARG, "factor material index out of range");
+        if ((scene->mat_kinds[factors[k]] & 0xffu) == OPX_MAT_ABSORBER) return fail(OPX_ERR_INVALID_ARG, "an absorber has no efficiency table");
+    }
+    if (opx_status st = check_cuda(cudaGetLastError(), "pending CUDA error before opx_prefilter_noalloc")) return st;
+    if (n == 0) return check_cuda(cudaMemsetAsync(d_n_kept, 0, 8, (cudaStream_t)cuda_stream), "cudaMemsetAsync");
+    if (!d_origins || !d_dirs || !d_wavelengths || !d_out_origins || !d_out_dirs || !d_out_wavelengths)
+        return fail(OPX_ERR_INVALID_ARG, "NULL photon pointer");
+    if (off(d_origins, 4) || off(d_dirs, 4) || off(d_wavelengths, 4) || off(d_out_origins, 4) || off(d_out_dirs, 4) ||
+        off(d_out_wavelengths, 4) || off(d_out_index, 4))
+        return fail(OPX_ERR_INVALID_ARG, "misaligned pointer");
+    if (d_out_origins == d_origins || d_out_dirs == d_dirs || d_out_wavelengths == d_wavelengths)
+        return fail(OPX_ERR_INVALID_ARG, "out arrays must not alias the inputs");
+    void* scratch = nullptr;
+    if (opx_status st = noalloc_scratch(&scratch)) return st;
+    // Nothing in the scratch has to start at zero: k_prefilter_mark writes every mask word and every per-CTA count that
+    // k_prefilter_scan and k_prefilter_compact read for this n, so what the previous call left behind is never seen.
+    return launch_prefilter(*scene, n, photon_id_base, d_origins, d_dirs, d_wavelengths, seed, factors, n_factors, d_out_origins,
+                            d_out_dirs, d_out_wavelengths, d_out_index, out_capacity, d_n_kept, scratch, (cudaStream_t)cuda_stream);
+}

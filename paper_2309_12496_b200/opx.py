@@ -19,11 +19,12 @@ OPX_OK, OPX_ERR_INVALID_ARG, OPX_ERR_BAD_STATE, OPX_ERR_WORKSPACE_TOO_SMALL, OPX
     OPX_ERR_UNSUPPORTED_DEVICE = range(6)
 
 FLAG_NO_EFFICIENCY = 1                   # opx_flags
+PREFILTER_NOALLOC_MAX_PHOTONS = 1 << 24  # OPX_PREFILTER_NOALLOC_MAX_PHOTONS
 TABLE_LINEAR, TABLE_HISTOGRAM = 0, 1     # opx_table_interp
 
 # the product boundary (include/opx.h) ...
 EXPORTS = ("opx_scene_create", "opx_scene_workspace_bytes", "opx_bvh_build", "opx_propagate",
-           "opx_propagate_flags", "opx_prefilter_workspace_bytes", "opx_prefilter", "opx_emit_cherenkov",
+           "opx_propagate_flags", "opx_prefilter_workspace_bytes", "opx_prefilter", "opx_prefilter_noalloc", "opx_emit_cherenkov",
            "opx_emit_cherenkov_filtered", "opx_propagate_host_workspace_bytes", "opx_propagate_host",
            "opx_propagate_detected_workspace_bytes", "opx_propagate_detected",
            "opx_propagate_host_detected_workspace_bytes", "opx_propagate_host_detected",
@@ -106,6 +107,7 @@ def load_library(path=LIB_PATH):
     lib.opx_propagate_flags.argtypes = [vp, u64, vp, u64, vp, vp, vp, u64, u32, vp, vp, vp, vp]
     lib.opx_prefilter_workspace_bytes.argtypes = [u64, vp]
     lib.opx_prefilter.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, u32, vp, vp, vp, vp, u64, vp, vp, C.c_size_t, vp]
+    lib.opx_prefilter_noalloc.argtypes = [vp, u64, u64, vp, vp, vp, u64, vp, u32, vp, vp, vp, vp, u64, vp, vp]
     lib.opx_emit_cherenkov.argtypes = [vp, u64, C.c_float, C.c_float, C.c_float, u64, u64, u64, vp, vp, vp, vp]
     lib.opx_emit_cherenkov_filtered.argtypes = [vp, vp, u64, C.c_float, C.c_float, C.c_float, u64, u64, u64, vp, u32,
                                                 vp, vp, vp, vp, u64, vp, vp, C.c_size_t, vp]
@@ -433,6 +435,25 @@ class Scene:
             fac, len(factors), out["origins"].data_ptr(), out["dirs"].data_ptr(), out["wavelengths"].data_ptr(),
             None if idx is None else idx.data_ptr(), int(out["wavelengths"].shape[0]), out["n_kept"].data_ptr(), _aligned(ws),
             need.value, C.c_void_p(st.cuda_stream)))
+        return out
+
+    def prefilter_noalloc(self, origins, dirs, wavelengths, factors, out, seed=0, photon_id_base=0, stream=None):
+        """opx_prefilter_noalloc: prefilter() for a caller that may not allocate device memory (a plug-in living on buffers
+        a framework's pool handed it, a worker thread that must not stall the other streams of its GPU with cudaMalloc).
+        Nothing is allocated here either: `out` is required and must already hold the caller's tensors origins (cap, 3),
+        dirs (cap, 3), wavelengths (cap,) float32, n_kept (1,) int64 and optionally index (cap,) int32; the scratch is
+        the library's built-in array, so n <= PREFILTER_NOALLOC_MAX_PHOTONS (OpxError otherwise) and calls that could
+        overlap on one GPU must be ordered by the caller.  Same survivors, same order, same bytes as prefilter()."""
+        import torch
+        n = int(wavelengths.shape[0])
+        fac = (C.c_uint32 * max(1, len(factors)))(*[int(f) for f in factors])
+        st = stream if stream is not None else torch.cuda.current_stream(wavelengths.device)
+        idx = out.get("index")
+        _check(load_library().opx_prefilter_noalloc(
+            self._h, n, int(photon_id_base), origins.data_ptr(), dirs.data_ptr(), wavelengths.data_ptr(), int(seed),
+            fac, len(factors), out["origins"].data_ptr(), out["dirs"].data_ptr(), out["wavelengths"].data_ptr(),
+            None if idx is None else idx.data_ptr(), int(out["wavelengths"].shape[0]), out["n_kept"].data_ptr(),
+            C.c_void_p(st.cuda_stream)))
         return out
 
     def emit_cherenkov_filtered(self, dev_steps, n, factors, photon_id_base=0, seed=0, n_index=1.0014, lambda1=200.0,
