@@ -9,6 +9,7 @@
 // never culls a triangle the contract test of DESIGN.md 3.3 accepts -- hence the padding here.
 #include <cfloat>
 #include <cmath>
+#include <mutex>
 
 #include "opx_internal.cuh"
 
@@ -374,7 +375,9 @@ __device__ __forceinline__ void collapse_level(const NodeDev* __restrict__ bn, c
     }
 }
 
-// Barrier across the CTAs of a grid that is resident as a whole (k_collapse_all is launched with at most two CTAs per SM).
+// Barrier across the CTAs of a grid that is resident as a whole.  k_collapse_all is launched with cudaLaunchCooperativeKernel
+// (launch_collapse below), so the runtime refuses a grid that could not be co-resident instead of letting it spin for ever;
+// where cooperative launches are not available the kernel runs as ONE CTA, for which the barrier is a __syncthreads.
 // bar[0] counts arrivals, bar[1] is the generation.
 __device__ __forceinline__ void grid_barrier(uint32_t* bar) {
     __syncthreads();
@@ -391,9 +394,9 @@ __device__ __forceinline__ void grid_barrier(uint32_t* bar) {
 // The whole collapse in ONE launch: the levels of the 32-wide tree are produced one after the other with a grid barrier in
 // between, the size of each level being known on the device only.  counters: [0] tasks of this level, [1] tasks of the next,
 // [2] wide nodes so far, [3] capacity overflow, [4..5] the barrier.  On exit *wide_count = number of wide nodes, or 0 if the
-// tree outgrew its capacity (packets then walk the binary tree).  The host reads nothing back: opx_bvh_build returns after
-// enqueueing and can be captured into a CUDA graph.
-__global__ void __launch_bounds__(256) k_collapse_all(const NodeDev* __restrict__ bn, int2* q0, int2* q1, uint32_t* counters, WNodeDev* wn,
+// tree outgrew its capacity or is deeper than the level loop (packets then walk the binary tree).  The host reads nothing
+// back: opx_bvh_build returns after enqueueing.
+__global__ void __launch_bounds__(256, 2) k_collapse_all(const NodeDev* __restrict__ bn, int2* q0, int2* q1, uint32_t* counters, WNodeDev* wn,
                                                       uint32_t cap_wn, uint32_t* wide_count) {
     int2* q_in = q0;
     int2* q_out = q1;
@@ -410,12 +413,58 @@ __global__ void __launch_bounds__(256) k_collapse_all(const NodeDev* __restrict_
         grid_barrier(counters + 4);
         int2* t = q_in; q_in = q_out; q_out = t;
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) *wide_count = atomicAdd(&counters[3], 0u) ? 0u : atomicAdd(&counters[2], 0u);
+    // counters[0] != 0 here: the level loop ran out with tasks still pending (a tree deeper than 128 wide levels) - no wide tree
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        *wide_count = (atomicAdd(&counters[3], 0u) || atomicAdd(&counters[0], 0u)) ? 0u : atomicAdd(&counters[2], 0u);
 }
 
 __global__ void k_collapse_init(int2* q, uint32_t* counters) {
     q[0] = make_int2(0, 0);
     counters[0] = 1u; counters[1] = 0u; counters[2] = 1u; counters[3] = 0u; counters[4] = 0u; counters[5] = 0u;
+}
+
+// Largest grid of k_collapse_all that is resident as a whole on the current device (at most two CTAs per SM: more only adds
+// arrivals at the barrier), and whether the device takes cooperative launches; queried once per device.
+constexpr int kCollapseThreads = 256;
+struct CollapseShape { int max_grid = 0; bool cooperative = false; bool known = false; };
+std::mutex g_collapse_mutex;
+CollapseShape g_collapse_shape[64];
+
+opx_status collapse_shape(CollapseShape* out) {
+    int dev = 0;
+    if (cudaError_t e = cudaGetDevice(&dev)) return check_cuda(e, "cudaGetDevice");
+    if (dev < 0 || dev >= 64) return fail(OPX_ERR_UNSUPPORTED_DEVICE, "device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(g_collapse_mutex);
+    CollapseShape& c = g_collapse_shape[dev];
+    if (!c.known) {
+        int coop = 0, sms = 0, per_sm = 0;
+        cudaError_t e;
+        if ((e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev)) ||
+            (e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) ||
+            (e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_collapse_all, kCollapseThreads, 0)))
+            return check_cuda(e, "k_collapse_all occupancy query");
+        c.cooperative = coop != 0 && per_sm >= 1 && sms >= 1;
+        c.max_grid = c.cooperative ? std::min(per_sm, 2) * sms : 1;
+        c.known = true;
+    }
+    *out = c;
+    return OPX_OK;
+}
+
+// One launch for all levels.  Cooperative: the runtime checks that the grid fits on the device (or the MIG slice / SM partition
+// the context really has) and returns an error otherwise, so a wrong guess is an OPX_ERR_CUDA, never a hang.
+opx_status launch_collapse(const NodeDev* nodes, int2* q0, int2* q1, uint32_t* counters, WNodeDev* wnodes, uint32_t cap,
+                           uint32_t* wide_count, size_t wanted_grid, cudaStream_t stream) {
+    CollapseShape shape;
+    if (opx_status st = collapse_shape(&shape)) return st;
+    const uint32_t grid = (uint32_t)std::max<size_t>(1, std::min<size_t>(wanted_grid, (size_t)shape.max_grid));
+    if (shape.cooperative) {
+        void* args[] = {(void*)&nodes, (void*)&q0, (void*)&q1, (void*)&counters, (void*)&wnodes, (void*)&cap, (void*)&wide_count};
+        return check_cuda(cudaLaunchCooperativeKernel((const void*)k_collapse_all, dim3(grid), dim3(kCollapseThreads), args, 0, stream),
+                          "k_collapse_all (cooperative launch)");
+    }
+    k_collapse_all<<<1, kCollapseThreads, 0, stream>>>(nodes, q0, q1, counters, wnodes, cap, wide_count);
+    return check_cuda(cudaGetLastError(), "k_collapse_all (single CTA)");
 }
 
 }  // namespace
@@ -547,8 +596,9 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
         WNodeDev* wnodes = (WNodeDev*)(ws + lay.wide_nodes);
         const uint32_t cap = (uint32_t)lay.wide_node_capacity;
         k_collapse_init<<<1, 1, 0, stream>>>(tmp.queue[0], tmp.wcount);
-        const uint32_t grid = (uint32_t)std::min<size_t>((lay.wide_node_capacity + 7) / 8, 296);      // resident as a whole: <= 2 CTAs per SM
-        k_collapse_all<<<grid, 256, 0, stream>>>(nodes, tmp.queue[0], tmp.queue[1], tmp.wcount, wnodes, cap, (uint32_t*)(ws + lay.wide_count));
+        if (opx_status st = launch_collapse(nodes, tmp.queue[0], tmp.queue[1], tmp.wcount, wnodes, cap, (uint32_t*)(ws + lay.wide_count),
+                                            (lay.wide_node_capacity + 7) / 8, stream))
+            return st;
         count_launch(2);
     } else {
         if ((e = cudaMemsetAsync(ws + lay.wide_count, 0, 4, stream))) return check_cuda(e, "memset wide count");
