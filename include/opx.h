@@ -26,7 +26,11 @@
  *     opx_last_error() gives a thread-local message for the last non-OK status.
  *   Device: requires compute capability 10.x (B200); anything else => OPX_ERR_UNSUPPORTED_DEVICE.
  *   Threading: a built scene is immutable; concurrent opx_propagate calls on different streams
- *     are allowed.
+ *     are allowed.  opx_bvh_build and opx_scene_destroy need the scene to themselves: no other call on
+ *     that scene may be running or start until they return.  The host-buffer calls (opx_propagate_host,
+ *     opx_propagate_host_detected, opx_tracks_host_detected) share one set of internal streams per scene:
+ *     concurrent ones wait for each other, and all of them must be made with the device current on which
+ *     the scene was built (OPX_ERR_BAD_STATE otherwise).
  */
 #ifndef OPX_H_
 #define OPX_H_

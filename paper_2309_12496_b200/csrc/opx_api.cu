@@ -195,6 +195,7 @@ opx_status opx_bvh_build(opx_scene* scene, void* d_scene_ws, size_t scene_bytes,
     scene->d_scene_ws = d_scene_ws;
     scene->scene_bytes = scene_bytes;
     scene->built = true;
+    drop_host_pipe_of_other_device(*scene);      // a rebuild on another GPU: the streams of the host-buffer calls follow
     return OPX_OK;
 }
 
@@ -358,12 +359,22 @@ void destroy_host_pipe(HostPipe* p) {
     delete p;
 }
 static std::mutex g_pipe_mutex;
+void drop_host_pipe_of_other_device(const SceneHost& s) {
+    std::lock_guard<std::mutex> lock(g_pipe_mutex);
+    int dev = 0;
+    if (!s.pipe || cudaGetDevice(&dev) != cudaSuccess || s.pipe->device == dev) return;
+    destroy_host_pipe(s.pipe);
+    s.pipe = nullptr;
+}
 // The scene's pipe, created on its first host-buffer call (streams and events are not created per call).
 static opx_status host_pipe(const SceneHost& s, HostPipe** out) {
     std::lock_guard<std::mutex> lock(g_pipe_mutex);
     int dev = 0;
     if (opx_status st = check_cuda(cudaGetDevice(&dev), "cudaGetDevice")) return st;
-    if (s.pipe && s.pipe->device != dev) { destroy_host_pipe(s.pipe); s.pipe = nullptr; }
+    // never torn down here: another thread may be inside propagate_host_impl with these streams (opx_bvh_build, which needs the
+    // scene to itself anyway, drops the pipe when the scene moves to another device)
+    if (s.pipe && s.pipe->device != dev)
+        return fail(OPX_ERR_BAD_STATE, "host-buffer call with another device current than the one this scene's host-buffer calls started on");
     if (!s.pipe) {
         HostPipe* p = new HostPipe;
         p->device = dev;

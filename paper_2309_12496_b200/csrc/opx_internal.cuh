@@ -77,6 +77,8 @@ struct DetOut {
 // Streams and events of the host-buffer calls (opx_propagate_host*), created once per scene at the first such call.
 struct HostPipe;
 void destroy_host_pipe(HostPipe* p);
+struct SceneHost;
+void drop_host_pipe_of_other_device(const SceneHost& s);   // opx_bvh_build only: needs the scene to itself
 
 // ------------------------------------------------------------------------------ host-side scene
 struct SceneHost {
@@ -120,7 +122,7 @@ opx_status build_bvh(SceneHost& s, void* d_scene_ws, void* d_tmp_ws, cudaStream_
 
 // propagate (opx_propagate.cu)
 enum WalkMode { kWalkProduct = 0, kWalkBrute = 1, kWalkBinary = 2 };   // product path / every triangle (debug) / binary tree only (debug)
-opx_status configure_device();      // per-device kernel attributes (dynamic shared memory sizes); idempotent, thread-safe
+opx_status configure_device(int* sms = nullptr);      // per-device kernel attributes (dynamic shared memory sizes) and SM count; idempotent, thread-safe
 opx_status propagate_common(const opx_scene* scene, WalkMode mode, uint64_t n, const uint64_t* d_n, uint64_t base, const float* o,
                             const float* d, const float* wl, uint64_t seed, uint32_t flags, const opx_hits* out, uint32_t* hitmap,
                             uint64_t* counters, void* stream);

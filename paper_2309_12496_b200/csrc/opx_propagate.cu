@@ -14,24 +14,28 @@ using Big = PacketSmemT<512, 4>;      // 2048-photon tiles, 4 packets per warp: 
 using Small = PacketSmemT<512, 1>;    // 512-photon tiles, 1 packet per warp: calls too small to fill the machine
 using Mid = PacketSmemT<256, 4>;      // 1024-photon tiles, 4 CTAs/SM: filtered (NO_EFFICIENCY) streams
 using Wave = PacketSmemT<1024, 1>;    // one CTA per SM, one packet per warp, run-time tile size: a small call in a single wave
-constexpr uint64_t kSMs = 148;
+constexpr int kMaxDevices = 64;
+static std::atomic<int> g_sms[kMaxDevices];      // SM count per device ordinal, 0 = not configured yet
 
 // The dynamic shared memory limit of a kernel is an attribute per device (context): set once per device, at the first
 // opx_bvh_build or launch on it, so that a later opx_propagate performs stream operations only (CUDA-graph capturable).
-opx_status configure_device() {
-    static std::atomic<uint64_t> done{0};
+// The device's SM count, which decides the kernel shape of a small call, is looked up at the same time (*sms, may be NULL).
+opx_status configure_device(int* sms) {
     int dev = 0;
     if (opx_status st = check_cuda(cudaGetDevice(&dev), "cudaGetDevice")) return st;
-    const uint64_t bit = 1ull << (dev & 63);
-    if (done.load(std::memory_order_acquire) & bit) return OPX_OK;
-    cudaError_t e = cudaSuccess;
+    if (dev < 0 || dev >= kMaxDevices) return fail(OPX_ERR_UNSUPPORTED_DEVICE, "device ordinal beyond 63");
+    if (const int known = g_sms[dev].load(std::memory_order_acquire)) { if (sms) *sms = known; return OPX_OK; }
+    int count = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&count, cudaDevAttrMultiProcessorCount, dev);
+    if (!e && count < 1) return fail(OPX_ERR_UNSUPPORTED_DEVICE, "device reports no multiprocessors");
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 4, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Big));
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<512, 1, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Small));
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<256, 4, 4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Mid));
     if (!e) e = cudaFuncSetAttribute(k_propagate_packet<1024, 1, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Wave));
     if (opx_status st = check_cuda(e, "cudaFuncSetAttribute")) return st;
-    done.fetch_or(bit, std::memory_order_release);      // two threads racing here both set the same attributes: harmless
+    g_sms[dev].store(count, std::memory_order_release);      // two threads racing here both set the same attributes: harmless
+    if (sms) *sms = count;
     return OPX_OK;
 }
 
@@ -62,7 +66,9 @@ static opx_status launch_propagate_impl(const SceneHost& s, WalkMode mode, uint6
         // stream (NO_EFFICIENCY: 1 photon in 7-9 survives, so packets are wide and differ widely in cost; a tile's warps wait at
         // its barrier for the slowest packet) runs fastest with 4 CTAs of 256 threads and 1024-photon tiles on every scene (C4
         // survivors of 4e7 photons: 3.38 ms against 4.12 with 2 x 512; toy scene 0.280 against 0.320).
-        if (opx_status st = configure_device()) return st;
+        int sm_count = 0;
+        if (opx_status st = configure_device(&sm_count)) return st;
+        const uint64_t kSMs = (uint64_t)sm_count;      // 148 on a B200; the thresholds below were measured there
         // A small call (the paper's own runs are 600 ... 6e5 photons) is latency-bound: its time is the dependent
         // chain of ONE packet times the packets a warp walks one after the other.  Up to 148 x 512 photons the 512-photon tiles
         // (one packet per warp) already put every packet in flight at once; from there to 148 x 1024 photons the call runs as a
@@ -95,7 +101,9 @@ static opx_status launch_propagate_impl(const SceneHost& s, WalkMode mode, uint6
     if (ev) cudaEventRecord(ev[1], stream);
     if (!binned && (hitmap || counters)) {
         const uint64_t bb = (n + 255) / 256;
-        const unsigned grid = (unsigned)(bb < 148ull * 8 ? bb : 148ull * 8);
+        int sm_count = 0;
+        if (opx_status st = configure_device(&sm_count)) return st;
+        const unsigned grid = (unsigned)(bb < (uint64_t)sm_count * 8 ? bb : (uint64_t)sm_count * 8);
         k_bin<<<grid, 256, 0, stream>>>(out.state, out.bounces, out.pixel, n, (const unsigned long long*)d_n, hitmap, (unsigned long long*)counters);
         count_launch(1);
     }
@@ -113,8 +121,9 @@ opx_status launch_propagate(const SceneHost& s, WalkMode mode, uint64_t n, const
 // per tile of the smallest tile size, and a staging list of `capacity` entries.
 struct DetWorkspace { unsigned long long* count; ulonglong2* table; unsigned long long* src; DetOut stage; size_t bytes; };
 static DetWorkspace det_workspace(void* ws, uint64_t n, uint64_t capacity) {
-    uint64_t tiles = (n + Small::kTile - 1) / Small::kTile + 1;      // the smallest fixed tile size ...
-    if (tiles < kSMs + 1) tiles = kSMs + 1;                         // ... and the single-wave shape's at most 148 tiles
+    // the smallest fixed tile size bounds the tile count of every shape: the single-wave shape runs only where it makes tiles
+    // of more than Small::kTile photons (n > SMs x Small::kTile dealt out over SMs tiles)
+    const uint64_t tiles = (n + Small::kTile - 1) / Small::kTile + 1;
     char* p = (char*)ws;
     auto take = [&](size_t bytes) { char* r = p; p += align_up(bytes, 256); return r; };
     DetWorkspace w{};
