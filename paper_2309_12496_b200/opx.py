@@ -230,8 +230,7 @@ class Scene:
         _check(lib.opx_scene_info(self._h, C.byref(nt), C.byref(nn), C.byref(npix), C.byref(ns)))
         self.n_triangles, self.n_nodes, self.n_pixels, self.n_surfaces = nt.value, nn.value, npix.value, ns.value
         self.workspace = None
-        self._host_ws = None
-        self._det_ws = None
+        self._ws = {}       # cached device workspaces, one per (kind, device, stream): see _workspace()
 
     def __del__(self):
         if getattr(self, "_h", None) and _lib is not None:
@@ -322,6 +321,23 @@ class Scene:
                     dir=torch.empty((capacity, 3), dtype=torch.float32, device=device),
                     n_detected=torch.zeros(1, dtype=torch.int64, device=device))
 
+    def _workspace(self, kind, nbytes, device, stream):
+        """Cached scratch tensor of at least nbytes + 256 bytes for calls of `kind` on `device` and `stream`.  Calls on
+        different streams or devices never share one (they could run at the same time); `stream` None is for the
+        host-buffer calls, which synchronise before they return.  A buffer that has to grow is handed back to torch's
+        allocator only after the work already queued on its stream (record_stream)."""
+        import torch
+        device = torch.device(device)
+        if device.index is None:
+            device = torch.device("cuda", torch.cuda.current_device())
+        key = (kind, device.index, None if stream is None else int(stream.cuda_stream))
+        ws = self._ws.get(key)
+        if ws is None or ws.numel() < nbytes + 256:
+            if ws is not None and stream is not None:
+                ws.record_stream(stream)
+            ws = self._ws[key] = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
+        return ws
+
     def propagate_detected(self, origins, dirs, wavelengths, seed=0, photon_id_base=0, capacity=None, out=None, hitmap=None,
                            counters=None, stream=None, flags=0, n_dev=None, index=None):
         """opx_propagate_detected: the DETECTED photons appended to `out` (alloc_detected) in photon-id order; out["n_detected"]
@@ -339,13 +355,12 @@ class Scene:
         lib = load_library()
         need = C.c_size_t()
         _check(lib.opx_propagate_detected_workspace_bytes(n, cap, C.byref(need)))
-        if self._det_ws is None or self._det_ws.numel() < need.value + 256 or self._det_ws.device != dev:
-            self._det_ws = torch.empty(need.value + 256, dtype=torch.uint8, device=dev)
         d = Detected(*(out[k].data_ptr() for k in ("id", "pixel", "pos", "dir")))
         st = stream if stream is not None else torch.cuda.current_stream(dev)
+        ws = self._workspace("detected", need.value, dev, st)
         _check(lib.opx_propagate_detected(self._h, n, None if n_dev is None else n_dev.data_ptr(), int(photon_id_base),
                                           origins.data_ptr(), dirs.data_ptr(), wavelengths.data_ptr(), int(seed), int(flags),
-                                          None if index is None else index.data_ptr(), C.byref(d), cap, out["n_detected"].data_ptr(), _aligned(self._det_ws), need.value,
+                                          None if index is None else index.data_ptr(), C.byref(d), cap, out["n_detected"].data_ptr(), _aligned(ws), need.value,
                                           hitmap.data_ptr(), counters.data_ptr(), C.c_void_p(st.cuda_stream)))
         res = dict(out)
         res["hitmap"], res["counters"] = hitmap[:self.n_pixels], counters
@@ -363,15 +378,14 @@ class Scene:
         cap = int(out["id"].shape[0])
         need = C.c_size_t()
         _check(lib.opx_propagate_host_detected_workspace_bytes(self._h, chunk, cap, C.byref(need)))
-        if self._host_ws is None or self._host_ws.numel() < need.value + 256:
-            self._host_ws = torch.empty(need.value + 256, dtype=torch.uint8, device=device)
+        ws = self._workspace("host", need.value, torch.device(device), None)
         ptr = (lambda t: t.data_ptr()) if isinstance(wavelengths, torch.Tensor) else (lambda a: a.ctypes.data)
         d = Detected(*(out[k].data_ptr() for k in ("id", "pixel", "pos", "dir")))
         nd = C.c_uint64(0)
         st = stream if stream is not None else torch.cuda.current_stream(device)
         _check(lib.opx_propagate_host_detected(self._h, n, int(photon_id_base), ptr(origins), ptr(dirs), ptr(wavelengths), int(seed),
                                                int(flags), C.byref(d), cap, C.byref(nd), out["hitmap"].data_ptr(),
-                                               out["counters"].data_ptr(), _aligned(self._host_ws), need.value, chunk,
+                                               out["counters"].data_ptr(), _aligned(ws), need.value, chunk,
                                                C.c_void_p(st.cuda_stream)))
         out["n_detected"] = int(nd.value)
         return out
@@ -394,15 +408,14 @@ class Scene:
         cap = int(out["id"].shape[0])
         need = C.c_size_t()
         _check(lib.opx_tracks_host_detected_workspace_bytes(self._h, S, chunk, cap, C.byref(need)))
-        if self._host_ws is None or self._host_ws.numel() < need.value + 256:
-            self._host_ws = torch.empty(need.value + 256, dtype=torch.uint8, device=device)
+        ws = self._workspace("host", need.value, torch.device(device), None)
         fac = (C.c_uint32 * max(1, len(factors)))(*factors)
         d = Detected(*(out[k].data_ptr() for k in ("id", "pixel", "pos", "dir")))
         nd = C.c_uint64(0)
         st = stream if stream is not None else torch.cuda.current_stream(device)
         _check(lib.opx_tracks_host_detected(self._h, C.byref(ts), int(first[-1]), n_index, lambda1, lambda2, int(n), int(photon_id_base),
                                             int(seed), fac, len(factors), C.byref(d), cap, C.byref(nd), out["hitmap"].data_ptr(),
-                                            out["counters"].data_ptr(), _aligned(self._host_ws), need.value, chunk,
+                                            out["counters"].data_ptr(), _aligned(ws), need.value, chunk,
                                             C.c_void_p(st.cuda_stream)))
         out["n_detected"] = int(nd.value)
         return out
@@ -544,8 +557,7 @@ class Scene:
         chunk = max(1, min(int(chunk), max(n, 1)))
         need = C.c_size_t()
         _check(lib.opx_propagate_host_workspace_bytes(self._h, chunk, C.byref(need)))
-        if self._host_ws is None or self._host_ws.numel() < need.value + 256:
-            self._host_ws = torch.empty(need.value + 256, dtype=torch.uint8, device=device)
+        ws = self._workspace("host", need.value, torch.device(device), None)
         if out is None:
             out = alloc_host_records(n, self.n_pixels)
         ptr = (lambda t: t.data_ptr()) if isinstance(wavelengths, torch.Tensor) else (lambda a: a.ctypes.data)
@@ -553,7 +565,7 @@ class Scene:
         st = stream if stream is not None else torch.cuda.current_stream(device)
         _check(lib.opx_propagate_host(self._h, n, int(photon_id_base), ptr(origins), ptr(dirs), ptr(wavelengths),
                                       int(seed), C.byref(h), out["hitmap"].data_ptr(), out["counters"].data_ptr(),
-                                      _aligned(self._host_ws), need.value, chunk, C.c_void_p(st.cuda_stream)))
+                                      _aligned(ws), need.value, chunk, C.c_void_p(st.cuda_stream)))
         return out
 
 
