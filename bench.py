@@ -33,7 +33,16 @@ UNIT = "photons/s"
 # FLOP model of SURVEY.md 8(d) / DESIGN.md 9: FMA = 2, add/mul/min/max/compare/divide = 1
 FLOP_NODE, FLOP_TRI, FLOP_SEGMENT, FLOP_INTERACTION = 48, 50, 15, 35
 BYTES_IN, BYTES_OUT = 28, 34                        # per photon: inputs, hit record
-L2_BYTES = 126e6
+L2_BYTES = 126e6                                    # replaced by the device's own L2 size in main() (device_constants)
+N_SMS = 148                                         # likewise: the device's SM count
+
+
+def device_constants(torch, dev):
+    """L2 size and SM count of the device the bench runs on (they decide how small configs are timed and the derived peak)."""
+    global L2_BYTES, N_SMS
+    prop = torch.cuda.get_device_properties(dev)
+    L2_BYTES = float(getattr(prop, "L2_cache_size", 0) or L2_BYTES)
+    N_SMS = int(prop.multi_processor_count)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the step's kernel, from the `ncu --set full` captures
 # summarised under profiles/ (per config, at the launch size this bench times; None until a capture exists)
 NCU_TRAFFIC_BYTES = {"C2": (565296128, 10_000_000), "C4": (6683452000, 100_000_000)}      # (bytes, photons of the captured launch)
@@ -188,7 +197,7 @@ class Timed:
         return sum(a.elapsed_time(b) for a, b in evs)
 
 
-def roofline_record(pkg, scene, photons, n, id_base, seed, kernel_ms, step_ms, peaks, fma_peak, config):
+def roofline_record(pkg, scene, photons, n, id_base, seed, kernel_ms, step_ms, peaks, fma_peak, config, kernel_ms_all=None):
     """algorithmic FLOPs (instrumented single-ray walk: segments, node visits, triangle tests,
     interactions) and bytes (62 B/photon) of one launch over the kernel's measured duration; the slower bound is named."""
     d_o, d_d, d_l = photons
@@ -196,7 +205,7 @@ def roofline_record(pkg, scene, photons, n, id_base, seed, kernel_ms, step_ms, p
     flop = (FLOP_NODE * stats["nodes"] + FLOP_TRI * stats["triangle_tests"] + FLOP_SEGMENT * stats["segments"]
             + FLOP_INTERACTION * stats["interactions"])
     t = kernel_ms * 1e-3
-    derived = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    derived = N_SMS * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
     peak = fma_peak if fma_peak else derived
     alu = flop / t / 1e12
     hbm_bytes = (BYTES_IN + BYTES_OUT) * n
@@ -205,7 +214,7 @@ def roofline_record(pkg, scene, photons, n, id_base, seed, kernel_ms, step_ms, p
     if t_alu >= t_hbm:
         roof = {"bound": "alu", "achieved": alu, "peak": peak, "unit": "TFLOP/s", "frac": alu / peak,
                 "peak_source": "measured (FP32 FMA micro-benchmark opx_measure_fp32_peak on this device)" if fma_peak
-                               else "derived (148 SMs x 128 FP32 lanes x 2 FLOP x sm_max_mhz)"}
+                               else f"derived ({N_SMS} SMs x 128 FP32 lanes x 2 FLOP x sm_max_mhz)"}
     else:
         roof = {"bound": "hbm", "achieved": hbm, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": hbm / peaks["hbm_gbs"],
                 "peak_source": peaks["source"]}
@@ -213,48 +222,22 @@ def roofline_record(pkg, scene, photons, n, id_base, seed, kernel_ms, step_ms, p
         # the capture's bytes, scaled when this launch has another photon count than the captured one (the default sizes match)
         "traffic": (NCU_TRAFFIC_BYTES[config][0] * n // NCU_TRAFFIC_BYTES[config][1]) if config in NCU_TRAFFIC_BYTES else None,
         "traffic_source": NCU_TRAFFIC_SOURCE.get(config),
+        # not a measurement of THIS run: the bytes of an earlier ncu capture (a run under ncu is never a bench run)
+        "traffic_measured_in_run": False,
+        "traffic_scaled_from_capture": bool(config in NCU_TRAFFIC_BYTES and n != NCU_TRAFFIC_BYTES[config][1]),
         "kernel": pkg.last_kernel(), "kernel_ms": kernel_ms, "kernel_share_of_step": kernel_ms / step_ms,
+        # median and best of the per-launch times next to the mean the fractions above use
+        "kernel_ms_median": statistics.median(kernel_ms_all) if kernel_ms_all else None,
+        "kernel_ms_best": min(kernel_ms_all) if kernel_ms_all else None,
+        "kernel_ms_launches": len(kernel_ms_all) if kernel_ms_all else 0,
         "fp32_peak_derived_tflops": derived, "frac_of_derived_peak": alu / derived,
-        "fp32_peak_derivation": "148 SMs x 128 FP32 lanes x 2 FLOP x sm_max_mhz (only the clock is measured)",
+        "fp32_peak_derivation": f"{N_SMS} SMs x 128 FP32 lanes x 2 FLOP x sm_max_mhz (only the clock is measured)",
         "flop_per_photon": flop / n, "bytes_per_photon": BYTES_IN + BYTES_OUT,
         "segments_per_photon": stats["segments"] / n, "nodes_per_segment": stats["nodes"] / max(1, stats["segments"]),
         "triangle_tests_per_segment": stats["triangle_tests"] / max(1, stats["segments"]),
         "alu_tflops": alu, "hbm_gbs": hbm, "hbm_frac": hbm / peaks["hbm_gbs"], "hbm_peak_source": peaks["source"],
         "photons_per_s_alu_bound": n / t_alu, "photons_per_s_hbm_bound": n / t_hbm})
     return roof
-
-
-def measure_in_flight(pkg, torch, tm, scene, photons, n, id_base, seed, steps, warmup, records=None, allreduce=None):
-    """`steps` timed opx_propagate calls over the resident batch.  Returns (total ms, mean kernel ms, launches, counters)."""
-    d_o, d_d, d_l = photons
-    dev = d_l.device
-    records = records if records is not None else scene.alloc_records(n, dev)
-    hitmap, counters = scene.alloc_accumulators(dev)
-
-    def step():
-        hitmap.zero_(); counters.zero_()
-        scene.propagate(d_o, d_d, d_l, seed=seed, photon_id_base=id_base, records=records, hitmap=hitmap,
-                        counters=counters, stream=tm.stream)
-        if allreduce is not None:
-            allreduce(hitmap, counters)                               # the one exchange step (no-op at N = 1)
-    flush = (BYTES_IN + BYTES_OUT) * n <= L2_BYTES
-    for _ in range(warmup):
-        step()
-    scene.profile_begin(steps)
-    l0 = pkg.launch_count()
-    ms_total = tm.run(step, steps, 0, flush_l2=flush)
-    launches = pkg.launch_count() - l0
-    ms_prop, _ = scene.profile_end()
-    return ms_total, statistics.mean(ms_prop), launches, counters.cpu().numpy(), flush, records
-
-
-def steps_for(pkg, torch, tm, scene, photons, n, seed, target_s, lo, hi):
-    """Number of timed steps that makes the timed region about target_s long (probed with 3 calls)."""
-    d_o, d_d, d_l = photons
-    rec = scene.alloc_records(n, d_l.device)
-    hm, ct = scene.alloc_accumulators(d_l.device)
-    ms = tm.run(lambda: scene.propagate(d_o, d_d, d_l, seed=seed, records=rec, hitmap=hm, counters=ct, stream=tm.stream), 3, 2)
-    return int(min(hi, max(lo, target_s / max(1e-6, ms / 3 * 1e-3)))), rec
 
 
 def run_sweep(args, scene, photons, records, hitmap, counters, n, stream, w, pkg):
@@ -355,11 +338,11 @@ def sub_record(pkg, torch, tm, name, dev, seed, peaks, fma_peak, target_s, n=Non
     ms_step = ms_total / steps
     # counters of the last step (batch K-1)
     cnt = counters.cpu().numpy()
-    roof = roofline_record(pkg, scene, batches[(steps - 1) % K][0], n, ((steps - 1) % K) * n, seed, kernel_ms, ms_step, peaks, fma_peak, name)
+    roof = roofline_record(pkg, scene, batches[(steps - 1) % K][0], n, ((steps - 1) % K) * n, seed, kernel_ms, ms_step, peaks, fma_peak, name, ms_prop)
     return {"workload": workload_name(name, w.scene, n), "value": n / (ms_step * 1e-3), "unit": UNIT, "steps": steps,
             "ms_per_step": ms_step, "gpu_launches": int(launches),
             "l2": (f"a stream of calls over {K} distinct resident batches ({K * (BYTES_IN + BYTES_OUT) * n / 1e6:.0f} MB of inputs + outputs, "
-                   f"twice the 126 MB L2): no step finds its photons in L2, the scene stays warm") if K > 1 else "inputs + outputs per step exceed the 126 MB L2",
+                   f"twice the {L2_BYTES / 1e6:.0f} MB L2): no step finds its photons in L2, the scene stays warm") if K > 1 else f"inputs + outputs per step exceed the {L2_BYTES / 1e6:.0f} MB L2",
             "roofline": roof, "states": dict(zip(pkg.STATE_NAMES, (int(x) for x in cnt[:7])))}
 
 
@@ -403,6 +386,7 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    device_constants(torch, dev)
     dist = None
     if world > 1:
         import torch.distributed as dist
@@ -418,7 +402,17 @@ def main():
         from workloads.scenes import toy_rich_scene
         w.scene = toy_rich_scene("flat" if args.config == "C1" else "c2", smooth=True)
     id_base, n = shard_range(n * world, rank, world)                  # contiguous global id range of this rank
-    pin = pinned_photons(w, id_base, n)
+    ranks = [{"rank": rank, "id_base": int(id_base), "photons": int(n), "device": torch.cuda.get_device_name(dev)}]
+    if dist is not None:
+        gathered = [None] * world
+        dist.all_gather_object(gathered, ranks[0])
+        ranks = gathered
+        if rank == 0:      # what a cold N > 1 run is: communicator size and each rank's id range, before anything is timed
+            print(f"[bench] world {world}, NCCL communicator of {dist.get_world_size()} ranks: " +
+                  "; ".join(f"rank {r['rank']} ids [{r['id_base']}, {r['id_base'] + r['photons']})" for r in ranks), file=sys.stderr)
+    # the ranks of one node generate their photons side by side: share the host cores instead of 8 threads each
+    gen_threads = max(1, min(8, (os.cpu_count() or 8) // max(1, world)))
+    pin = pinned_photons(w, id_base, n, threads=gen_threads)
     d_o, d_d, d_l = (x.to(dev, non_blocking=True) for x in pin)
     stream = torch.cuda.current_stream(dev)
     tm = Timed(torch, stream, dev)
@@ -555,7 +549,7 @@ def main():
     peaks = measured_peaks()
     fma = pkg.measure_fp32_peak(dev)          # FMA micro-benchmark on this device
     pkg_kernel = kernel_name
-    roof = roofline_record(pkg, scene, (d_o, d_d, d_l), n, id_base, args.seed, statistics.mean(ms_prop), ms_step, peaks, fma, args.config)
+    roof = roofline_record(pkg, scene, (d_o, d_d, d_l), n, id_base, args.seed, statistics.mean(ms_prop), ms_step, peaks, fma, args.config, ms_prop)
     roof["kernel"] = pkg_kernel
 
     paper = emit = None
@@ -686,9 +680,10 @@ def main():
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": workload_name(args.config, w.scene, n, args.smooth),
-                   "l2": "every step timed on its own after a 256 MB fill that flushes L2" if flush else "inputs + outputs per step exceed the 126 MB L2",
+                   "l2": "every step timed on its own after a 256 MB fill that flushes L2" if flush else f"inputs + outputs per step exceed the {L2_BYTES / 1e6:.0f} MB L2",
                    "photons_per_gpu": n, "triangles": w.scene.n_triangles, "pixels": scene.n_pixels, "seed": args.seed,
-                   "id_partition": "contiguous global photon-id range per rank; scene + BVH replicated"},
+                   "id_partition": "contiguous global photon-id range per rank; scene + BVH replicated",
+                   "ranks": [[r["id_base"], r["photons"]] for r in ranks]},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
         "configs": subs, "paper_pipeline": paper, "emit": emit, "bvh_build_ms": min(t_build), "bvh_build_launches": int(build_launches),
         "states": dict(zip(pkg.STATE_NAMES, (int(x) for x in cnt[:7]))),

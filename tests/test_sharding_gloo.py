@@ -106,3 +106,14 @@ def test_two_rank_emit_filter_trace_chain_reproduces_single_rank(tmp_path):
     assert np.array_equal(np.load(tmp_path / "hitmap.npy").astype(np.uint32), ref["hitmap"])
     assert np.array_equal(np.load(tmp_path / "counters.npy").astype(np.uint64), ref["counters"])
     assert ref["hitmap"].sum() > 100
+
+
+def test_bench_id_ranges_for_two_and_eight_ranks():
+    """bench.py's weak-scaling arithmetic without CUDA: rank r of `world` takes shard_range(n * world, r, world) of a job of
+    n photons per GPU; the ranges are n photons each, contiguous, and tile ids [0, n * world) for world = 2 and 8 (the sizes
+    the driver's scaling run uses) -- also when n is not a multiple of anything."""
+    for world in (2, 8):
+        for n in (100_000_000, 600_000, 12_345_677):
+            spans = [shard_range(n * world, r, world) for r in range(world)]
+            assert [c for _, c in spans] == [n] * world
+            assert [s for s, _ in spans] == [r * n for r in range(world)]
