@@ -362,8 +362,9 @@ opx_status opx_propagate_host_detected(const opx_scene* scene, uint64_t n, uint6
 /* The paper's whole loop, memory-resident (photons are written to a file by Geant4 today, "the rendering
  * loop" should run from memory): track steps in HOST memory in, the list of detected photons in HOST memory out; the photons
  * themselves never exist outside the device.  h_steps holds HOST pointers (opx_track_steps); photons photon_id_base ..
- * photon_id_base + n - 1 of its first[] are generated (opx_emit_cherenkov) and propagated in chunks of `chunk`, the
- * detected ones appended to h_out as in opx_propagate_host_detected.  n_factors = 0: efficiencies drawn in flight
+ * photon_id_base + n - 1 of its first[] are generated (opx_emit_cherenkov) and propagated in chunks of at most `chunk` (the
+ * first few and the last are shorter; the step table goes up slice by slice and the list comes down chunk by chunk on internal
+ * streams while other chunks are traced), the detected ones appended to h_out as in opx_propagate_host_detected.  n_factors = 0: efficiencies drawn in flight
  * (opx_emit_cherenkov then opx_propagate_detected).  n_factors > 0: the paper's own pipeline - the pre-propagation filter
  * on `factors` fused with the emission (opx_emit_cherenkov_filtered), the survivors traced with OPX_FLAG_NO_EFFICIENCY; the
  * list carries the original photon ids either way.  By definition the result is that of those calls.  Moves 40 B per track

@@ -1,5 +1,6 @@
 // C-ABI entry points of libopx.so (include/opx.h): argument validation, scene flattening (A0),
 // workspace accounting, error reporting and the host-buffer streaming form of propagate.
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdio>
@@ -339,6 +340,7 @@ opx_status opx_propagate_detected(const opx_scene* scene, uint64_t n, const uint
 #define OPX_HOST_SLOTS 3
 #endif
 static constexpr int kSlots = OPX_HOST_SLOTS;
+static_assert(kSlots >= 2, "the host-buffer calls alternate between at least two slots / events");
 }  // extern "C"
 
 namespace opx {
@@ -634,20 +636,76 @@ opx_status opx_tracks_host_detected(const opx_scene* scene, const opx_track_step
     uint64_t* d_counters = (uint64_t*)take(128);
     uint64_t* d_n_det = d_counters + 8;
 
+    // The step table goes up in slices on a side stream while the chunks before it are being traced: chunk k's emission needs
+    // only the steps its photon ids fall into (a photon depends on its step's data, not on the step's index, so the kernels get
+    // the slice as a table of its own), and the host knows which those are from first[].  The first kernel starts after the
+    // first slice (a few MB) instead of after the whole table.
+    HostPipe* pipe = nullptr;
+    if (opx_status st0 = host_pipe(*scene, &pipe)) return st0;
+    std::lock_guard<std::mutex> lock(pipe->busy);
+    cudaStream_t up = pipe->st[0];
+    cudaEvent_t slice_up = pipe->done[0];
     cudaError_t err = cudaSuccess;
     auto ck = [&](cudaError_t e) { if (e != cudaSuccess && err == cudaSuccess) err = e; };
-    ck(cudaMemcpyAsync(dx, h_steps->x, S * 12, cudaMemcpyHostToDevice, main));
-    ck(cudaMemcpyAsync(dw, h_steps->w, S * 12, cudaMemcpyHostToDevice, main));
-    ck(cudaMemcpyAsync(dl, h_steps->length, S * 4, cudaMemcpyHostToDevice, main));
-    ck(cudaMemcpyAsync(db, h_steps->beta, S * 4, cudaMemcpyHostToDevice, main));
-    ck(cudaMemcpyAsync(df, h_steps->first, (S + 1) * 8, cudaMemcpyHostToDevice, main));
+    ck(cudaEventRecord(pipe->start, main));                  // the side stream starts after whatever used the workspace before
+    ck(cudaStreamWaitEvent(up, pipe->start, 0));
     ck(cudaMemsetAsync(d_hitmap, 0, scene->n_pixels * 4 + 4, main));
     ck(cudaMemsetAsync(d_counters, 0, 128, main));
-    const opx_track_steps dsteps{dx, dw, dl, db, df, S};
+    const uint64_t* hf = h_steps->first;
+    uint64_t uploaded = 0;                                   // steps [0, uploaded) and first[0 .. uploaded] are on their way
+    bool first_slice = true;
     opx_status st = OPX_OK;
-    for (uint64_t done = 0; done < n && st == OPX_OK && err == cudaSuccess; done += chunk) {
-        const uint64_t m = n - done < chunk ? n - done : chunk;
+    // Chunk sizes: at most `chunk`; the first three are short (2^20, 2^22, 2^24 photons) so that tracing starts after a small
+    // slice of the table, and a long last chunk leaves 2^22 photons to a chunk of their own so that little of the list is
+    // still on the device when the last kernel ends.  Any chunking gives the same list (ids key the random streams).
+    std::vector<uint64_t> sizes;
+    for (uint64_t left = n; left;) {
+        uint64_t c = chunk < left ? chunk : left;
+        if (sizes.size() < 3) c = std::min<uint64_t>(c, 1ull << (20 + 2 * sizes.size()));
+        if (c == left && c > (1ull << 24)) c -= 1ull << 22;
+        sizes.push_back(c);
+        left -= c;
+    }
+    // The list goes down chunk by chunk on a second side stream: once chunk k is queued the host reads the list's length as
+    // chunk k-1 left it (a copy parked in a slot of its own, so that chunk k's scan cannot be seen half-way) and sends the
+    // new entries on their way while chunk k runs.  Entries below `capacity` are never rewritten by a later chunk.
+    cudaStream_t down = pipe->st[1];
+    uint64_t* d_len = d_counters + 9;                        // 4 slots: the list's length after chunk k, k mod 4
+    uint64_t downloaded = 0;
+    auto fetch = [&](uint64_t upto) {
+        const uint64_t hi = upto < capacity ? upto : capacity;
+        if (hi <= downloaded) return;
+        const uint64_t a = downloaded, c = hi - a;
+        ck(cudaMemcpyAsync(h_out->id + a, det.id + a, c * 8, cudaMemcpyDeviceToHost, down));
+        ck(cudaMemcpyAsync(h_out->pixel + a, det.pixel + a, c * 4, cudaMemcpyDeviceToHost, down));
+        ck(cudaMemcpyAsync(h_out->pos + 3 * a, det.pos + 3 * a, c * 12, cudaMemcpyDeviceToHost, down));
+        ck(cudaMemcpyAsync(h_out->dir + 3 * a, det.dir + 3 * a, c * 12, cudaMemcpyDeviceToHost, down));
+        downloaded = hi;
+    };
+    uint64_t done = 0;
+    for (size_t k = 0; k < sizes.size() && st == OPX_OK && err == cudaSuccess; done += sizes[k], ++k) {
+        const uint64_t m = sizes[k];
         const uint64_t base = photon_id_base + done;
+        // steps of this chunk: s_lo = the last step with first[s] <= base, s_hi = the first step with first[s] > base + m - 1
+        const uint64_t s_lo = (uint64_t)(std::upper_bound(hf, hf + S + 1, base) - hf) - 1;
+        uint64_t s_hi = (uint64_t)(std::upper_bound(hf, hf + S + 1, base + m - 1) - hf);
+        if (s_lo >= S || hf[0] > base) { st = fail(OPX_ERR_INVALID_ARG, "first[] does not cover the photon ids (first[0] must be 0, first[n_steps] = n_total)"); break; }
+        if (s_hi > S) s_hi = S;
+        const uint64_t from = first_slice ? s_lo : uploaded;      // a call that starts in the middle of the table skips what lies before
+        if (s_hi > from || first_slice) {
+            const uint64_t cnt_steps = s_hi - from;
+            ck(cudaMemcpyAsync(dx + 3 * from, h_steps->x + 3 * from, cnt_steps * 12, cudaMemcpyHostToDevice, up));
+            ck(cudaMemcpyAsync(dw + 3 * from, h_steps->w + 3 * from, cnt_steps * 12, cudaMemcpyHostToDevice, up));
+            ck(cudaMemcpyAsync(dl + from, h_steps->length + from, cnt_steps * 4, cudaMemcpyHostToDevice, up));
+            ck(cudaMemcpyAsync(db + from, h_steps->beta + from, cnt_steps * 4, cudaMemcpyHostToDevice, up));
+            const uint64_t f0 = first_slice ? from : from + 1;    // first[from] went up with the slice before
+            ck(cudaMemcpyAsync(df + f0, hf + f0, (s_hi + 1 - f0) * 8, cudaMemcpyHostToDevice, up));
+            ck(cudaEventRecord(slice_up, up));
+            ck(cudaStreamWaitEvent(main, slice_up, 0));      // waits for THIS record; the event is recorded again for the next slice
+            uploaded = s_hi;
+            first_slice = false;
+        }
+        const opx_track_steps dsteps{dx + 3 * s_lo, dw + 3 * s_lo, dl + s_lo, db + s_lo, df + s_lo, s_hi - s_lo};
         if (n_factors) {
             st = launch_emit_filtered(*scene, dsteps, n_index, lambda1_nm, lambda2_nm, m, base, seed, factors, n_factors, po, pd, pw, pidx, m,
                                       d_n_kept, pf_ws, main);
@@ -660,6 +718,16 @@ opx_status opx_tracks_host_detected(const opx_scene* scene, const opx_track_step
                 st = launch_propagate_detected(*scene, m, nullptr, base, po, pd, pw, seed, 0u, det, capacity, d_n_det, nullptr, det_ws, d_hitmap,
                                                d_counters, main);
         }
+        if (st != OPX_OK) break;
+        ck(cudaMemcpyAsync(d_len + (k & 3), d_n_det, 8, cudaMemcpyDeviceToDevice, main));
+        ck(cudaEventRecord(pipe->kernel[k % kSlots], main));
+        if (k >= 1) {
+            uint64_t len = 0;
+            ck(cudaStreamWaitEvent(down, pipe->kernel[(k - 1) % kSlots], 0));
+            ck(cudaMemcpyAsync(&len, d_len + ((k - 1) & 3), 8, cudaMemcpyDeviceToHost, down));
+            ck(cudaStreamSynchronize(down));                 // chunk k-1 has ended; chunk k is queued or running
+            if (err == cudaSuccess) fetch(len);
+        }
     }
     std::vector<uint32_t> hm(scene->n_pixels);
     uint64_t cnt[9] = {0};
@@ -667,16 +735,11 @@ opx_status opx_tracks_host_detected(const opx_scene* scene, const opx_track_step
     ck(cudaMemcpyAsync(cnt, d_counters, 72, cudaMemcpyDeviceToHost, main));
     ck(cudaStreamSynchronize(main));
     if (st == OPX_OK && err == cudaSuccess) {
-        const uint64_t have = cnt[8] < capacity ? cnt[8] : capacity;
-        if (have) {
-            ck(cudaMemcpyAsync(h_out->id, det.id, have * 8, cudaMemcpyDeviceToHost, main));
-            ck(cudaMemcpyAsync(h_out->pixel, det.pixel, have * 4, cudaMemcpyDeviceToHost, main));
-            ck(cudaMemcpyAsync(h_out->pos, det.pos, have * 12, cudaMemcpyDeviceToHost, main));
-            ck(cudaMemcpyAsync(h_out->dir, det.dir, have * 12, cudaMemcpyDeviceToHost, main));
-            ck(cudaStreamSynchronize(main));
-        }
+        fetch(cnt[8]);                                       // what the last chunk added
         *h_n_detected = cnt[8];
     }
+    ck(cudaStreamSynchronize(down));                         // the side streams are idle when the call returns, whatever happened
+    ck(cudaStreamSynchronize(up));
     if (st != OPX_OK) return st;
     if (err != cudaSuccess) return check_cuda(err, "opx_tracks_host_detected");
     for (uint64_t i = 0; i < scene->n_pixels; ++i) h_hitmap[i] += hm[i];

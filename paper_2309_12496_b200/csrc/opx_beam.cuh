@@ -36,6 +36,9 @@ constexpr int kCullMin = OPX_CULL_MIN;   // per-lane cull when the beam enters a
 #define OPX_CULL_SLOTS 16
 #endif
 constexpr int kCullSlots = OPX_CULL_SLOTS;   // candidate boxes a warp stages in shared memory per culling round
+#ifndef OPX_RECULL
+#define OPX_RECULL 0                          // 1: per-lane candidates nearest-first, re-tested against the current best hit
+#endif
 
 struct Beam {
     // entry bound of axis a: fma(near_a, rn_a, cn_a); exit bound: fma(far_a, rf_a, cf_a), where
@@ -212,6 +215,10 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayR&
                     __syncwarp();
                     const float cap = alive ? h.t : -1.f;
                     unsigned mine = 0u;                  // the candidates (slots) this lane still has to test
+#if OPX_RECULL
+                    float near_en = kInf;                // the candidate whose box this lane's ray enters first
+                    int near_c = 0;
+#endif
 #pragma unroll
                     for (int c = 0; c < kCullSlots; ++c) {       // unrolled: slot addresses and mask bits are immediates
                         if (c >= cnt) break;
@@ -219,8 +226,36 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayR&
                         const float e0 = __fmaf_rn(n4.x, ix, qx), e1 = __fmaf_rn(n4.y, iy, qy), e2 = __fmaf_rn(n4.z, iz, qz);
                         const float x0 = __fmaf_rn(f4.x, ix, qx), x1 = __fmaf_rn(f4.y, iy, qy), x2 = __fmaf_rn(f4.z, iz, qz);
                         const float en = fmaxf(fmaxf(e0, e1), fmaxf(e2, 0.f)), exi = fminf(fminf(x0, x1), fminf(x2, cap));
-                        if (en <= exi && ~__float_as_int(n4.w) != last_j) mine |= 1u << c;
+                        if (en <= exi && ~__float_as_int(n4.w) != last_j) {
+                            mine |= 1u << c;
+#if OPX_RECULL
+                            if (en < near_en) { near_en = en; near_c = c; }
+#endif
+                        }
                     }
+#if OPX_RECULL
+                    // Nearest box first, and every later candidate is tested against the lane's CURRENT best hit before its
+                    // triangle is fetched: a hit on the facet in front (a mirror) drops the candidates whose boxes begin
+                    // behind it (its backing plate).  The box test is the cull's own (entry bound <= best t, ties kept), so
+                    // the surviving set still holds every triangle that could win.  The warp iterates while ANY lane has a
+                    // candidate left: lanes skip their pruned candidates without spending an iteration of the warp on them.
+                    unsigned tested = 0u, t_iter = 0u;
+                    int c = near_c;
+                    for (;;) {
+                        int j = -1;
+                        while (mine) {
+                            mine &= ~(1u << c);
+                            const float4 n4 = s_cb[c];
+                            const float en = fmaxf(fmaxf(__fmaf_rn(n4.x, ix, qx), __fmaf_rn(n4.y, iy, qy)), __fmaf_rn(n4.z, iz, qz));
+                            c = __ffs(mine) - 1;
+                            if (en <= h.t) { j = ~__float_as_int(n4.w); break; }
+                        }
+                        if (!__any_sync(full, j >= 0)) break;
+                        if (kStats) { ++t_iter; tested += j >= 0; }
+                        if (j >= 0) consider_rot(sc, rr, j, tmin, last_j, h);
+                    }
+                    if (kStats) { stats.pairs += __reduce_add_sync(full, tested); stats.tris += t_iter; }
+#else
                     if (kStats) {
                         stats.pairs += __reduce_add_sync(full, (unsigned)__popc(mine));
                         stats.tris += __reduce_max_sync(full, (unsigned)__popc(mine));
@@ -230,6 +265,7 @@ __device__ __forceinline__ bool closest_hit_beam(const SceneDev& sc, const RayR&
                         mine &= mine - 1u;
                         consider_rot(sc, rr, ~__float_as_int(s_cb[c].w), tmin, last_j, h);
                     }
+#endif
                     __syncwarp();
                 } while (rem);
             }
