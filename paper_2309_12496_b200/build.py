@@ -26,10 +26,13 @@ def _deps():
 
 
 def build(force=False, verbose=False):
+    """OPX_NVCC_FLAGS (environment, optional): extra nvcc flags, e.g. the -D switches of the measured-and-rejected
+    variants that profiles/ names (a build with them is for measuring, not the product; it always rebuilds)."""
     os.makedirs(LIBDIR, exist_ok=True)
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
+    extra = os.environ.get("OPX_NVCC_FLAGS", "").split()
+    if not force and not extra and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
         return LIB
-    cmd = [NVCC, *FLAGS, *(["-Xptxas", "-v"] if verbose else []), *sources(), "-o", LIB + ".tmp"]
+    cmd = [NVCC, *FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), *sources(), "-o", LIB + ".tmp"]
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)
     return LIB
