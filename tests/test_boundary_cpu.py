@@ -138,3 +138,15 @@ def test_bench_reference_arm_prints_one_json_line():
     assert line["impl"] == "reference" and line["unit"] == "photons/s" and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["gpu_launches"] == 0
+
+
+def test_prefilter_noalloc_checks_its_arguments_before_touching_a_device(lib):
+    """opx_prefilter_noalloc (the filter for callers that cannot allocate device memory) validates like opx_prefilter:
+    a NULL scene and a scene that was never built are refused on the host, with no CUDA call made."""
+    args = (0, 0, None, None, None, 0, None, 0, None, None, None, None, 0, None, None)
+    assert lib.opx_prefilter_noalloc(None, *args) == opx.OPX_ERR_INVALID_ARG and b"scene is NULL" in lib.opx_last_error()
+    s = pkg.Scene(wl.toy_rich_scene(cells=4))
+    assert lib.opx_prefilter_noalloc(s._h, *args) == opx.OPX_ERR_BAD_STATE
+    assert b"opx_prefilter_noalloc before opx_bvh_build" in lib.opx_last_error()
+    header = open(os.path.join(ROOT, "include", "opx.h")).read()
+    assert f"#define OPX_PREFILTER_NOALLOC_MAX_PHOTONS {opx.PREFILTER_NOALLOC_MAX_PHOTONS}ull" in header
